@@ -1,0 +1,110 @@
+"""ctypes loader for oracle.c (TEST INFRASTRUCTURE -- see oracle/__init__.py)."""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def lib_path():
+    return _LIB
+
+
+def build(force=False):
+    """Compile oracle.c with gcc (plain C11, no CUDA)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    tmp = _LIB + f".tmp{os.getpid()}"
+    subprocess.check_call(["gcc", "-std=c11", "-O2", "-Wall", "-Wextra", "-shared", "-fPIC",
+                           _SRC, "-o", tmp])
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+        L.oracle_rank_partition.argtypes = [i32, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        L.oracle_rank_partition.restype = C.c_int
+        L.oracle_bruteforce_partition.argtypes = [i32, vp, vp, i64, i64, vp, vp, vp]
+        L.oracle_bruteforce_partition.restype = C.c_int
+        for f in (L.oracle_demote, L.oracle_promote):
+            f.argtypes = [i32, i64, vp, i64, vp, i64, i64, vp, vp]
+            f.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def rank_partition(iota, s, prev_tier, cap_gpu, cap_cpu):
+    """oracle_rank_partition -> dict(order, tier, bounds, used, lists (list of 5 arrays))."""
+    iota = np.ascontiguousarray(iota, dtype=np.float32)
+    s = np.ascontiguousarray(s, dtype=np.int32)
+    n = int(iota.shape[0])
+    assert s.shape == (n,)
+    prev = None if prev_tier is None else np.ascontiguousarray(prev_tier, dtype=np.uint8)
+    order = np.empty(n, np.int32)
+    tier = np.empty(n, np.uint8)
+    bounds = np.zeros(2, np.int32)
+    used = np.zeros(2, np.int64)
+    lists = np.full((5, max(n, 1)), -1, np.int32)[:, :n].copy() if n else np.zeros((5, 0), np.int32)
+    counts = np.zeros(5, np.int32)
+    rc = _load().oracle_rank_partition(n, _p(iota), _p(s), _p(prev), int(cap_gpu), int(cap_cpu),
+                                       _p(order), _p(tier), _p(bounds), _p(used),
+                                       _p(lists) if prev is not None else None,
+                                       _p(counts) if prev is not None else None)
+    if rc != 0:
+        raise ValueError(f"oracle_rank_partition: bad argument (rc={rc})")
+    out = dict(order=order, tier=tier, bounds=bounds, used=used)
+    if prev is not None:
+        out["lists"] = [lists[k, :counts[k]].copy() for k in range(5)]
+    return out
+
+
+def bruteforce_partition(iota, s, cap_gpu, cap_cpu):
+    iota = np.ascontiguousarray(iota, dtype=np.float32)
+    s = np.ascontiguousarray(s, dtype=np.int32)
+    n = int(iota.shape[0])
+    tier = np.zeros(max(n, 1), np.uint8)
+    bounds = np.zeros(2, np.int32)
+    nbest = C.c_int32(0)
+    rc = _load().oracle_bruteforce_partition(n, _p(iota), _p(s), int(cap_gpu), int(cap_cpu),
+                                             _p(tier), _p(bounds), C.byref(nbest))
+    if rc != 0:
+        raise ValueError(f"oracle_bruteforce_partition: bad argument (rc={rc})")
+    return dict(tier=tier[:n], bounds=bounds, n_best=int(nbest.value))
+
+
+def _move(fn, n_layers, chunk, pool, arena, a, b):
+    assert pool.dtype == np.uint8 and arena.dtype == np.uint8
+    assert pool.flags.c_contiguous and arena.flags.c_contiguous
+    page_bytes = n_layers * chunk
+    assert pool.size % page_bytes == 0 and arena.size % page_bytes == 0
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    b = np.ascontiguousarray(b, dtype=np.int32)
+    assert a.shape == b.shape
+    rc = fn(n_layers, chunk, _p(pool), pool.size // page_bytes, _p(arena),
+            arena.size // page_bytes, a.size, _p(a), _p(b))
+    if rc != 0:
+        raise ValueError(f"oracle mover: bad argument (rc={rc})")
+
+
+def demote(n_layers, chunk, pool, arena, gpu_pages, host_slots):
+    """pool (flat uint8 [L][P][chunk]) -> arena (flat uint8 [S][L][chunk]), in place."""
+    _move(_load().oracle_demote, n_layers, chunk, pool, arena, gpu_pages, host_slots)
+
+
+def promote(n_layers, chunk, pool, arena, host_slots, gpu_pages):
+    _move(_load().oracle_promote, n_layers, chunk, pool, arena, host_slots, gpu_pages)

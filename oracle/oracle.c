@@ -1,0 +1,217 @@
+/*
+ * oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded CPU statement of what the MORI hot path computes
+ * (arxiv/paper_2606_00866; citations "P:Lnnn" are lines of /root/reference/PAPER.md).
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may load this.  It shares no source, header, helper or table with
+ * paper_2606_00866_b200/csrc/ and never includes include/mori.h.
+ *
+ * The method reaches a plainly defined result (a capacity-constrained split of a sorted list,
+ * and a byte permutation), so each function below is that definition written out:
+ *
+ *   oracle_rank_partition      P:L11, L45, L149-152 (rank by relative idleness, busiest -> GPU),
+ *                              P:L176-177 (capacity invariants of both tiers),
+ *                              P:L147, L178 (admission control; overflow -> Waiting, discarded),
+ *                              P:L351 ("filling from the busiest end of the ranking until local
+ *                              capacity is reached"), P:L206/L208 (order of the move lists).
+ *   oracle_bruteforce_partition  the same result stated WITHOUT a sort or a prefix sum:
+ *                              enumeration of all 3^n tier maps (pins the function above).
+ *   oracle_demote / oracle_promote   P:L177 ("offloaded to CPU DRAM"), P:L182 ("CPU-to-GPU
+ *                              transfer"), P:L184 (reload restores the cache): per-(page, layer)
+ *                              memcpy between a paged pool and a page-major arena.
+ *
+ * Readings of the paper adopted where it is silent are listed in DESIGN.md section 3 (R1..R14);
+ * the ones that matter here are repeated next to the code.
+ *
+ * Pins (tests/test_oracle_pins.py): brute force on n <= 9, numpy stable argsort / cumsum /
+ * searchsorted restatement, closed forms (equal sizes, zero and infinite capacity), the
+ * ordering / capacity / maximality invariants, list set identities, and for the movers the
+ * numpy fancy-index gather and the demote->promote round trip.
+ */
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORACLE_OK 0
+#define ORACLE_ERR_ARG (-1)
+
+enum { TIER_GPU = 0, TIER_CPU = 1, TIER_WAIT = 2 };
+
+/* Total order on programs (R1, R2, R11, R12):
+ *   a before b  iff  iota_a < iota_b, or they compare equal as floats (so -0 == +0) and a < b.
+ *   NaN is greater than every non-NaN; NaNs tie among themselves (then by index).
+ * Rank 0 is the LEAST idle (busiest) program: it is the first to get GPU HBM. */
+typedef struct { float iota; int32_t idx; } prog_key;
+
+static int is_nan_f(float x) { return x != x; }
+
+static int before(const prog_key *a, const prog_key *b) {
+  int na = is_nan_f(a->iota), nb = is_nan_f(b->iota);
+  if (na != nb) return nb;              /* the non-NaN one comes first */
+  if (!na) {
+    if (a->iota < b->iota) return 1;
+    if (b->iota < a->iota) return 0;
+  }
+  return a->idx < b->idx;
+}
+
+static int cmp_keys(const void *pa, const void *pb) {
+  const prog_key *a = (const prog_key *)pa, *b = (const prog_key *)pb;
+  if (before(a, b)) return -1;
+  if (before(b, a)) return 1;
+  return 0;                              /* only for a == b: the order is total */
+}
+
+/*
+ * Placement.  Inputs: iota[n] (any float), s[n] (KV footprint in pages, >= 0), prev_tier[n] or
+ * NULL, capacities in pages (>= 0).  Outputs (each may be NULL except order/tier):
+ *   order[r]      program at rank r
+ *   tier[p]       0 GPU, 1 CPU, 2 WAIT, indexed by program
+ *   bounds[2]     b_gpu, b_cpu: GPU tier = ranks [0,b_gpu), CPU tier = ranks [b_gpu,b_cpu)
+ *   used[2]       pages held by the GPU tier and by the CPU tier
+ *   lists[5*n]    row 0 demote  (prev GPU -> CPU)  most idle first  ("highest idleness first")
+ *                 row 1 promote (prev CPU -> GPU)  least idle first ("lowest idleness first")
+ *                 row 2 drop    (prev GPU|CPU -> WAIT) most idle first
+ *                 row 3 admit   (prev WAIT -> GPU) least idle first
+ *                 row 4 reserve (prev WAIT -> CPU) least idle first
+ *   counts[5]     lengths of the rows.  prev_tier values other than 0 and 1 mean WAIT.
+ */
+int oracle_rank_partition(int32_t n, const float *iota, const int32_t *s, const uint8_t *prev_tier,
+                          int64_t cap_gpu, int64_t cap_cpu, int32_t *order, uint8_t *tier,
+                          int32_t *bounds, int64_t *used, int32_t *lists, int32_t *counts) {
+  if (n < 0 || cap_gpu < 0 || cap_cpu < 0) return ORACLE_ERR_ARG;
+  if (n > 0 && (!iota || !s || !order || !tier)) return ORACLE_ERR_ARG;
+  for (int32_t p = 0; p < n; ++p) if (s[p] < 0) return ORACLE_ERR_ARG;
+
+  /* step 1: sort by the total order (library routine; the comparator is total, so no
+   * stability is needed) */
+  prog_key *keys = (prog_key *)malloc(sizeof(prog_key) * (size_t)(n > 0 ? n : 1));
+  if (!keys) return ORACLE_ERR_ARG;
+  for (int32_t p = 0; p < n; ++p) { keys[p].iota = iota[p]; keys[p].idx = p; }
+  qsort(keys, (size_t)n, sizeof(prog_key), cmp_keys);
+  for (int32_t r = 0; r < n; ++r) order[r] = keys[r].idx;
+  free(keys);
+
+  /* step 2: GPU tier = the longest prefix of the ranking whose footprint does not exceed the
+   * GPU capacity ("does not exceed" -> <=; P:L351 stop at the first that does not fit) */
+  int32_t b_gpu = 0; int64_t sum_gpu = 0;
+  while (b_gpu < n && sum_gpu + s[order[b_gpu]] <= cap_gpu) { sum_gpu += s[order[b_gpu]]; ++b_gpu; }
+
+  /* step 3: CPU tier = the longest run after it that fits the CPU capacity ("enforced
+   * analogously"; "CPU queue if CPU capacity permits, or to the Waiting queue otherwise") */
+  int32_t b_cpu = b_gpu; int64_t sum_cpu = 0;
+  while (b_cpu < n && sum_cpu + s[order[b_cpu]] <= cap_cpu) { sum_cpu += s[order[b_cpu]]; ++b_cpu; }
+
+  /* step 4: the rest is not admitted anywhere */
+  for (int32_t r = 0; r < n; ++r)
+    tier[order[r]] = (uint8_t)(r < b_gpu ? TIER_GPU : (r < b_cpu ? TIER_CPU : TIER_WAIT));
+
+  if (bounds) { bounds[0] = b_gpu; bounds[1] = b_cpu; }
+  if (used) { used[0] = sum_gpu; used[1] = sum_cpu; }
+
+  /* step 5: transition lists */
+  if (prev_tier && lists && counts) {
+    for (int k = 0; k < 5; ++k) counts[k] = 0;
+    /* ascending rank = least idle first */
+    for (int32_t r = 0; r < n; ++r) {
+      int32_t p = order[r];
+      int was = prev_tier[p] == 0 ? TIER_GPU : (prev_tier[p] == 1 ? TIER_CPU : TIER_WAIT);
+      int now = tier[p];
+      if (was == TIER_CPU && now == TIER_GPU) lists[1 * (size_t)n + counts[1]++] = p;
+      if (was == TIER_WAIT && now == TIER_GPU) lists[3 * (size_t)n + counts[3]++] = p;
+      if (was == TIER_WAIT && now == TIER_CPU) lists[4 * (size_t)n + counts[4]++] = p;
+    }
+    /* descending rank = most idle first */
+    for (int32_t r = n - 1; r >= 0; --r) {
+      int32_t p = order[r];
+      int was = prev_tier[p] == 0 ? TIER_GPU : (prev_tier[p] == 1 ? TIER_CPU : TIER_WAIT);
+      int now = tier[p];
+      if (was == TIER_GPU && now == TIER_CPU) lists[0 * (size_t)n + counts[0]++] = p;
+      if (was != TIER_WAIT && now == TIER_WAIT) lists[2 * (size_t)n + counts[2]++] = p;
+    }
+  }
+  return ORACLE_OK;
+}
+
+/*
+ * The same placement with no sort and no prefix sum (n <= 12).  Enumerate every map
+ * t: programs -> {GPU, CPU, WAIT}; keep those with
+ *   (i)   sum of s over t = GPU  <= cap_gpu
+ *   (ii)  sum of s over t = CPU  <= cap_cpu
+ *   (iii) t(a) < t(b)  =>  a is before b in the total order              (every
+ *         GPU-tier program is busier than every CPU-tier program, and so on down)
+ * and return the one that maximises (|GPU tier|, then |CPU tier|) -- "filling each tier to
+ * capacity".  *n_best receives how many maps attain the maximum (must be 1).
+ */
+int oracle_bruteforce_partition(int32_t n, const float *iota, const int32_t *s, int64_t cap_gpu,
+                                int64_t cap_cpu, uint8_t *tier, int32_t *bounds, int32_t *n_best) {
+  if (n < 0 || n > 12 || cap_gpu < 0 || cap_cpu < 0) return ORACLE_ERR_ARG;
+  long total = 1;
+  for (int i = 0; i < n; ++i) total *= 3;
+  int best_g = -1, best_c = -1, ties = 0;
+  uint8_t t[12], best_t[12];
+  memset(best_t, 0, sizeof best_t);
+  for (long code = 0; code < total; ++code) {
+    long c = code; int64_t sg = 0, sc = 0; int ng = 0, nc = 0;
+    for (int p = 0; p < n; ++p) {
+      t[p] = (uint8_t)(c % 3); c /= 3;
+      if (t[p] == TIER_GPU) { sg += s[p]; ++ng; }
+      if (t[p] == TIER_CPU) { sc += s[p]; ++nc; }
+    }
+    if (sg > cap_gpu || sc > cap_cpu) continue;
+    int ok = 1;
+    for (int a = 0; a < n && ok; ++a)
+      for (int b = 0; b < n; ++b)
+        if (t[a] < t[b]) {
+          prog_key ka = { iota[a], a }, kb = { iota[b], b };
+          if (!before(&ka, &kb)) { ok = 0; break; }
+        }
+    if (!ok) continue;
+    if (ng > best_g || (ng == best_g && nc > best_c)) {
+      best_g = ng; best_c = nc; ties = 1; memcpy(best_t, t, sizeof t);
+    } else if (ng == best_g && nc == best_c) {
+      ++ties;
+    }
+  }
+  for (int p = 0; p < n; ++p) tier[p] = best_t[p];
+  if (bounds) { bounds[0] = best_g; bounds[1] = best_g + best_c; }
+  if (n_best) *n_best = ties;
+  return ORACLE_OK;
+}
+
+/*
+ * KV movement.  chunk = 2 (K,V) * kv_heads * page_tokens * head_dim * elem_bytes is the
+ * contiguous run of one (layer, physical page) in the device pool, whose layout is
+ * [layers][pool_pages][K/V][kv_heads][page_tokens][head_dim] (BASELINE.json north_star; the
+ * paper only says the cache is paged).  The host arena is page-major:
+ * [slots][layers][K/V][kv_heads][page_tokens][head_dim] (R7).
+ *   pool  address of (layer l, page g)  = pool  + (l * pool_pages + g) * chunk
+ *   arena address of (slot h, layer l)  = arena + (h * n_layers  + l) * chunk
+ * Whole pages always move, all layers, K and V ("exactly one tier"; R8).
+ */
+int oracle_demote(int32_t n_layers, int64_t chunk, const uint8_t *pool, int64_t pool_pages,
+                  uint8_t *arena, int64_t arena_slots, int64_t total_pages,
+                  const int32_t *gpu_pages, const int32_t *host_slots) {
+  if (n_layers <= 0 || chunk <= 0 || total_pages < 0) return ORACLE_ERR_ARG;
+  for (int64_t j = 0; j < total_pages; ++j) {
+    int64_t g = gpu_pages[j], h = host_slots[j];
+    if (g < 0 || g >= pool_pages || h < 0 || h >= arena_slots) return ORACLE_ERR_ARG;
+    for (int64_t l = 0; l < n_layers; ++l)
+      memcpy(arena + (h * n_layers + l) * chunk, pool + (l * pool_pages + g) * chunk, (size_t)chunk);
+  }
+  return ORACLE_OK;
+}
+
+int oracle_promote(int32_t n_layers, int64_t chunk, uint8_t *pool, int64_t pool_pages,
+                   const uint8_t *arena, int64_t arena_slots, int64_t total_pages,
+                   const int32_t *host_slots, const int32_t *gpu_pages) {
+  if (n_layers <= 0 || chunk <= 0 || total_pages < 0) return ORACLE_ERR_ARG;
+  for (int64_t j = 0; j < total_pages; ++j) {
+    int64_t g = gpu_pages[j], h = host_slots[j];
+    if (g < 0 || g >= pool_pages || h < 0 || h >= arena_slots) return ORACLE_ERR_ARG;
+    for (int64_t l = 0; l < n_layers; ++l)
+      memcpy(pool + (l * pool_pages + g) * chunk, arena + (h * n_layers + l) * chunk, (size_t)chunk);
+  }
+  return ORACLE_OK;
+}

@@ -1,0 +1,72 @@
+"""numpy restatement of the oracle (TEST INFRASTRUCTURE -- see oracle/__init__.py).
+
+A second, independent statement of the definitions in oracle.c, made of library routines
+(``np.argsort(kind="stable")``, ``np.cumsum``, ``np.searchsorted``, fancy indexing) so that the
+C oracle is pinned to something other than itself.  Citations as in oracle.c.
+"""
+import numpy as np
+
+
+def sort_key(iota):
+    """Canonical float key: -0 -> +0 (float ==, R12); NaN -> +inf bucket after +inf (R11)."""
+    x = np.asarray(iota, dtype=np.float32).astype(np.float64)   # exact widening
+    x = x + 0.0                                                 # -0.0 + 0.0 == +0.0
+    nan = np.isnan(x)
+    return np.where(nan, 0.0, x), nan
+
+
+def rank(iota):
+    """Programs in rank order: ascending idleness, ties by index, NaN last."""
+    x, nan = sort_key(iota)
+    # lexsort: last key is primary.  primary = is-NaN, then value; stable => ties by index.
+    return np.lexsort((x, nan)).astype(np.int32)
+
+
+def rank_partition(iota, s, prev_tier, cap_gpu, cap_cpu):
+    s = np.asarray(s, dtype=np.int64)
+    n = s.shape[0]
+    if (s < 0).any() or cap_gpu < 0 or cap_cpu < 0:
+        raise ValueError("negative size or capacity")
+    order = rank(iota)
+    incl = np.cumsum(s[order])                                  # inclusive prefix sums, int64
+    # largest b with sum_{r<b} s <= C  ==  number of inclusive sums <= C (sums are non-decreasing)
+    b_gpu = int(np.searchsorted(incl, cap_gpu, side="right"))
+    base = int(incl[b_gpu - 1]) if b_gpu > 0 else 0
+    b_cpu = int(np.searchsorted(incl, base + cap_cpu, side="right"))
+    b_cpu = max(b_cpu, b_gpu)
+    tier = np.full(n, 2, np.uint8)
+    tier[order[:b_gpu]] = 0
+    tier[order[b_gpu:b_cpu]] = 1
+    used = np.array([base, (int(incl[b_cpu - 1]) if b_cpu > 0 else 0) - base], np.int64)
+    out = dict(order=order, tier=tier, bounds=np.array([b_gpu, b_cpu], np.int32), used=used)
+    if prev_tier is not None:
+        prev = np.asarray(prev_tier, dtype=np.uint8)
+        prev = np.where(prev > 2, 2, prev)
+        was, now = prev[order], tier[order]
+        asc, desc = order, order[::-1]
+        wa, na, wd, nd = was, now, was[::-1], now[::-1]
+        out["lists"] = [
+            desc[(wd == 0) & (nd == 1)],      # demote, most idle first
+            asc[(wa == 1) & (na == 0)],       # promote, least idle first
+            desc[(wd != 2) & (nd == 2)],      # drop
+            asc[(wa == 2) & (na == 0)],       # admit
+            asc[(wa == 2) & (na == 1)],       # reserve
+        ]
+    return out
+
+
+def demote(n_layers, chunk, pool, arena, gpu_pages, host_slots):
+    """arena[h_j, l] = pool[l, g_j]  for all j, l  (fancy-index statement of oracle_demote)."""
+    pv = pool.reshape(n_layers, -1, chunk)
+    av = arena.reshape(-1, n_layers, chunk)
+    g = np.asarray(gpu_pages, dtype=np.int64)
+    h = np.asarray(host_slots, dtype=np.int64)
+    av[h] = pv[:, g].transpose(1, 0, 2)
+
+
+def promote(n_layers, chunk, pool, arena, host_slots, gpu_pages):
+    pv = pool.reshape(n_layers, -1, chunk)
+    av = arena.reshape(-1, n_layers, chunk)
+    g = np.asarray(gpu_pages, dtype=np.int64)
+    h = np.asarray(host_slots, dtype=np.int64)
+    pv[:, g] = av[h].transpose(1, 0, 2)

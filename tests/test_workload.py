@@ -1,0 +1,166 @@
+"""Host logic: the seeded input generators and the epoch planner (no method arithmetic there),
+and the oracle driven over whole synthetic runs (brute force on every cfg-1 epoch)."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_00866_b200 import workload as W
+from test_oracle_pins import check_invariants, check_lists
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def test_eq1_closed_forms():
+    for line in open(os.path.join(GOLD, "eq1_examples.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        r, a, want = [x.split() for x in line.split("|")]
+        got = W.windowed_idleness(np.array(r, float), np.array(a, float))
+        assert got == np.float32(float(want[0]))
+    assert np.isnan(W.windowed_idleness(np.zeros(5), np.zeros(5)))
+
+
+def test_eq1_responsive_and_outlier_robust():
+    # an ongoing long tool call soon dominates; one outlier among k=5 is diluted
+    base_r, base_a = [4.0] * 4, [1.0] * 4
+    prev = 0.0
+    for elapsed in (1, 10, 60, 600):
+        i = W.windowed_idleness(np.array(base_r + [4.0]), np.array(base_a + [elapsed]))
+        assert i > prev
+        prev = i
+    assert prev > 0.95
+    assert W.windowed_idleness(np.array([4.0] * 5), np.array([1, 1, 1, 1, 8.0])) < 0.4
+
+
+def test_config_shapes_match_baseline_json():
+    want = {1: (8 << 10, 16 << 10, 64, 256), 2: (64 << 10, 2 << 20, 30720, 65536),
+            3: (64 << 10, 4 << 20, 20480, 40960), 4: (128 << 10, 10 << 20, 10240, 20480),
+            5: (64 << 10, 2 << 20, 30720, 65536)}
+    for i, (chunk, page, gp, cp) in want.items():
+        c = W.get_config(i)
+        assert (c.shape.chunk_bytes, c.shape.page_bytes, c.gpu_pool_pages, c.cpu_pool_pages) == (chunk, page, gp, cp)
+    c = W.get_config(3, scale=16)
+    assert c.gpu_pool_pages == 1280 and c.shape == W.get_config(3).shape and c.n_programs == 128
+
+
+def test_trace_is_seed_deterministic_and_in_range():
+    cfg = W.get_config(2, scale=16)
+    a, b = W.Trace(cfg, 866), W.Trace(cfg, 866)
+    tier = np.zeros(cfg.n_programs, np.uint8)
+    for _ in range(30):
+        ia, ta, ra = a.advance(tier)
+        ib, tb, rb = b.advance(tier)
+        assert np.array_equal(ia, ib) and np.array_equal(ta, tb) and np.array_equal(ra, rb)
+        assert ia.dtype == np.float32 and ((ia >= 0) & (ia <= 1)).all()
+        assert (ta >= cfg.ctx_lo).all() and (ta <= cfg.ctx_hi).all()
+    c = W.Trace(cfg, 867)
+    assert not np.array_equal(c.advance(tier)[0], ia)
+
+
+def test_gated_time_is_excluded():
+    # a program that is never on the GPU never accrues reasoning time
+    cfg = W.get_config(1)
+    t = W.Trace(cfg, 1)
+    tier = np.full(cfg.n_programs, W.TIER_WAIT, np.uint8)
+    first, _, _ = t.advance(tier)
+    for _ in range(50):
+        iota, _, rep = t.advance(tier)
+    assert not rep.any() and np.array_equal(iota, first)
+
+
+def test_page_content_generator():
+    sh = W.KVShape(2, 2, 64, 16)
+    a = W.page_content(866, 3, 5, sh)
+    assert a.shape == (2, sh.chunk_bytes) and a.dtype == np.uint8
+    assert np.array_equal(a, W.page_content(866, 3, 5, sh))
+    assert not np.array_equal(a, W.page_content(866, 3, 6, sh))
+    assert not np.array_equal(a, W.page_content(866, 4, 5, sh))
+    assert not np.array_equal(a[0], a[1])
+    # bf16 values ~ N(0,1)
+    v = (a.reshape(-1).view(np.uint16).astype(np.uint32) << 16).view(np.float32)
+    assert abs(v.mean()) < 0.05 and 0.9 < v.std() < 1.1
+
+
+def _run(cfg, seed, epochs, brute=False, mirror=False):
+    sim = W.Sim(cfg, seed)
+    sh = cfg.shape
+    if mirror:
+        pool = np.zeros(sh.n_layers * cfg.gpu_pool_pages * sh.chunk_bytes, np.uint8)
+        arena = np.zeros(cfg.cpu_pool_pages * sh.page_bytes, np.uint8)
+    seen = np.zeros(3, int)
+    moved = 0
+    for _ in range(epochs):
+        plan = sim.begin_epoch()
+        r = oracle.rank_partition(plan.iota, plan.kv_pages, plan.prev_tier,
+                                  cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+        check_invariants(plan.iota, plan.kv_pages, cfg.cap_gpu_pages, cfg.cap_cpu_pages, r)
+        check_lists(plan.prev_tier, r)
+        if brute:
+            b = oracle.bruteforce_partition(plan.iota, plan.kv_pages, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+            assert b["n_best"] == 1 and np.array_equal(b["tier"], r["tier"])
+        sim.apply_placement(r["tier"], r["lists"])
+        if mirror:
+            for op in plan.ops:
+                if op[0] == "demote":
+                    oracle.demote(sh.n_layers, sh.chunk_bytes, pool, arena, op[3], op[4])
+                elif op[0] == "promote":
+                    oracle.promote(sh.n_layers, sh.chunk_bytes, pool, arena, op[3], op[4])
+        sim.end_epoch()
+        if mirror:
+            pv = pool.reshape(sh.n_layers, cfg.gpu_pool_pages, sh.chunk_bytes)
+            for uid, first, pages in plan.fills:
+                for j, g in enumerate(pages):
+                    pv[:, g] = W.page_content(seed, uid, first + j, sh)
+            # every resident logical page holds exactly its generated content
+            av = arena.reshape(cfg.cpu_pool_pages, sh.n_layers, sh.chunk_bytes)
+            for p in range(cfg.n_programs):
+                uid = int(sim.trace.uid[p])
+                for j, g in enumerate(sim.gpu_pages[p]):
+                    assert np.array_equal(pv[:, g], W.page_content(seed, uid, j, sh))
+                for j, h in enumerate(sim.host_slots[p]):
+                    assert np.array_equal(av[h], W.page_content(seed, uid, j, sh))
+        # no page / slot owned twice; tiers own what they should
+        gp = np.concatenate(sim.gpu_pages)
+        hs = np.concatenate(sim.host_slots)
+        assert len(set(gp.tolist())) == gp.size and len(set(hs.tolist())) == hs.size
+        assert not sim.gpu_alloc.free[gp].any() and not sim.cpu_alloc.free[hs].any()
+        assert sim.gpu_alloc.free.sum() + gp.size == cfg.gpu_pool_pages
+        assert sim.cpu_alloc.free.sum() + hs.size == cfg.cpu_pool_pages
+        for p in range(cfg.n_programs):
+            if sim.tier[p] == W.TIER_GPU:
+                assert sim.gpu_pages[p].size == plan.kv_pages[p] and sim.host_slots[p].size == 0
+            elif sim.tier[p] == W.TIER_CPU:
+                assert sim.gpu_pages[p].size == 0 and sim.host_slots[p].size <= plan.kv_pages[p]
+            else:
+                assert sim.gpu_pages[p].size == 0 and sim.host_slots[p].size == 0
+        seen += np.bincount(sim.tier, minlength=3)
+        moved += plan.demote_pages + plan.promote_pages
+    return seen, moved
+
+
+@pytest.mark.parametrize("seed", [866, 867, 868])
+def test_cfg1_oracle_run_bruteforce_every_epoch_with_byte_mirror(seed):
+    cfg = W.get_config(1)
+    seen, moved = _run(cfg, seed, cfg.epochs, brute=True, mirror=True)
+    assert seen[0] > 0
+
+
+@pytest.mark.parametrize("idx,scale,epochs", [(2, 32, 60), (3, 32, 40), (4, 32, 30), (5, 32, 20)])
+def test_scaled_twins_oracle_run(idx, scale, epochs):
+    cfg = W.get_config(idx, scale=scale)
+    seen, moved = _run(cfg, 866, epochs)
+    assert seen.min() > 0 and moved > 0          # all three tiers occur and pages move
+
+
+def test_cfg3_busy_fraction_moves_the_boundary():
+    frac = []
+    for f in (0.25, 0.5, 0.75):
+        cfg = W.get_config(3, scale=32, f_busy=f)
+        t = W.Trace(cfg, 866)
+        tier = np.zeros(cfg.n_programs, np.uint8)
+        for _ in range(40):
+            iota, _, _ = t.advance(tier)
+        frac.append(float((iota < 0.5).mean()))
+    assert frac[0] < frac[1] < frac[2]
