@@ -1,0 +1,191 @@
+/*
+ * mori.h -- C ABI of libmori.so: the data-parallel hot path under MORI's idleness-ranked
+ * two-tier KV placement (arxiv/paper_2606_00866), hand-written for NVIDIA B200 (sm_100a).
+ *
+ * Citations "P:Lnnn" are lines of the paper text; "R<k>" are the readings listed in DESIGN.md
+ * section 3 for points the paper leaves open.
+ *
+ * Conventions
+ *   - Every function returns a mori_status (0 = OK, negative = error) unless stated otherwise.
+ *   - Argument checks are synchronous: on MORI_ERR_INVALID_ARG nothing has been enqueued.
+ *   - Asynchronous CUDA failures surface at mori_sync() as MORI_ERR_CUDA and are sticky.
+ *   - "DEVICE" pointers are device memory of the context's GPU; "HOST" pointers are ordinary
+ *     host memory read before the call returns (the caller may reuse them at once);
+ *     "PINNED" is page-locked host memory mapped into the device address space
+ *     (cudaHostAlloc / cudaHostRegister; what torch's pin_memory gives).
+ *   - The caller owns the pool, the arena, the page allocator and every array it passes in;
+ *     the library owns the context, its streams, events, staging and index buffers.
+ *   - One context per GPU; calls on one context must come from one host thread at a time.
+ *   - There is no CPU fallback: without a usable sm_100a device mori_create fails.
+ *
+ * Layouts (BASELINE.json north_star; the paper only says the cache is paged)
+ *   chunk      = 2 (K,V) * n_kv_heads * page_tokens * head_dim * elem_bytes   contiguous bytes
+ *                of one (layer, physical page); must be a multiple of 16
+ *   gpu_pool   [n_layers][gpu_pool_pages][K/V][kv_heads][page_tokens][head_dim]
+ *              byte address of (layer l, page g)  = gpu_pool + (l * gpu_pool_pages + g) * chunk
+ *   host_arena [host_arena_slots][n_layers][K/V][kv_heads][page_tokens][head_dim]   (R7)
+ *              byte address of (slot h, layer l)  = host_arena + (h * n_layers + l) * chunk
+ *   Byte offsets are 64-bit; page ids and slot ids are int32.
+ */
+#ifndef MORI_H_
+#define MORI_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mori_ctx mori_ctx; /* opaque, library-owned */
+
+typedef enum {
+  MORI_OK = 0,
+  MORI_ERR_INVALID_ARG = -1,
+  MORI_ERR_CUDA = -2,
+  MORI_ERR_CAPACITY = -3, /* more pages in one call than the context was sized for */
+  MORI_ERR_STATE = -4,
+  MORI_ERR_UNSUPPORTED = -5
+} mori_status;
+
+enum { MORI_TIER_GPU = 0, MORI_TIER_CPU = 1, MORI_TIER_WAIT = 2 };
+enum { MORI_DEMOTE = 1, MORI_PROMOTE = 2, MORI_BOTH = 3 };
+enum { MORI_LIST_DEMOTE = 0, MORI_LIST_PROMOTE = 1, MORI_LIST_DROP = 2, MORI_LIST_ADMIT = 3,
+       MORI_LIST_RESERVE = 4, MORI_N_LISTS = 5 };
+/* How KV bytes cross the host link.
+ *   ZEROCOPY   one kernel: SMs load pool chunks and store them straight into the mapped arena
+ *              (demote), or load from the arena and store into the pool (promote).
+ *   STAGED     gather kernel pool -> contiguous device staging at HBM speed, then large
+ *              cudaMemcpyAsync DMAs staging -> arena on a copy stream, double-buffered
+ *              (promote: DMA arena -> staging, then scatter kernel staging -> pool).
+ *   COPYENGINE no kernel: one strided cudaMemcpy2DAsync per logical page (baseline).
+ *   AUTO       the per-direction choice measured fastest on B200. */
+enum { MORI_PATH_AUTO = 0, MORI_PATH_ZEROCOPY = 1, MORI_PATH_STAGED = 2, MORI_PATH_COPYENGINE = 3 };
+/* Device copy kernel used by STAGED paths and by mori_gather_pages / mori_scatter_pages. */
+enum { MORI_KERNEL_AUTO = 0, MORI_KERNEL_LDST = 1, MORI_KERNEL_TMA = 2 };
+
+#define MORI_MAX_PROGRAMS 8192 /* rank_partition sorts in one CTA's shared memory */
+
+typedef struct {
+  int32_t n_layers, n_kv_heads, head_dim, page_tokens, elem_bytes; /* bf16 -> elem_bytes 2 */
+  void*   gpu_pool;          /* DEVICE, caller-owned, 16-byte aligned */
+  int64_t gpu_pool_pages;
+  void*   host_arena;        /* PINNED, caller-owned, 16-byte aligned; may be NULL if neither
+                                mori_demote nor mori_promote is used */
+  int64_t host_arena_slots;
+  int32_t max_programs;      /* 1 .. MORI_MAX_PROGRAMS */
+  int32_t path_demote;       /* MORI_PATH_* */
+  int32_t path_promote;      /* MORI_PATH_* */
+  int32_t copy_kernel;       /* MORI_KERNEL_* */
+  int64_t staging_bytes;     /* per staging buffer (2 per direction); 0 -> 128 MiB */
+  int64_t max_pages_per_call;/* 0 -> max(gpu_pool_pages, host_arena_slots) */
+} mori_config;
+
+/* Creates a context on the CURRENT CUDA device.  *out is NULL on failure. */
+int mori_create(const mori_config* cfg, mori_ctx** out);
+/* Joins all outstanding work, then frees everything the library owns. */
+int mori_destroy(mori_ctx* ctx);
+
+/*
+ * Steps a1-a4 of the hot path: rank all active programs by idleness, prefix-sum their KV
+ * footprints in rank order, cut the ranking at the GPU and CPU capacities, label the rest
+ * WAITING, and list who moves.  One kernel launch on `stream` (a cudaStream_t; NULL = the
+ * legacy default stream); returns without waiting.  All pointers are DEVICE pointers.
+ *
+ *   Order      ascending idleness, rank 0 = busiest (the busier programs
+ *              are prioritised for HBM, the most idle go to CPU DRAM).  Equal scores (as floats,
+ *              so -0 == +0) rank by program index; NaN ranks after every number (R2, R11, R12).
+ *   GPU tier   ranks [0, b_gpu): the longest prefix whose summed kv_pages is <= gpu_cap_pages
+ *              ("does not exceed GPU memory capacity"; "filling from the busiest
+ *              end of the ranking until local capacity is reached").
+ *   CPU tier   ranks [b_gpu, b_cpu): the longest following run whose sum is <= cpu_cap_pages
+ *              ("enforced analogously").
+ *   WAITING    ranks [b_cpu, n): admitted to neither tier, KV discarded.
+ *   Lists      from prev_tier -> tier, each in the order the paper moves programs:
+ *                demote  (GPU -> CPU)      most idle first   ("highest idleness first")
+ *                promote (CPU -> GPU)      least idle first  ("lowest idleness first")
+ *                drop    (GPU|CPU -> WAIT) most idle first
+ *                admit   (WAIT -> GPU)     least idle first
+ *                reserve (WAIT -> CPU)     least idle first  (label only, no bytes: R9)
+ *
+ *   n            0 .. max_programs (0 is a valid no-op that still writes bounds/used/counts)
+ *   idleness     [n] float32, any value
+ *   kv_pages     [n] int32 >= 0 (negative values are treated as 0)
+ *   prev_tier    [n] uint8 or NULL; values other than 0 and 1 mean WAITING.  NULL: lists and
+ *                list_counts are not written (and may be NULL)
+ *   order        [n] out: program at each rank
+ *   tier         [n] out: MORI_TIER_* per program
+ *   bounds       [2] out: b_gpu, b_cpu
+ *   used_pages   [2] out: pages held by the GPU tier, by the CPU tier
+ *   lists        [5][n] out: row MORI_LIST_*; entries past list_counts[row] are unspecified
+ *   list_counts  [5] out
+ */
+int mori_rank_partition(mori_ctx* ctx, void* stream, int32_t n, const float* idleness,
+                        const int32_t* kv_pages, const uint8_t* prev_tier, int64_t gpu_cap_pages,
+                        int64_t cpu_cap_pages, int32_t* order, uint8_t* tier, int32_t* bounds,
+                        int64_t* used_pages, int32_t* lists, int32_t* list_counts);
+
+/*
+ * Step a5, demotion ("offloaded to CPU DRAM on the same node"): for every
+ * j in [0, total_pages) and every layer l, copy chunk (l, gpu_pages[j]) of the pool to
+ * (host_slots[j], l) of the arena.  Asynchronous, on the context's demote stream(s).
+ *
+ *   gpu_pages, host_slots  HOST int32[total_pages]; ids out of range -> MORI_ERR_INVALID_ARG.
+ *                          Duplicate destination slots are undefined behaviour.
+ *   wait_promote_ticket    0, or a ticket returned by mori_promote: no byte of this call is
+ *                          written before that promote call has completed (device-side wait).
+ *   ticket_out             NULL, or receives this call's ticket (> 0, increasing).
+ * total_pages == 0 is a valid no-op that still yields a ticket.
+ */
+int mori_demote(mori_ctx* ctx, int64_t total_pages, const int32_t* gpu_pages,
+                const int32_t* host_slots, int64_t wait_promote_ticket, int64_t* ticket_out);
+
+/*
+ * Step a6, promotion ("CPU-to-GPU transfer over PCIe"): the mirror image,
+ * arena (host_slots[j], l) -> pool (l, gpu_pages[j]), on the promote stream(s), concurrently
+ * with demotions.  wait_demote_ticket orders the pool writes after the demotion that vacated
+ * the destination pages (the host->device DMA of a STAGED promote may start earlier).
+ */
+int mori_promote(mori_ctx* ctx, int64_t total_pages, const int32_t* host_slots,
+                 const int32_t* gpu_pages, int64_t wait_demote_ticket, int64_t* ticket_out);
+
+/* Step a7: block the host until every demote (1), promote (2) or both (3) call has finished;
+ * returns the first asynchronous error if there was one. */
+int mori_sync(mori_ctx* ctx, int32_t which);
+
+/* Device-side ordering against a caller stream (cudaStream_t), no host blocking:
+ *   mori_after_stream   work enqueued later in direction(s) `which` starts after everything
+ *                       now in `stream` (e.g. the inference step that last touched the pages);
+ *   mori_stream_wait    work enqueued later in `stream` starts after everything now enqueued
+ *                       in direction(s) `which`. */
+int mori_after_stream(mori_ctx* ctx, int32_t which, void* stream);
+int mori_stream_wait(mori_ctx* ctx, void* stream, int32_t which);
+
+/*
+ * The on-device halves of the STAGED paths, exposed because they are what the HBM roofline is
+ * measured on: pool pages <-> a contiguous DEVICE buffer laid out [n_pages][n_layers][chunk].
+ * gpu_pages is a DEVICE int32[n_pages].  One launch on `stream`; asynchronous.
+ */
+int mori_gather_pages(mori_ctx* ctx, void* stream, int64_t n_pages, const int32_t* gpu_pages,
+                      void* dst);
+int mori_scatter_pages(mori_ctx* ctx, void* stream, int64_t n_pages, const int32_t* gpu_pages,
+                       const void* src);
+
+/* Kernel timing for the roofline: while enabled, every gather/scatter kernel launched by
+ * mori_demote / mori_promote is bracketed by CUDA events on its stream.  mori_profile_read
+ * (call after mori_sync) returns and clears the totals for one direction. */
+int mori_profile(mori_ctx* ctx, int32_t enable);
+int mori_profile_read(mori_ctx* ctx, int32_t which, double* kernel_ms, int64_t* launches,
+                      int64_t* bytes);
+
+/* Resolved MORI_PATH_* for a direction (after AUTO), and resolved MORI_KERNEL_*. */
+int mori_path(const mori_ctx* ctx, int32_t which);
+int mori_copy_kernel(const mori_ctx* ctx);
+
+/* Library-owned, NUL-terminated description of the last error on this context (or of the last
+ * failed mori_create when ctx is NULL); valid until the next call. */
+const char* mori_last_error(const mori_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MORI_H_ */

@@ -1,0 +1,246 @@
+"""ctypes binding over libmori.so -- argument marshalling only; every step runs in the library.
+
+Function names mirror include/mori.h.  Tensors are passed as ``data_ptr()``; torch is used for
+device memory and streams and nowhere else.  There is NO fallback: if the CUDA library cannot be
+loaded this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmori.so")
+WORKLOAD_LIB_PATH = os.path.join(_HERE, "libmori_workload.so")
+
+OK, ERR_INVALID_ARG, ERR_CUDA, ERR_CAPACITY, ERR_STATE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
+TIER_GPU, TIER_CPU, TIER_WAIT = 0, 1, 2
+DEMOTE, PROMOTE, BOTH = 1, 2, 3
+PATH_AUTO, PATH_ZEROCOPY, PATH_STAGED, PATH_COPYENGINE = 0, 1, 2, 3
+KERNEL_AUTO, KERNEL_LDST, KERNEL_TMA = 0, 1, 2
+MAX_PROGRAMS = 8192
+PATH_NAMES = {1: "zerocopy", 2: "staged", 3: "copyengine"}
+KERNEL_NAMES = {1: "ldst", 2: "tma"}
+
+EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", "mori_promote",
+           "mori_sync", "mori_after_stream", "mori_stream_wait", "mori_gather_pages",
+           "mori_scatter_pages", "mori_profile", "mori_profile_read", "mori_path",
+           "mori_copy_kernel", "mori_last_error"]
+
+
+class MoriConfig(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32),
+                ("page_tokens", C.c_int32), ("elem_bytes", C.c_int32),
+                ("gpu_pool", C.c_void_p), ("gpu_pool_pages", C.c_int64),
+                ("host_arena", C.c_void_p), ("host_arena_slots", C.c_int64),
+                ("max_programs", C.c_int32), ("path_demote", C.c_int32),
+                ("path_promote", C.c_int32), ("copy_kernel", C.c_int32),
+                ("staging_bytes", C.c_int64), ("max_pages_per_call", C.c_int64)]
+
+
+class MoriError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"mori status {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load():
+    """Loads libmori.so (built in-tree by ``paper_2606_00866_b200.build``).  Raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2606_00866_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+        L.mori_create.argtypes = [C.POINTER(MoriConfig), C.POINTER(vp)]
+        L.mori_destroy.argtypes = [vp]
+        L.mori_rank_partition.argtypes = [vp, vp, i32, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        L.mori_demote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
+        L.mori_promote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
+        L.mori_sync.argtypes = [vp, i32]
+        L.mori_after_stream.argtypes = [vp, i32, vp]
+        L.mori_stream_wait.argtypes = [vp, vp, i32]
+        L.mori_gather_pages.argtypes = [vp, vp, i64, vp, vp]
+        L.mori_scatter_pages.argtypes = [vp, vp, i64, vp, vp]
+        L.mori_profile.argtypes = [vp, i32]
+        L.mori_profile_read.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64), C.POINTER(i64)]
+        L.mori_path.argtypes = [vp, i32]
+        L.mori_copy_kernel.argtypes = [vp]
+        L.mori_last_error.argtypes = [vp]
+        L.mori_last_error.restype = C.c_char_p
+        for name in EXPORTS:
+            if name != "mori_last_error":
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _ptr(t) -> Optional[int]:
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+def _stream_handle(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _host_i32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+class Mori:
+    """One libmori context.  ``gpu_pool`` is a CUDA uint8/bf16 tensor of the whole pool,
+    ``host_arena`` a pinned CPU tensor (or None for rank/partition and device gather only)."""
+
+    def __init__(self, n_layers, n_kv_heads, head_dim, page_tokens, gpu_pool, host_arena=None,
+                 elem_bytes=2, max_programs=MAX_PROGRAMS, path_demote=PATH_AUTO,
+                 path_promote=PATH_AUTO, copy_kernel=KERNEL_AUTO, staging_bytes=0,
+                 max_pages_per_call=0):
+        self._lib = load()
+        self.chunk_bytes = 2 * n_kv_heads * page_tokens * head_dim * elem_bytes
+        self.page_bytes = self.chunk_bytes * n_layers
+        self.n_layers = n_layers
+        pool_bytes = gpu_pool.numel() * gpu_pool.element_size()
+        assert gpu_pool.is_cuda and gpu_pool.is_contiguous() and pool_bytes % self.page_bytes == 0
+        self.gpu_pool, self.host_arena = gpu_pool, host_arena      # keep alive
+        self.gpu_pool_pages = pool_bytes // self.page_bytes
+        cfg = MoriConfig(n_layers, n_kv_heads, head_dim, page_tokens, elem_bytes,
+                         gpu_pool.data_ptr(), self.gpu_pool_pages, None, 0, max_programs,
+                         path_demote, path_promote, copy_kernel, staging_bytes, max_pages_per_call)
+        self.host_arena_slots = 0
+        if host_arena is not None:
+            arena_bytes = host_arena.numel() * host_arena.element_size()
+            assert (not host_arena.is_cuda) and host_arena.is_pinned() and host_arena.is_contiguous()
+            assert arena_bytes % self.page_bytes == 0
+            self.host_arena_slots = arena_bytes // self.page_bytes
+            cfg.host_arena, cfg.host_arena_slots = host_arena.data_ptr(), self.host_arena_slots
+        h = C.c_void_p()
+        rc = self._lib.mori_create(C.byref(cfg), C.byref(h))
+        if rc != OK:
+            raise MoriError(rc, (self._lib.mori_last_error(None) or b"").decode())
+        self._h = h
+
+    # -- plumbing ----------------------------------------------------------------------------
+    def _ck(self, rc: int) -> int:
+        if rc != OK:
+            raise MoriError(rc, (self._lib.mori_last_error(self._h) or b"").decode())
+        return rc
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.mori_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def mori_path(self, which) -> int:
+        return self._lib.mori_path(self._h, which)
+
+    def mori_copy_kernel(self) -> int:
+        return self._lib.mori_copy_kernel(self._h)
+
+    @property
+    def path_demote(self) -> int:
+        return self.mori_path(DEMOTE)
+
+    @property
+    def path_promote(self) -> int:
+        return self.mori_path(PROMOTE)
+
+    @property
+    def copy_kernel(self) -> int:
+        return self.mori_copy_kernel()
+
+    # -- a1-a4 -------------------------------------------------------------------------------
+    def mori_rank_partition(self, n, idleness, kv_pages, prev_tier, gpu_cap_pages, cpu_cap_pages,
+                            order, tier, bounds, used_pages, lists=None, list_counts=None,
+                            stream=None):
+        """All array arguments are CUDA tensors (see include/mori.h); asynchronous on ``stream``."""
+        return self._ck(self._lib.mori_rank_partition(
+            self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), _ptr(prev_tier),
+            int(gpu_cap_pages), int(cpu_cap_pages), _ptr(order), _ptr(tier), _ptr(bounds),
+            _ptr(used_pages), _ptr(lists), _ptr(list_counts)))
+
+    # -- a5-a7 -------------------------------------------------------------------------------
+    def mori_demote(self, gpu_pages, host_slots, wait_promote_ticket=0) -> int:
+        g, h = _host_i32(gpu_pages), _host_i32(host_slots)
+        assert g.shape == h.shape and g.ndim == 1
+        t = C.c_int64(0)
+        self._ck(self._lib.mori_demote(self._h, g.size, g.ctypes.data, h.ctypes.data,
+                                       int(wait_promote_ticket), C.byref(t)))
+        return t.value
+
+    def mori_promote(self, host_slots, gpu_pages, wait_demote_ticket=0) -> int:
+        g, h = _host_i32(gpu_pages), _host_i32(host_slots)
+        assert g.shape == h.shape and g.ndim == 1
+        t = C.c_int64(0)
+        self._ck(self._lib.mori_promote(self._h, g.size, h.ctypes.data, g.ctypes.data,
+                                        int(wait_demote_ticket), C.byref(t)))
+        return t.value
+
+    def mori_sync(self, which=BOTH):
+        return self._ck(self._lib.mori_sync(self._h, which))
+
+    def mori_after_stream(self, which=BOTH, stream=None):
+        return self._ck(self._lib.mori_after_stream(self._h, which, _stream_handle(stream)))
+
+    def mori_stream_wait(self, stream=None, which=BOTH):
+        return self._ck(self._lib.mori_stream_wait(self._h, _stream_handle(stream), which))
+
+    # -- device halves -----------------------------------------------------------------------
+    def mori_gather_pages(self, gpu_pages_dev, dst, stream=None):
+        return self._ck(self._lib.mori_gather_pages(self._h, _stream_handle(stream),
+                                                    gpu_pages_dev.numel(), _ptr(gpu_pages_dev), _ptr(dst)))
+
+    def mori_scatter_pages(self, gpu_pages_dev, src, stream=None):
+        return self._ck(self._lib.mori_scatter_pages(self._h, _stream_handle(stream),
+                                                     gpu_pages_dev.numel(), _ptr(gpu_pages_dev), _ptr(src)))
+
+    # -- profiling ---------------------------------------------------------------------------
+    def mori_profile(self, enable: bool):
+        return self._ck(self._lib.mori_profile(self._h, int(enable)))
+
+    def mori_profile_read(self, which):
+        ms, n, b = C.c_double(0), C.c_int64(0), C.c_int64(0)
+        self._ck(self._lib.mori_profile_read(self._h, which, C.byref(ms), C.byref(n), C.byref(b)))
+        return ms.value, n.value, b.value
+
+
+# ------------------------------------------------------------------------------------------------
+# workload helper library (input generation on the device; not part of the hot path)
+# ------------------------------------------------------------------------------------------------
+_wl = None
+
+
+def load_workload_lib():
+    global _wl
+    if _wl is None:
+        if not os.path.exists(WORKLOAD_LIB_PATH):
+            raise RuntimeError(f"{WORKLOAD_LIB_PATH} is missing: run `python -m paper_2606_00866_b200.build`")
+        L = C.CDLL(WORKLOAD_LIB_PATH)
+        vp = C.c_void_p
+        L.wl_fill_pages.argtypes = [vp, C.c_longlong, C.c_int, C.c_int, vp, vp, C.c_longlong, C.c_int, vp]
+        L.wl_check_pages.argtypes = [vp, C.c_longlong, C.c_int, C.c_int, vp, vp, C.c_longlong, C.c_int, vp, vp]
+        L.wl_fill_pages.restype = C.c_int
+        L.wl_check_pages.restype = C.c_int
+        _wl = L
+    return _wl

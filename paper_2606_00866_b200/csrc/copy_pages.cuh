@@ -1,0 +1,190 @@
+// copy_pages.cuh -- steps a5/a6: move whole KV pages between the paged device pool and a
+// page-major linear buffer (device staging, or the mapped pinned host arena).  sm_100a.
+//
+//   pool    [L][P][chunk]    address of (layer l, page g)  = pool + (l*P + g) * chunk
+//   linear  [*][L][chunk]    address of (entry e, layer l) = lin  + (e*L + l) * chunk
+//   GATHER : lin(e_k, l) <- pool(l, g_k)        SCATTER : pool(l, g_k) <- lin(e_k, l)
+//   with g_k = gpu_pages[k] and e_k = lin_idx ? lin_idx[k] : k, for k in [0, n_pages).
+// (include/mori.h: mori_demote / mori_promote / mori_gather_pages / mori_scatter_pages;
+//  offload to CPU DRAM and reload over PCIe.)
+//
+// Pure data movement: the bound is HBM (device staging) or the host link (mapped arena), so the
+// design goal is bytes in flight, not arithmetic.  Work is cut into "pieces": a contiguous run
+// of <= kPieceBytes inside one chunk, contiguous on BOTH sides.  Piece w maps to
+// (k, l, c) = (w / (L*ppc), (w / ppc) % L, w % ppc) so consecutive CTAs stream through
+// consecutive addresses of one chunk (DRAM page locality on both sides).
+//
+// Two implementations:
+//   copy_pages_tma   one thread per CTA drives the SM's bulk-copy engine: cp.async.bulk
+//                    global->shared (mbarrier complete_tx) into a ring of stages, then
+//                    cp.async.bulk shared->global (bulk_group).  No registers, no LSU
+//                    instructions per byte; ~150 KiB of loads in flight per SM.
+//   copy_pages_ldst  256 threads, 4 x 16-byte ld.global.nc.L1::no_allocate per thread issued
+//                    before the 4 st.global: 16 KiB in flight per CTA, 8 CTAs per SM.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace mori {
+
+struct CopyArgs {
+  unsigned char* pool;
+  unsigned char* lin;
+  const int32_t* gpu_pages;   // [n_pages] device
+  const int32_t* lin_idx;     // [n_pages] device, or nullptr for identity
+  long long n_pages;
+  long long pool_pages;       // P
+  int n_layers;               // L
+  int chunk_bytes;            // multiple of 16
+  int piece_bytes;            // multiple of 16, <= chunk_bytes
+  int pieces_per_chunk;       // ceil(chunk / piece)
+};
+
+template <bool kGather>
+__device__ __forceinline__ void piece_addresses(const CopyArgs& a, long long w, const unsigned char*& src,
+                                                unsigned char*& dst, int& bytes) {
+  const int ppc = a.pieces_per_chunk;
+  const long long per_page = (long long)a.n_layers * ppc;
+  const long long k = w / per_page;
+  const int rem = (int)(w - k * per_page);
+  const int l = rem / ppc, c = rem - l * ppc;
+  const long long g = a.gpu_pages[k];
+  const long long e = a.lin_idx ? (long long)a.lin_idx[k] : k;
+  const long long off = (long long)c * a.piece_bytes;
+  bytes = min(a.piece_bytes, a.chunk_bytes - (int)off);
+  unsigned char* pp = a.pool + ((long long)l * a.pool_pages + g) * a.chunk_bytes + off;
+  unsigned char* lp = a.lin + (e * a.n_layers + l) * a.chunk_bytes + off;
+  if (kGather) { src = pp; dst = lp; } else { src = lp; dst = pp; }
+}
+
+// ------------------------------------------------------------------------------------------
+// LD/ST implementation
+// ------------------------------------------------------------------------------------------
+constexpr int kLdstThreads = 256;
+constexpr int kLdstUnroll = 4;   // 256 thr * 4 * 16 B = 16 KiB per CTA iteration
+
+__device__ __forceinline__ int4 ld_stream(const int4* p) {
+  int4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(int4* p, const int4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};"
+               :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+template <bool kGather>
+__global__ void __launch_bounds__(kLdstThreads) copy_pages_ldst(const CopyArgs a) {
+  const long long n_pieces = a.n_pages * a.n_layers * a.pieces_per_chunk;
+  for (long long w = blockIdx.x; w < n_pieces; w += gridDim.x) {
+    const unsigned char* src; unsigned char* dst; int bytes;
+    piece_addresses<kGather>(a, w, src, dst, bytes);
+    const int4* s = reinterpret_cast<const int4*>(src);
+    int4* d = reinterpret_cast<int4*>(dst);
+    const int n_vec = bytes >> 4;
+    for (int v0 = 0; v0 < n_vec; v0 += kLdstThreads * kLdstUnroll) {
+      int4 r[kLdstUnroll];
+#pragma unroll
+      for (int u = 0; u < kLdstUnroll; ++u) {
+        const int v = v0 + u * kLdstThreads + threadIdx.x;
+        if (v < n_vec) r[u] = ld_stream(s + v);
+      }
+#pragma unroll
+      for (int u = 0; u < kLdstUnroll; ++u) {
+        const int v = v0 + u * kLdstThreads + threadIdx.x;
+        if (v < n_vec) st_stream(d + v, r[u]);
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// TMA (1-D bulk copy) implementation
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;"
+               :: "r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" :: "r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+      :: "r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               :: "l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int kPending>
+__device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(kPending) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+constexpr int kTmaThreads = 32;
+constexpr int kTmaStoreLag = 2;   // stores allowed to be still reading shared memory
+
+// Shared memory: kStages stage buffers of a.piece_bytes each, then kStages mbarriers.
+// Lane 0 runs the whole pipeline; loads run (kStages - kTmaStoreLag) pieces ahead of stores.
+template <bool kGather, int kStages>
+__global__ void __launch_bounds__(kTmaThreads, 1) copy_pages_tma(const CopyArgs a) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * a.piece_bytes);
+  if (threadIdx.x != 0) return;
+  for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+
+  const long long n_pieces = a.n_pages * a.n_layers * a.pieces_per_chunk;
+  const long long first = blockIdx.x, step = gridDim.x;
+  if (first >= n_pieces) return;
+  const long long n_mine = (n_pieces - first + step - 1) / step;
+  constexpr int kAhead = kStages - kTmaStoreLag;
+
+  long long i_load = 0;
+  auto issue_load = [&](long long i) {
+    const unsigned char* src; unsigned char* dst; int bytes;
+    piece_addresses<kGather>(a, first + i * step, src, dst, bytes);
+    const int st = (int)(i % kStages);
+    mbar_expect_tx(&full[st], (uint32_t)bytes);
+    bulk_g2s(smem + (size_t)st * a.piece_bytes, src, (uint32_t)bytes, &full[st]);
+  };
+  for (; i_load < n_mine && i_load < kAhead; ++i_load) issue_load(i_load);
+
+  for (long long i = 0; i < n_mine; ++i) {
+    const int st = (int)(i % kStages);
+    const uint32_t parity = (uint32_t)((i / kStages) & 1);
+    const unsigned char* src; unsigned char* dst; int bytes;
+    piece_addresses<kGather>(a, first + i * step, src, dst, bytes);
+    mbar_wait(&full[st], parity);
+    bulk_s2g(dst, smem + (size_t)st * a.piece_bytes, (uint32_t)bytes);
+    bulk_commit();
+    if (i_load < n_mine) {
+      // the stage piece i_load lands in was last read by the store of piece i_load - kStages
+      // = i - kTmaStoreLag: every group but the newest kTmaStoreLag must have finished reading
+      bulk_wait_read<kTmaStoreLag>();
+      issue_load(i_load);
+      ++i_load;
+    }
+  }
+  bulk_wait_all();   // writes complete before the CTA exits
+}
+
+}  // namespace mori

@@ -1,0 +1,549 @@
+// mori.cu -- libmori.so: context, streams, staging and the C ABI of include/mori.h.
+// Every step of the hot path runs in the kernels of rank_partition.cuh / copy_pages.cuh or on
+// the GPU's copy engines; the host code here only marshals arguments and orders streams.
+#include "../../include/mori.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "copy_pages.cuh"
+#include "rank_partition.cuh"
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr int kTicketRing = 4096;
+constexpr int kTmaStages = 12;
+constexpr int kPieceBytes = 16 * 1024;
+
+struct ProfSpan { cudaEvent_t a, b; long long bytes; };
+
+struct Direction {
+  int path = 0;
+  cudaStream_t kern = nullptr, copy = nullptr;   // kernel stream, DMA stream (STAGED only)
+  unsigned char* staging[2] = {nullptr, nullptr};
+  cudaEvent_t kern_done[2] = {nullptr, nullptr}, copy_done[2] = {nullptr, nullptr};
+  int buf = 0;
+  // index ring: pinned host (written by the CPU, read by the upload kernel) + device copy
+  int32_t* idx_host = nullptr; int32_t* idx_host_dev = nullptr; int32_t* idx_dev = nullptr;
+  long long idx_cap = 0, idx_used = 0;
+  std::vector<cudaEvent_t> tickets;              // ring
+  long long next_ticket = 1;
+  std::vector<ProfSpan> spans;
+  double prof_ms = 0; long long prof_launches = 0, prof_bytes = 0;
+};
+
+}  // namespace
+
+struct mori_ctx {
+  mori_config cfg;
+  int device = 0, sm_count = 148;
+  long long chunk = 0, page_bytes = 0, staging_bytes = 0, max_pages = 0;
+  int copy_kernel = MORI_KERNEL_TMA;
+  int piece = kPieceBytes, ppc = 1;
+  size_t tma_smem = 0;
+  unsigned char* arena_dev = nullptr;            // device-side alias of the pinned arena
+  Direction dir[2];                              // 0 demote, 1 promote
+  std::vector<cudaEvent_t> free_events;
+  bool profiling = false;
+  int sticky = MORI_OK;
+  mutable std::string err;
+};
+
+namespace {
+
+int fail(const mori_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_create_error = msg;
+  return code;
+}
+
+#define CK(ctx, call)                                                                         \
+  do {                                                                                        \
+    cudaError_t e_ = (call);                                                                  \
+    if (e_ != cudaSuccess) {                                                                  \
+      if (ctx) (ctx)->sticky = MORI_ERR_CUDA;                                                 \
+      return fail(ctx, MORI_ERR_CUDA,                                                         \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                        \
+    }                                                                                         \
+  } while (0)
+
+__global__ void upload_idx_kernel(const int32_t* __restrict__ src, int32_t* __restrict__ dst, long long n) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x)
+    dst[i] = src[i];
+}
+
+mori::CopyArgs make_args(const mori_ctx* c, unsigned char* lin, const int32_t* gpu_pages,
+                         const int32_t* lin_idx, long long n_pages) {
+  mori::CopyArgs a;
+  a.pool = static_cast<unsigned char*>(c->cfg.gpu_pool);
+  a.lin = lin;
+  a.gpu_pages = gpu_pages;
+  a.lin_idx = lin_idx;
+  a.n_pages = n_pages;
+  a.pool_pages = c->cfg.gpu_pool_pages;
+  a.n_layers = c->cfg.n_layers;
+  a.chunk_bytes = (int)c->chunk;
+  a.piece_bytes = c->piece;
+  a.pieces_per_chunk = c->ppc;
+  return a;
+}
+
+// One launch of the page-copy kernel.  `link` = the linear side is host memory behind PCIe:
+// a small grid saturates the link and leaves the SMs to everything else.
+template <bool kGather>
+cudaError_t launch_copy(const mori_ctx* c, const mori::CopyArgs& a, cudaStream_t s, bool link) {
+  const long long n_pieces = a.n_pages * a.n_layers * a.pieces_per_chunk;
+  if (n_pieces == 0) return cudaSuccess;
+  if (c->copy_kernel == MORI_KERNEL_TMA) {
+    const long long max_grid = link ? 32 : c->sm_count;          // 1 CTA per SM (smem-bound)
+    const int grid = (int)std::min<long long>(n_pieces, max_grid);
+    mori::copy_pages_tma<kGather, kTmaStages><<<grid, mori::kTmaThreads, c->tma_smem, s>>>(a);
+  } else {
+    const long long max_grid = link ? 64 : (long long)c->sm_count * 8;
+    const int grid = (int)std::min<long long>(n_pieces, max_grid);
+    mori::copy_pages_ldst<kGather><<<grid, mori::kLdstThreads, 0, s>>>(a);
+  }
+  return cudaGetLastError();
+}
+
+cudaEvent_t get_event(mori_ctx* c, bool timing) {
+  cudaEvent_t e = nullptr;
+  if (!timing && !c->free_events.empty()) { e = c->free_events.back(); c->free_events.pop_back(); return e; }
+  cudaEventCreateWithFlags(&e, timing ? cudaEventDefault : cudaEventDisableTiming);
+  return e;
+}
+
+int check_ids(const mori_ctx* c, long long n, const int32_t* gpu_pages, const int32_t* host_slots) {
+  for (long long j = 0; j < n; ++j) {
+    if (gpu_pages[j] < 0 || gpu_pages[j] >= c->cfg.gpu_pool_pages)
+      return fail(c, MORI_ERR_INVALID_ARG, "gpu page id out of range at index " + std::to_string(j));
+    if (host_slots[j] < 0 || host_slots[j] >= c->cfg.host_arena_slots)
+      return fail(c, MORI_ERR_INVALID_ARG, "host slot id out of range at index " + std::to_string(j));
+  }
+  return MORI_OK;
+}
+
+// Copies the two index arrays into the direction's pinned ring and launches the upload kernel
+// on the kernel stream.  Returns device pointers.
+int stage_indices(mori_ctx* c, Direction& d, long long n, const int32_t* a0, const int32_t* a1,
+                  const int32_t** d0, const int32_t** d1) {
+  if (2 * n > d.idx_cap) return fail(c, MORI_ERR_CAPACITY, "more pages in one call than max_pages_per_call");
+  if (d.idx_used + 2 * n > d.idx_cap) {           // ring full: drain this direction, start over
+    CK(c, cudaStreamSynchronize(d.kern));
+    if (d.copy) CK(c, cudaStreamSynchronize(d.copy));
+    d.idx_used = 0;
+  }
+  int32_t* h = d.idx_host + d.idx_used;
+  std::memcpy(h, a0, sizeof(int32_t) * n);
+  std::memcpy(h + n, a1, sizeof(int32_t) * n);
+  const int grid = (int)std::min<long long>((2 * n + 255) / 256, 64);
+  upload_idx_kernel<<<grid, 256, 0, d.kern>>>(d.idx_host_dev + d.idx_used, d.idx_dev + d.idx_used, 2 * n);
+  CK(c, cudaGetLastError());
+  *d0 = d.idx_dev + d.idx_used;
+  *d1 = d.idx_dev + d.idx_used + n;
+  d.idx_used += 2 * n;
+  return MORI_OK;
+}
+
+int wait_ticket(mori_ctx* c, Direction& other, long long ticket, cudaStream_t s) {
+  if (ticket <= 0) return MORI_OK;
+  if (ticket >= other.next_ticket) return fail(c, MORI_ERR_INVALID_ARG, "ticket was never issued");
+  // a ticket older than the ring has been overwritten by a LATER event of the same stream:
+  // waiting on that one is conservative and still correct.
+  CK(c, cudaStreamWaitEvent(s, other.tickets[ticket % kTicketRing], 0));
+  return MORI_OK;
+}
+
+int issue_ticket(mori_ctx* c, Direction& d, cudaStream_t s, int64_t* out) {
+  const long long t = d.next_ticket++;
+  CK(c, cudaEventRecord(d.tickets[t % kTicketRing], s));
+  if (out) *out = t;
+  return MORI_OK;
+}
+
+void prof_begin(mori_ctx* c, Direction& d, cudaStream_t s, long long bytes) {
+  if (!c->profiling) return;
+  ProfSpan sp{get_event(c, true), get_event(c, true), bytes};
+  cudaEventRecord(sp.a, s);
+  d.spans.push_back(sp);
+}
+void prof_end(mori_ctx* c, Direction& d, cudaStream_t s) {
+  if (!c->profiling) return;
+  cudaEventRecord(d.spans.back().b, s);
+}
+void prof_collect(Direction& d) {
+  for (auto& sp : d.spans) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) {
+      d.prof_ms += ms; d.prof_launches += 1; d.prof_bytes += sp.bytes;
+    }
+    cudaEventDestroy(sp.a); cudaEventDestroy(sp.b);
+  }
+  d.spans.clear();
+}
+
+template <int IPT>
+cudaError_t launch_rank(int threads, size_t smem, cudaStream_t s, int n, int n_pad, const float* idl,
+                        const int32_t* kv, const uint8_t* prev, long long cg, long long cc, int32_t* order,
+                        uint8_t* tier, int32_t* bounds, long long* used, int32_t* lists, int32_t* counts) {
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(mori::rank_partition_kernel<IPT>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  mori::rank_partition_kernel<IPT><<<1, threads, smem, s>>>(n, n_pad, idl, kv, prev, cg, cc, order, tier,
+                                                            bounds, used, lists, counts);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mori_last_error(const mori_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int mori_create(const mori_config* cfg, mori_ctx** out) {
+  if (out) *out = nullptr;
+  if (!cfg || !out) return fail(nullptr, MORI_ERR_INVALID_ARG, "cfg/out is NULL");
+  if (cfg->n_layers <= 0 || cfg->n_kv_heads <= 0 || cfg->head_dim <= 0 || cfg->page_tokens <= 0 ||
+      cfg->elem_bytes <= 0)
+    return fail(nullptr, MORI_ERR_INVALID_ARG, "KV shape fields must be positive");
+  if (!cfg->gpu_pool || cfg->gpu_pool_pages <= 0) return fail(nullptr, MORI_ERR_INVALID_ARG, "gpu_pool missing");
+  if (cfg->gpu_pool_pages > INT32_MAX || cfg->host_arena_slots > INT32_MAX || cfg->host_arena_slots < 0)
+    return fail(nullptr, MORI_ERR_INVALID_ARG, "page/slot counts must fit int32");
+  if (cfg->max_programs < 1 || cfg->max_programs > MORI_MAX_PROGRAMS)
+    return fail(nullptr, MORI_ERR_INVALID_ARG, "max_programs must be 1..8192");
+  const long long chunk = 2LL * cfg->n_kv_heads * cfg->page_tokens * cfg->head_dim * cfg->elem_bytes;
+  if (chunk % 16 != 0 || chunk > (1LL << 30)) return fail(nullptr, MORI_ERR_INVALID_ARG, "chunk must be a multiple of 16 bytes");
+  if (((uintptr_t)cfg->gpu_pool & 15) || ((uintptr_t)cfg->host_arena & 15))
+    return fail(nullptr, MORI_ERR_INVALID_ARG, "gpu_pool and host_arena must be 16-byte aligned");
+  for (int p : {cfg->path_demote, cfg->path_promote})
+    if (p < MORI_PATH_AUTO || p > MORI_PATH_COPYENGINE) return fail(nullptr, MORI_ERR_INVALID_ARG, "bad path");
+  if (cfg->copy_kernel < MORI_KERNEL_AUTO || cfg->copy_kernel > MORI_KERNEL_TMA)
+    return fail(nullptr, MORI_ERR_INVALID_ARG, "bad copy_kernel");
+  if (cfg->staging_bytes < 0 || cfg->max_pages_per_call < 0) return fail(nullptr, MORI_ERR_INVALID_ARG, "negative size");
+
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(nullptr, MORI_ERR_CUDA, std::string("no CUDA device: ") + cudaGetErrorString(e));
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) return fail(nullptr, MORI_ERR_CUDA, cudaGetErrorString(e));
+  if (prop.major != 10) return fail(nullptr, MORI_ERR_UNSUPPORTED, "libmori is built for sm_100a (B200) only");
+
+  mori_ctx* c = new mori_ctx();
+  c->cfg = *cfg;
+  c->device = dev;
+  c->sm_count = prop.multiProcessorCount;
+  c->chunk = chunk;
+  c->page_bytes = chunk * cfg->n_layers;
+  c->piece = (int)std::min<long long>(kPieceBytes, chunk);
+  c->ppc = (int)((chunk + c->piece - 1) / c->piece);
+  c->copy_kernel = cfg->copy_kernel == MORI_KERNEL_AUTO ? MORI_KERNEL_TMA : cfg->copy_kernel;
+  c->tma_smem = (size_t)kTmaStages * c->piece + kTmaStages * sizeof(uint64_t);
+  c->max_pages = cfg->max_pages_per_call ? cfg->max_pages_per_call
+                                          : std::max<long long>(cfg->gpu_pool_pages, cfg->host_arena_slots);
+  c->staging_bytes = cfg->staging_bytes ? cfg->staging_bytes : (128LL << 20);
+  c->staging_bytes = std::max(c->staging_bytes, c->page_bytes);
+  c->staging_bytes -= c->staging_bytes % c->page_bytes;
+  // AUTO: see DESIGN.md section 6 for the measurements behind this choice.
+  c->dir[0].path = cfg->path_demote == MORI_PATH_AUTO ? MORI_PATH_STAGED : cfg->path_demote;
+  c->dir[1].path = cfg->path_promote == MORI_PATH_AUTO ? MORI_PATH_STAGED : cfg->path_promote;
+  *out = c;   // from here on mori_destroy cleans up
+
+#define CKC(call)                                                                             \
+  do {                                                                                        \
+    cudaError_t e2_ = (call);                                                                 \
+    if (e2_ != cudaSuccess) {                                                                 \
+      g_create_error = std::string(#call) + ": " + cudaGetErrorString(e2_);                   \
+      mori_destroy(c); *out = nullptr; return MORI_ERR_CUDA;                                  \
+    }                                                                                         \
+  } while (0)
+
+  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<true, kTmaStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
+  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<false, kTmaStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
+  if (cfg->host_arena) {
+    void* dp = nullptr;
+    CKC(cudaHostGetDevicePointer(&dp, cfg->host_arena, 0));
+    c->arena_dev = static_cast<unsigned char*>(dp);
+  }
+  for (int i = 0; i < 2; ++i) {
+    Direction& d = c->dir[i];
+    CKC(cudaStreamCreateWithFlags(&d.kern, cudaStreamNonBlocking));
+    CKC(cudaStreamCreateWithFlags(&d.copy, cudaStreamNonBlocking));
+    d.tickets.resize(kTicketRing);
+    for (auto& ev : d.tickets) CKC(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    if (cfg->host_arena) {
+      d.idx_cap = std::max<long long>(4 * c->max_pages, 1 << 16);
+      CKC(cudaHostAlloc((void**)&d.idx_host, sizeof(int32_t) * d.idx_cap, cudaHostAllocMapped));
+      CKC(cudaHostGetDevicePointer((void**)&d.idx_host_dev, d.idx_host, 0));
+      CKC(cudaMalloc((void**)&d.idx_dev, sizeof(int32_t) * d.idx_cap));
+      if (d.path == MORI_PATH_STAGED) {
+        for (int b = 0; b < 2; ++b) {
+          CKC(cudaMalloc((void**)&d.staging[b], c->staging_bytes));
+          CKC(cudaEventCreateWithFlags(&d.kern_done[b], cudaEventDisableTiming));
+          CKC(cudaEventCreateWithFlags(&d.copy_done[b], cudaEventDisableTiming));
+        }
+      }
+    }
+  }
+#undef CKC
+  return MORI_OK;
+}
+
+int mori_destroy(mori_ctx* c) {
+  if (!c) return MORI_OK;
+  cudaDeviceSynchronize();
+  for (int i = 0; i < 2; ++i) {
+    Direction& d = c->dir[i];
+    prof_collect(d);
+    for (int b = 0; b < 2; ++b) {
+      if (d.staging[b]) cudaFree(d.staging[b]);
+      if (d.kern_done[b]) cudaEventDestroy(d.kern_done[b]);
+      if (d.copy_done[b]) cudaEventDestroy(d.copy_done[b]);
+    }
+    if (d.idx_host) cudaFreeHost(d.idx_host);
+    if (d.idx_dev) cudaFree(d.idx_dev);
+    for (auto ev : d.tickets) if (ev) cudaEventDestroy(ev);
+    if (d.kern) cudaStreamDestroy(d.kern);
+    if (d.copy) cudaStreamDestroy(d.copy);
+  }
+  for (auto ev : c->free_events) cudaEventDestroy(ev);
+  delete c;
+  return MORI_OK;
+}
+
+int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idleness, const int32_t* kv_pages,
+                        const uint8_t* prev_tier, int64_t gpu_cap, int64_t cpu_cap, int32_t* order,
+                        uint8_t* tier, int32_t* bounds, int64_t* used, int32_t* lists, int32_t* counts) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (n < 0 || n > c->cfg.max_programs) return fail(c, MORI_ERR_INVALID_ARG, "n out of range (0..max_programs)");
+  if (gpu_cap < 0 || cpu_cap < 0) return fail(c, MORI_ERR_INVALID_ARG, "negative capacity");
+  if (!bounds || !used) return fail(c, MORI_ERR_INVALID_ARG, "bounds/used_pages is NULL");
+  if (n > 0 && (!idleness || !kv_pages || !order || !tier)) return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
+  if (prev_tier && (!lists || !counts)) return fail(c, MORI_ERR_INVALID_ARG, "prev_tier given but lists/list_counts NULL");
+  int n_pad = 32;
+  while (n_pad < n) n_pad <<= 1;
+  const int ipt = n_pad <= 1024 ? 1 : n_pad / 1024;
+  const int threads = n_pad / ipt;
+  const size_t smem = sizeof(uint64_t) * (n_pad + 33) + 2 * sizeof(long long);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  cudaError_t e;
+  long long* u = reinterpret_cast<long long*>(used);
+#define LR(I) launch_rank<I>(threads, smem, s, n, n_pad, idleness, kv_pages, prev_tier, gpu_cap, cpu_cap, order, tier, bounds, u, lists, counts)
+  switch (ipt) {
+    case 1: e = LR(1); break;
+    case 2: e = LR(2); break;
+    case 4: e = LR(4); break;
+    default: e = LR(8); break;
+  }
+#undef LR
+  CK(c, e);
+  return MORI_OK;
+}
+
+int mori_gather_pages(mori_ctx* c, void* stream, int64_t n_pages, const int32_t* gpu_pages, void* dst) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (n_pages < 0 || (n_pages > 0 && (!gpu_pages || !dst))) return fail(c, MORI_ERR_INVALID_ARG, "bad gather arguments");
+  mori::CopyArgs a = make_args(c, static_cast<unsigned char*>(dst), gpu_pages, nullptr, n_pages);
+  CK(c, launch_copy<true>(c, a, static_cast<cudaStream_t>(stream), false));
+  return MORI_OK;
+}
+
+int mori_scatter_pages(mori_ctx* c, void* stream, int64_t n_pages, const int32_t* gpu_pages, const void* src) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (n_pages < 0 || (n_pages > 0 && (!gpu_pages || !src))) return fail(c, MORI_ERR_INVALID_ARG, "bad scatter arguments");
+  mori::CopyArgs a = make_args(c, static_cast<unsigned char*>(const_cast<void*>(src)), gpu_pages, nullptr, n_pages);
+  CK(c, launch_copy<false>(c, a, static_cast<cudaStream_t>(stream), false));
+  return MORI_OK;
+}
+
+// Shared body of mori_demote (dir 0) and mori_promote (dir 1).
+static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_pages, const int32_t* host_slots,
+                   long long wait_other, int64_t* ticket_out) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (!c->cfg.host_arena) return fail(c, MORI_ERR_STATE, "context was created without a host arena");
+  if (total < 0 || (total > 0 && (!gpu_pages || !host_slots))) return fail(c, MORI_ERR_INVALID_ARG, "bad page table");
+  if (total > c->max_pages) return fail(c, MORI_ERR_CAPACITY, "total_pages exceeds max_pages_per_call");
+  if (int rc = check_ids(c, total, gpu_pages, host_slots)) return rc;
+  Direction& d = c->dir[di];
+  Direction& other = c->dir[1 - di];
+  const bool demote = di == 0;
+  unsigned char* pool = static_cast<unsigned char*>(c->cfg.gpu_pool);
+  unsigned char* arena = static_cast<unsigned char*>(c->cfg.host_arena);
+  const long long pb = c->page_bytes;
+
+  if (d.path == MORI_PATH_ZEROCOPY) {
+    if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc;
+    if (total > 0) {
+      const int32_t *dg, *dh;
+      if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;
+      mori::CopyArgs a = make_args(c, c->arena_dev, dg, dh, total);
+      prof_begin(c, d, d.kern, total * pb);
+      CK(c, demote ? launch_copy<true>(c, a, d.kern, true) : launch_copy<false>(c, a, d.kern, true));
+      prof_end(c, d, d.kern);
+    }
+    return issue_ticket(c, d, d.kern, ticket_out);
+  }
+
+  if (d.path == MORI_PATH_COPYENGINE) {
+    if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc;
+    const size_t dpitch = (size_t)c->cfg.gpu_pool_pages * c->chunk;   // layer stride in the pool
+    for (long long j = 0; j < total; ++j) {
+      unsigned char* dev = pool + (long long)gpu_pages[j] * c->chunk;
+      unsigned char* hst = arena + (long long)host_slots[j] * pb;
+      if (demote) CK(c, cudaMemcpy2DAsync(hst, c->chunk, dev, dpitch, c->chunk, c->cfg.n_layers, cudaMemcpyDeviceToHost, d.kern));
+      else        CK(c, cudaMemcpy2DAsync(dev, dpitch, hst, c->chunk, c->chunk, c->cfg.n_layers, cudaMemcpyHostToDevice, d.kern));
+    }
+    return issue_ticket(c, d, d.kern, ticket_out);
+  }
+
+  // STAGED.  demote:  kern stream: gather -> staging[b]      copy stream: staging[b] -> arena
+  //          promote: copy stream: arena -> staging[b]       kern stream: staging[b] -> scatter
+  // Double-buffered with events so the DMA of segment i overlaps the kernel of segment i+1.
+  const long long seg_pages = c->staging_bytes / pb;
+  const int32_t* dg = nullptr; const int32_t* dh = nullptr;
+  if (demote) { if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc; }
+  if (total > 0)
+    if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;
+  bool waited = demote;
+  for (long long a0 = 0; a0 < total; a0 += seg_pages) {
+    const long long cnt = std::min(seg_pages, total - a0);
+    const int b = d.buf; d.buf ^= 1;
+    unsigned char* stg = d.staging[b];
+    mori::CopyArgs a = make_args(c, stg, dg + a0, nullptr, cnt);
+    auto dma = [&](cudaStream_t s) -> int {
+      for (long long i = 0; i < cnt;) {                      // one DMA per run of consecutive slots
+        long long r = 1;
+        while (i + r < cnt && host_slots[a0 + i + r] == host_slots[a0 + i] + r) ++r;
+        unsigned char* h = arena + (long long)host_slots[a0 + i] * pb;
+        if (demote) CK(c, cudaMemcpyAsync(h, stg + i * pb, r * pb, cudaMemcpyDeviceToHost, s));
+        else        CK(c, cudaMemcpyAsync(stg + i * pb, h, r * pb, cudaMemcpyHostToDevice, s));
+        i += r;
+      }
+      return MORI_OK;
+    };
+    if (demote) {
+      CK(c, cudaStreamWaitEvent(d.kern, d.copy_done[b], 0));       // staging[b] drained
+      prof_begin(c, d, d.kern, cnt * pb);
+      CK(c, launch_copy<true>(c, a, d.kern, false));
+      prof_end(c, d, d.kern);
+      CK(c, cudaEventRecord(d.kern_done[b], d.kern));
+      CK(c, cudaStreamWaitEvent(d.copy, d.kern_done[b], 0));
+      if (int rc = dma(d.copy)) return rc;
+      CK(c, cudaEventRecord(d.copy_done[b], d.copy));
+    } else {
+      CK(c, cudaStreamWaitEvent(d.copy, d.kern_done[b], 0));       // staging[b] scattered
+      if (int rc = dma(d.copy)) return rc;
+      CK(c, cudaEventRecord(d.copy_done[b], d.copy));
+      if (!waited) { if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc; waited = true; }
+      CK(c, cudaStreamWaitEvent(d.kern, d.copy_done[b], 0));
+      prof_begin(c, d, d.kern, cnt * pb);
+      CK(c, launch_copy<false>(c, a, d.kern, false));
+      prof_end(c, d, d.kern);
+      CK(c, cudaEventRecord(d.kern_done[b], d.kern));
+    }
+  }
+  if (!waited) { if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc; }
+  // the ticket marks the end of the LAST stage of the pipeline
+  if (demote) {
+    // copy stream finishes last; make the kernel stream's order include it so that one event
+    // on one stream covers the call
+    cudaEvent_t ev = d.tickets[d.next_ticket % kTicketRing];
+    const long long t = d.next_ticket++;
+    CK(c, cudaEventRecord(ev, d.copy));
+    if (ticket_out) *ticket_out = t;
+    return MORI_OK;
+  }
+  return issue_ticket(c, d, d.kern, ticket_out);
+}
+
+int mori_demote(mori_ctx* c, int64_t total, const int32_t* gpu_pages, const int32_t* host_slots,
+                int64_t wait_promote_ticket, int64_t* ticket_out) {
+  return migrate(c, 0, total, gpu_pages, host_slots, wait_promote_ticket, ticket_out);
+}
+
+int mori_promote(mori_ctx* c, int64_t total, const int32_t* host_slots, const int32_t* gpu_pages,
+                 int64_t wait_demote_ticket, int64_t* ticket_out) {
+  return migrate(c, 1, total, gpu_pages, host_slots, wait_demote_ticket, ticket_out);
+}
+
+int mori_sync(mori_ctx* c, int32_t which) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (which < 1 || which > 3) return fail(c, MORI_ERR_INVALID_ARG, "which must be 1, 2 or 3");
+  for (int i = 0; i < 2; ++i) {
+    if (!(which & (1 << i))) continue;
+    Direction& d = c->dir[i];
+    cudaError_t e1 = cudaStreamSynchronize(d.kern);
+    cudaError_t e2 = cudaStreamSynchronize(d.copy);
+    if (e1 != cudaSuccess || e2 != cudaSuccess) {
+      c->sticky = MORI_ERR_CUDA;
+      return fail(c, MORI_ERR_CUDA, std::string("asynchronous failure: ") + cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+    }
+    d.idx_used = 0;
+    prof_collect(d);
+  }
+  return c->sticky;
+}
+
+int mori_after_stream(mori_ctx* c, int32_t which, void* stream) {
+  if (!c || which < 1 || which > 3) return MORI_ERR_INVALID_ARG;
+  cudaEvent_t ev = get_event(c, false);
+  CK(c, cudaEventRecord(ev, static_cast<cudaStream_t>(stream)));
+  for (int i = 0; i < 2; ++i)
+    if (which & (1 << i)) {
+      CK(c, cudaStreamWaitEvent(c->dir[i].kern, ev, 0));
+      CK(c, cudaStreamWaitEvent(c->dir[i].copy, ev, 0));
+    }
+  c->free_events.push_back(ev);
+  return MORI_OK;
+}
+
+int mori_stream_wait(mori_ctx* c, void* stream, int32_t which) {
+  if (!c || which < 1 || which > 3) return MORI_ERR_INVALID_ARG;
+  for (int i = 0; i < 2; ++i)
+    if (which & (1 << i))
+      for (cudaStream_t s : {c->dir[i].kern, c->dir[i].copy}) {
+        cudaEvent_t ev = get_event(c, false);
+        CK(c, cudaEventRecord(ev, s));
+        CK(c, cudaStreamWaitEvent(static_cast<cudaStream_t>(stream), ev, 0));
+        c->free_events.push_back(ev);
+      }
+  return MORI_OK;
+}
+
+int mori_profile(mori_ctx* c, int32_t enable) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  c->profiling = enable != 0;
+  return MORI_OK;
+}
+
+int mori_profile_read(mori_ctx* c, int32_t which, double* ms, int64_t* launches, int64_t* bytes) {
+  if (!c || (which != MORI_DEMOTE && which != MORI_PROMOTE)) return MORI_ERR_INVALID_ARG;
+  Direction& d = c->dir[which - 1];
+  if (ms) *ms = d.prof_ms;
+  if (launches) *launches = d.prof_launches;
+  if (bytes) *bytes = d.prof_bytes;
+  d.prof_ms = 0; d.prof_launches = 0; d.prof_bytes = 0;
+  return MORI_OK;
+}
+
+int mori_path(const mori_ctx* c, int32_t which) {
+  if (!c || (which != MORI_DEMOTE && which != MORI_PROMOTE)) return MORI_ERR_INVALID_ARG;
+  return c->dir[which - 1].path;
+}
+
+int mori_copy_kernel(const mori_ctx* c) { return c ? c->copy_kernel : MORI_ERR_INVALID_ARG; }
+
+}  // extern "C"

@@ -1,0 +1,199 @@
+// rank_partition.cuh -- steps a1-a4 of the MORI hot path in ONE launch of ONE CTA (sm_100a).
+//
+// What it computes is declared in include/mori.h (mori_rank_partition): rank by idleness
+// (P:L11, L151-152), prefix-sum the KV footprints, cut at both capacities,
+// label the overflow WAITING and compact the five transition lists.
+//
+// n <= 8192 programs fit one CTA's shared memory as 64-bit (key, index) pairs, so the whole
+// path is latency-bound: one launch, no global atomics, no host round trip.  The sort is a
+// bitonic network over keys padded to a power of two; stages with stride < ITEMS run inside a
+// thread's registers... (kept simple here: every stage is one shared-memory pass).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace mori {
+
+constexpr int kRankMaxN = 8192;
+constexpr int kRankMaxThreads = 1024;
+
+// Order-preserving 32-bit key of a float: canonical NaN last, -0 folded onto +0.
+__device__ __forceinline__ uint32_t idleness_key(float x) {
+  uint32_t b = __float_as_uint(x);
+  if ((b & 0x7FFFFFFFu) > 0x7F800000u) return 0xFFFFFFFFu;  // any NaN
+  if (b == 0x80000000u) b = 0u;                              // -0 == +0
+  return b ^ ((b >> 31) ? 0xFFFFFFFFu : 0x80000000u);
+}
+
+// Exclusive scan of one 64-bit value per thread across the CTA (blockDim.x multiple of 32).
+// `warp_tot` is 33 words of shared memory; returns the exclusive prefix, *total gets the sum.
+__device__ __forceinline__ uint64_t block_excl_scan(uint64_t v, uint64_t* warp_tot, uint64_t* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  uint64_t incl = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    uint64_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+    if (lane >= d) incl += o;
+  }
+  __syncthreads();  // warp_tot may still be read from a previous scan
+  if (lane == 31) warp_tot[warp] = incl;
+  __syncthreads();
+  if (warp == 0) {
+    uint64_t w = lane < n_warps ? warp_tot[lane] : 0;
+    uint64_t wi = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      uint64_t o = __shfl_up_sync(0xFFFFFFFFu, wi, d);
+      if (lane >= d) wi += o;
+    }
+    if (lane < n_warps) warp_tot[lane] = wi - w;  // exclusive warp offsets
+    if (lane == 31) warp_tot[32] = wi;            // grand total
+  }
+  __syncthreads();
+  *total = warp_tot[32];
+  return warp_tot[warp] + incl - v;
+}
+
+// IPT = ranks per thread (n_pad / blockDim.x), blocked: thread t owns ranks [t*IPT, (t+1)*IPT).
+template <int IPT>
+__global__ void __launch_bounds__(kRankMaxThreads, 1)
+rank_partition_kernel(int n, int n_pad, const float* __restrict__ idleness,
+                      const int32_t* __restrict__ kv_pages, const uint8_t* __restrict__ prev_tier,
+                      long long cap_gpu, long long cap_cpu, int32_t* __restrict__ order,
+                      uint8_t* __restrict__ tier, int32_t* __restrict__ bounds,
+                      long long* __restrict__ used, int32_t* __restrict__ lists,
+                      int32_t* __restrict__ list_counts) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n_pad]
+  uint64_t* warp_tot = keys + n_pad;                                 // [33]
+  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
+  const int tid = threadIdx.x, nt = blockDim.x;
+
+  // ---- a1: keys ------------------------------------------------------------------------------
+  for (int i = tid; i < n_pad; i += nt)
+    keys[i] = i < n ? ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i
+                    : 0xFFFFFFFFFFFFFFFFull;                         // padding sorts last
+  __syncthreads();
+
+  // ---- a1: bitonic sort, ascending ------------------------------------------------------------
+  for (int k = 2; k <= n_pad; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int t = tid; t < (n_pad >> 1); t += nt) {
+        const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+        const int p = i | j;
+        const uint64_t a = keys[i], b = keys[p];
+        const bool up = (i & k) == 0;
+        if ((a > b) == up) { keys[i] = b; keys[p] = a; }
+      }
+      __syncthreads();
+    }
+  }
+
+  // ---- a2: footprints in rank order + exclusive prefix sum (int64) ----------------------------
+  int prog[IPT];
+  long long sz[IPT];
+  long long tsum = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    const int r = tid * IPT + i;
+    prog[i] = r < n ? (int)(uint32_t)keys[r] : -1;
+    int s = r < n ? kv_pages[prog[i]] : 0;
+    sz[i] = s > 0 ? s : 0;
+    tsum += sz[i];
+  }
+  uint64_t total_pages;
+  long long run = (long long)block_excl_scan((uint64_t)tsum, warp_tot, &total_pages);
+  long long incl[IPT];
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) { run += sz[i]; incl[i] = run; }
+
+  // ---- a3: GPU boundary: inclusive sums are non-decreasing, so the longest prefix that fits is
+  //          the COUNT of ranks whose inclusive sum is <= capacity ------------------------------
+  int c = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) c += (tid * IPT + i < n) && (incl[i] <= cap_gpu);
+  uint64_t tot;
+  block_excl_scan((uint64_t)c, warp_tot, &tot);
+  const int b_gpu = (int)tot;
+  if (tid == 0) bcast[0] = 0;
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < IPT; ++i)
+    if (tid * IPT + i == b_gpu - 1) bcast[0] = incl[i];              // pages held by the GPU tier
+  __syncthreads();
+  const long long base = bcast[0];
+
+  // ---- a3: CPU boundary, same argument on the sums past the GPU tier --------------------------
+  c = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    const int r = tid * IPT + i;
+    c += (r < n) && (r >= b_gpu) && (incl[i] - base <= cap_cpu);
+  }
+  block_excl_scan((uint64_t)c, warp_tot, &tot);
+  const int b_cpu = b_gpu + (int)tot;
+  if (tid == 0) bcast[1] = base;
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < IPT; ++i)
+    if (tid * IPT + i == b_cpu - 1) bcast[1] = incl[i];
+  __syncthreads();
+  if (tid == 0) {
+    bounds[0] = b_gpu;
+    bounds[1] = b_cpu;
+    used[0] = base;
+    used[1] = bcast[1] - base;
+  }
+
+  // ---- a3/a4: tiers, and the transition class of every rank ------------------------------------
+  // counters packed 16 bits each (n <= 8192 < 65536): demote | promote | drop | admit ; reserve
+  int cls[IPT];
+  uint64_t packed = 0, rsv = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    const int r = tid * IPT + i;
+    cls[i] = -1;
+    if (r < n) {
+      const int now = r < b_gpu ? 0 : (r < b_cpu ? 1 : 2);
+      tier[prog[i]] = (uint8_t)now;
+      order[r] = prog[i];
+      if (prev_tier != nullptr) {
+        const int pv = prev_tier[prog[i]];
+        const int was = pv == 0 ? 0 : (pv == 1 ? 1 : 2);
+        if (was == 0 && now == 1) cls[i] = 0;
+        else if (was == 1 && now == 0) cls[i] = 1;
+        else if (was != 2 && now == 2) cls[i] = 2;
+        else if (was == 2 && now == 0) cls[i] = 3;
+        else if (was == 2 && now == 1) cls[i] = 4;
+        if (cls[i] >= 0 && cls[i] < 4) packed += 1ull << (16 * cls[i]);
+        if (cls[i] == 4) rsv += 1;
+      }
+    }
+  }
+  if (prev_tier == nullptr) return;
+
+  // ---- a4: compaction by rank.  Ascending lists take the exclusive count below; descending
+  //          lists (demote, drop: most idle first) take total - inclusive count ------------------
+  uint64_t ptot, rtot;
+  uint64_t pex = block_excl_scan(packed, warp_tot, &ptot);
+  uint64_t rex = block_excl_scan(rsv, warp_tot, &rtot);
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    const int k = cls[i];
+    if (k < 0) continue;
+    int pos;
+    if (k == 4) {
+      pos = (int)rex++;
+    } else {
+      const int below = (int)((pex >> (16 * k)) & 0xFFFF);
+      pex += 1ull << (16 * k);
+      const int all = (int)((ptot >> (16 * k)) & 0xFFFF);
+      pos = (k == 0 || k == 2) ? all - 1 - below : below;
+    }
+    lists[(size_t)k * n + pos] = prog[i];
+  }
+  if (tid < 4) list_counts[tid] = (int)((ptot >> (16 * tid)) & 0xFFFF);
+  if (tid == 4) list_counts[4] = (int)rtot;
+}
+
+}  // namespace mori

@@ -1,0 +1,158 @@
+"""Drives the CUDA path (through the C ABI binding) over the epochs a ``workload.Sim`` plans.
+
+Used by tests/, bench.py and __graft_entry__.smoke().  Holds the device pool, the pinned arena
+and one libmori context.  No oracle here, no CPU fallback: placement comes from
+``mori_rank_partition`` and bytes move through ``mori_demote`` / ``mori_promote``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import List, Optional
+
+import numpy as np
+import torch
+
+from . import binding
+from . import workload as W
+
+
+class GpuRunner:
+    def __init__(self, cfg: W.Config, seed: int, path_demote=binding.PATH_AUTO,
+                 path_promote=binding.PATH_AUTO, copy_kernel=binding.KERNEL_AUTO,
+                 staging_bytes=0, arena: Optional[torch.Tensor] = None, device="cuda:0"):
+        self.cfg, self.seed = cfg, seed
+        sh = cfg.shape
+        self.dev = torch.device(device)
+        torch.cuda.set_device(self.dev)
+        self.pool = torch.zeros(sh.n_layers * cfg.gpu_pool_pages * sh.chunk_bytes, dtype=torch.uint8,
+                                device=self.dev)
+        arena_bytes = cfg.cpu_pool_pages * sh.page_bytes
+        if arena is None:
+            arena = torch.empty(arena_bytes, dtype=torch.uint8, pin_memory=True)
+        assert arena.numel() >= arena_bytes and arena.is_pinned()
+        self.arena = arena[:arena_bytes]
+        self.mori = binding.Mori(sh.n_layers, sh.n_kv_heads, sh.head_dim, sh.page_tokens, self.pool,
+                                 self.arena, elem_bytes=sh.elem_bytes,
+                                 max_programs=max(1, min(binding.MAX_PROGRAMS, cfg.n_programs)),
+                                 path_demote=path_demote, path_promote=path_promote,
+                                 copy_kernel=copy_kernel, staging_bytes=staging_bytes)
+        n = cfg.n_programs
+        d = self.dev
+        # device-side inputs/outputs of rank_partition + pinned mirrors for the small copies
+        self.d_iota = torch.empty(n, dtype=torch.float32, device=d)
+        self.d_kv = torch.empty(n, dtype=torch.int32, device=d)
+        self.d_prev = torch.empty(n, dtype=torch.uint8, device=d)
+        # one output blob so a single D2H brings everything back:
+        #   order i32[n] | lists i32[5n] | counts i32[5] | bounds i32[2] | pad | used i64[2] | tier u8[n]
+        self._o_order, self._o_lists, self._o_counts = 0, 4 * n, 4 * n + 20 * n
+        self._o_bounds = self._o_counts + 20
+        self._o_used = (self._o_bounds + 8 + 7) // 8 * 8
+        self._o_tier = self._o_used + 16
+        self.d_out = torch.zeros(self._o_tier + n, dtype=torch.uint8, device=d)
+        self.h_out = torch.zeros(self._o_tier + n, dtype=torch.uint8, pin_memory=True)
+        self.h_in = torch.zeros(9 * n, dtype=torch.uint8, pin_memory=True)    # iota | kv | prev
+        self.d_in = torch.zeros(9 * n, dtype=torch.uint8, device=d)
+        self._wl = None
+
+    # -- a1-a4 through the C ABI with HOST inputs and outputs (H2D + kernel + D2H) ---------------
+    def place(self, iota: np.ndarray, kv_pages: np.ndarray, prev_tier: np.ndarray, stream=None):
+        n = self.cfg.n_programs
+        hin = self.h_in.numpy()
+        hin[:4 * n].view(np.float32)[:] = iota
+        hin[4 * n:8 * n].view(np.int32)[:] = kv_pages
+        hin[8 * n:] = prev_tier
+        s = stream or torch.cuda.current_stream()
+        with torch.cuda.stream(s):
+            self.d_in.copy_(self.h_in, non_blocking=True)
+            self._launch_rank(self.d_in, s)
+            self.h_out.copy_(self.d_out, non_blocking=True)
+        s.synchronize()
+        return self._unpack(self.h_out.numpy())
+
+    def _launch_rank(self, d_in, s):
+        n = self.cfg.n_programs
+        base = self.d_out.data_ptr()
+        p = d_in.data_ptr()
+        self.mori._ck(self.mori._lib.mori_rank_partition(
+            self.mori._h, s.cuda_stream, n, p, p + 4 * n, p + 8 * n,
+            self.cfg.cap_gpu_pages, self.cfg.cap_cpu_pages,
+            base + self._o_order, base + self._o_tier, base + self._o_bounds, base + self._o_used,
+            base + self._o_lists, base + self._o_counts))
+
+    def _unpack(self, buf: np.ndarray):
+        n = self.cfg.n_programs
+        counts = buf[self._o_counts:self._o_counts + 20].view(np.int32).copy()
+        lists2d = buf[self._o_lists:self._o_lists + 20 * n].view(np.int32).reshape(5, n)
+        return dict(order=buf[self._o_order:self._o_order + 4 * n].view(np.int32).copy(),
+                    tier=buf[self._o_tier:self._o_tier + n].copy(),
+                    bounds=buf[self._o_bounds:self._o_bounds + 8].view(np.int32).copy(),
+                    used=buf[self._o_used:self._o_used + 16].view(np.int64).copy(),
+                    lists=[lists2d[k, :counts[k]].copy() for k in range(5)])
+
+    # -- a5-a7 ---------------------------------------------------------------------------------
+    def execute(self, plan: W.EpochPlan, sync=True):
+        tickets = {}
+        for op in plan.ops:
+            if op[0] == "demote":
+                tickets[op[1]] = self.mori.mori_demote(op[3], op[4])
+            elif op[0] == "promote":
+                dep = tickets.get(op[5], 0) if op[5] > 0 else 0
+                self.mori.mori_promote(op[3], op[4], wait_demote_ticket=dep)
+            elif op[0] == "sync_all":
+                self.mori.mori_sync(binding.BOTH)
+                tickets.clear()
+        if sync:
+            self.mori.mori_sync(binding.BOTH)
+
+    # -- input generation on the device (workload helper library; not the hot path) ------------
+    def _keys_pages(self, triples):
+        uids = np.concatenate([np.full(len(pg), uid, np.int64) for uid, first, pg in triples])
+        logical = np.concatenate([first + np.arange(len(pg), dtype=np.int64) for uid, first, pg in triples])
+        pages = np.concatenate([np.asarray(pg, np.int32) for uid, first, pg in triples])
+        keys = W.page_keys(self.seed, uids, logical)
+        return (torch.from_numpy(keys.view(np.int64)).to(self.dev),
+                torch.from_numpy(pages).to(self.dev), len(pages))
+
+    def fill(self, fills):
+        """fills = [(uid, first_logical_page, gpu_pages)] -> generated content into the pool."""
+        if not fills:
+            return
+        wl = binding.load_workload_lib()
+        keys, pages, n = self._keys_pages(fills)
+        sh = self.cfg.shape
+        rc = wl.wl_fill_pages(self.pool.data_ptr(), self.cfg.gpu_pool_pages, sh.n_layers, sh.chunk_bytes,
+                              keys.data_ptr(), pages.data_ptr(), n, 0,
+                              torch.cuda.current_stream().cuda_stream)
+        assert rc == 0
+        torch.cuda.current_stream().synchronize()
+
+    def check(self, triples, arena=False) -> int:
+        """Mismatching 32-bit words between resident pages and the generator (device-side check;
+        for ``arena`` the kernel reads the pinned arena through its mapped address)."""
+        if not triples:
+            return 0
+        wl = binding.load_workload_lib()
+        keys, pages, n = self._keys_pages(triples)
+        sh = self.cfg.shape
+        bad = torch.zeros(1, dtype=torch.int64, device=self.dev)
+        buf = self.arena if arena else self.pool
+        P = self.cfg.cpu_pool_pages if arena else self.cfg.gpu_pool_pages
+        rc = wl.wl_check_pages(buf.data_ptr(), P, sh.n_layers, sh.chunk_bytes, keys.data_ptr(),
+                               pages.data_ptr(), n, 1 if arena else 0, bad.data_ptr(),
+                               torch.cuda.current_stream().cuda_stream)
+        assert rc == 0
+        return int(bad.item())
+
+    def resident(self, sim: W.Sim):
+        """(gpu triples, host triples) of every program's resident pages, for check()."""
+        g, h = [], []
+        for p in range(self.cfg.n_programs):
+            uid = int(sim.trace.uid[p])
+            if sim.gpu_pages[p].size:
+                g.append((uid, 0, sim.gpu_pages[p]))
+            if sim.host_slots[p].size:
+                h.append((uid, 0, sim.host_slots[p]))
+        return g, h
+
+    def close(self):
+        self.mori.close()

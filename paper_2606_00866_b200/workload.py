@@ -288,6 +288,13 @@ def page_key(seed: int, uid: int, logical_page: int) -> np.uint64:
     return k[0]
 
 
+def page_keys(seed: int, uids: np.ndarray, logical_pages: np.ndarray) -> np.ndarray:
+    """Vectorised page_key -> uint64[n] (what the device fill/check kernels take)."""
+    with np.errstate(over="ignore"):
+        u = (np.uint64(seed & 0xFFFFFFFF) << np.uint64(32)) ^ (np.asarray(uids).astype(np.uint64) & np.uint64(0xFFFFFFFF))
+        return _splitmix64(_splitmix64(u) ^ np.asarray(logical_pages).astype(np.uint64))
+
+
 def page_content(seed: int, uid: int, logical_page: int, shape: KVShape) -> np.ndarray:
     """uint8 [n_layers, chunk_bytes]: bf16 ~ N(0,1) (Irwin-Hall of 4 hash bytes), 2 values per
     64-bit hash.  Every byte is recomputable from (seed, uid, logical page, layer, offset)."""

@@ -1,0 +1,175 @@
+"""Parity of mori_demote / mori_promote / gather / scatter (CUDA, through the C ABI) with the CPU
+oracle's per-page memcpy: byte-exact pools and arenas, every path and both copy kernels."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_00866_b200 import workload as W
+from paper_2606_00866_b200.harness import GpuRunner
+
+pytestmark = pytest.mark.gpu
+
+PATHS = [1, 2, 3]          # zerocopy, staged, copyengine
+KERNELS = [1, 2]           # ldst, tma
+
+
+def _mk_ctx(mori, L, H, D, T, P, S, path, kernel, staging=0):
+    chunk = 2 * H * T * D * 2
+    g = torch.Generator(device="cpu").manual_seed(P * 31 + S)
+    pool_h = torch.randint(0, 256, (L * P * chunk,), dtype=torch.uint8, generator=g)
+    arena = torch.randint(0, 256, (S * L * chunk,), dtype=torch.uint8, generator=g).pin_memory()
+    pool = pool_h.cuda()
+    m = mori.Mori(L, H, D, T, pool, arena, path_demote=path, path_promote=path, copy_kernel=kernel,
+                  staging_bytes=staging)
+    return m, pool, arena, pool_h.numpy().copy(), arena.numpy().copy(), chunk
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("shape", [(2, 2, 64, 16, 64, 256),        # cfg-1 geometry: 8 KiB chunks
+                                   (5, 8, 128, 16, 300, 200),      # 64 KiB chunks
+                                   (3, 8, 128, 32, 70, 90),        # 128 KiB chunks
+                                   (3, 1, 24, 5, 50, 40)])         # ragged: 960-byte chunks
+def test_demote_then_promote_byte_exact(mori, path, kernel, shape):
+    L, H, D, T, P, S = shape
+    # small staging so that STAGED runs several segments with a ragged last one
+    m, pool, arena, pool_m, arena_m, chunk = _mk_ctx(mori, L, H, D, T, P, S, path, kernel,
+                                                      staging=7 * L * 2 * H * T * D * 2)
+    rng = np.random.default_rng(P)
+    k = min(P, S) // 2 + 3
+    g = rng.permutation(P)[:k].astype(np.int32)
+    h = rng.permutation(S)[:k].astype(np.int32)
+    h[: k // 2] = np.sort(h[: k // 2])                       # some consecutive-slot runs
+    t = m.mori_demote(g, h)
+    assert t > 0
+    m.mori_sync(mori.DEMOTE)
+    oracle.demote(L, chunk, pool_m, arena_m, g, h)
+    assert np.array_equal(arena.numpy(), arena_m), "arena differs after demote"
+    assert np.array_equal(pool.cpu().numpy(), pool_m), "pool changed by demote"
+    g2 = rng.permutation(P)[:k].astype(np.int32)
+    m.mori_promote(h, g2, wait_demote_ticket=t)
+    m.mori_sync(mori.BOTH)
+    oracle.promote(L, chunk, pool_m, arena_m, h, g2)
+    assert np.array_equal(pool.cpu().numpy(), pool_m), "pool differs after promote"
+    assert np.array_equal(arena.numpy(), arena_m), "arena changed by promote"
+    # empty calls are valid no-ops that still issue tickets
+    e = np.zeros(0, np.int32)
+    assert m.mori_demote(e, e) > t
+    assert m.mori_promote(e, e) > 0
+    m.mori_sync(mori.BOTH)
+    assert np.array_equal(pool.cpu().numpy(), pool_m)
+    m.close()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_gather_scatter_device(mori, kernel):
+    L, H, D, T, P = 4, 8, 128, 16, 400
+    m, pool, arena, pool_m, arena_m, chunk = _mk_ctx(mori, L, H, D, T, P, 8, 2, kernel)
+    rng = np.random.default_rng(3)
+    g = rng.permutation(P)[:157].astype(np.int32)
+    gd = torch.from_numpy(g).cuda()
+    stg = torch.zeros(157 * L * chunk, dtype=torch.uint8, device="cuda")
+    m.mori_gather_pages(gd, stg)
+    torch.cuda.synchronize()
+    want = np.zeros(157 * L * chunk, np.uint8)
+    oracle.demote(L, chunk, pool_m, want, g, np.arange(157, dtype=np.int32))
+    assert np.array_equal(stg.cpu().numpy(), want)
+    g2 = rng.permutation(P)[:157].astype(np.int32)
+    m.mori_scatter_pages(torch.from_numpy(g2).cuda(), stg)
+    torch.cuda.synchronize()
+    oracle.promote(L, chunk, pool_m, want, np.arange(157, dtype=np.int32), g2)
+    assert np.array_equal(pool.cpu().numpy(), pool_m)
+    m.mori_gather_pages(gd[:0], stg)           # empty
+    m.close()
+
+
+def test_migration_argument_errors(mori):
+    m, pool, arena, *_ = _mk_ctx(mori, 2, 2, 64, 16, 16, 8, 2, 2)
+    one = np.array([0], np.int32)
+    for g, h in [(np.array([16], np.int32), one), (np.array([-1], np.int32), one),
+                 (one, np.array([8], np.int32)), (one, np.array([-1], np.int32))]:
+        with pytest.raises(mori.MoriError) as e:
+            m.mori_demote(g, h)
+        assert e.value.code == mori.ERR_INVALID_ARG
+        with pytest.raises(mori.MoriError):
+            m.mori_promote(h, g)
+    with pytest.raises(mori.MoriError):
+        m.mori_promote(one, one, wait_demote_ticket=12345)          # never issued
+    with pytest.raises(mori.MoriError):
+        m.mori_sync(0)
+    m.mori_sync(mori.BOTH)
+    m.close()
+    # no arena -> STATE error
+    m2 = mori.Mori(2, 2, 64, 16, pool)
+    with pytest.raises(mori.MoriError) as e:
+        m2.mori_demote(one, one)
+    assert e.value.code == mori.ERR_STATE
+    m2.close()
+
+
+def test_device_fill_matches_numpy_generator(mori):
+    cfg = W.get_config(1)
+    r = GpuRunner(cfg, 866)
+    pages = np.array([5, 0, 63, 17], np.int32)
+    r.fill([(42, 3, pages)])
+    pv = r.pool.cpu().numpy().reshape(cfg.shape.n_layers, cfg.gpu_pool_pages, cfg.shape.chunk_bytes)
+    for j, g in enumerate(pages):
+        assert np.array_equal(pv[:, g], W.page_content(866, 42, 3 + j, cfg.shape))
+    assert r.check([(42, 3, pages)]) == 0
+    assert r.check([(42, 4, pages)]) > 0
+    r.close()
+
+
+def _epochs_with_mirror(mori, cfg, seed, epochs, path, kernel):
+    """Whole epochs: GPU placement must equal the oracle's; the CUDA movers and the oracle's
+    memcpy movers get identical tables; both pools are compared byte for byte every epoch."""
+    sh = cfg.shape
+    sim = W.Sim(cfg, seed)
+    r = GpuRunner(cfg, seed, path_demote=path, path_promote=path, copy_kernel=kernel,
+                  staging_bytes=max(sh.page_bytes * 3, 1 << 20))
+    pool_m = np.zeros(sh.n_layers * cfg.gpu_pool_pages * sh.chunk_bytes, np.uint8)
+    arena_m = np.zeros(cfg.cpu_pool_pages * sh.page_bytes, np.uint8)
+    r.arena.zero_()
+    moved = 0
+    for e in range(epochs):
+        plan = sim.begin_epoch()
+        want = oracle.rank_partition(plan.iota, plan.kv_pages, plan.prev_tier, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+        got = r.place(plan.iota, plan.kv_pages, plan.prev_tier)
+        for k in ("order", "tier", "bounds", "used"):
+            assert np.array_equal(got[k], want[k]), (cfg.name, e, k)
+        for k in range(5):
+            assert np.array_equal(got["lists"][k], want["lists"][k]), (cfg.name, e, k)
+        sim.apply_placement(got["tier"], got["lists"])
+        r.execute(plan)
+        for op in plan.ops:
+            if op[0] == "demote":
+                oracle.demote(sh.n_layers, sh.chunk_bytes, pool_m, arena_m, op[3], op[4])
+            elif op[0] == "promote":
+                oracle.promote(sh.n_layers, sh.chunk_bytes, pool_m, arena_m, op[3], op[4])
+        sim.end_epoch()
+        r.fill(plan.fills)
+        pv = pool_m.reshape(sh.n_layers, cfg.gpu_pool_pages, sh.chunk_bytes)
+        for uid, first, pages in plan.fills:
+            for j, g in enumerate(pages):
+                pv[:, g] = W.page_content(seed, uid, first + j, sh)
+        assert np.array_equal(r.pool.cpu().numpy(), pool_m), (cfg.name, e, "pool")
+        assert np.array_equal(r.arena.numpy(), arena_m), (cfg.name, e, "arena")
+        moved += plan.demote_pages + plan.promote_pages
+    gtri, htri = r.resident(sim)
+    assert r.check(gtri) == 0 and r.check(htri, arena=True) == 0
+    r.close()
+    return moved
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_cfg1_epochs_full_mirror(mori, path):
+    for seed in (866, 867, 868):
+        _epochs_with_mirror(mori, W.get_config(1), seed, 20, path, 2)
+
+
+@pytest.mark.parametrize("idx,scale,epochs", [(2, 64, 25), (3, 64, 15), (4, 64, 12), (5, 64, 8)])
+@pytest.mark.parametrize("path,kernel", [(1, 1), (2, 2)])
+def test_scaled_twins_epochs_full_mirror(mori, idx, scale, epochs, path, kernel):
+    moved = _epochs_with_mirror(mori, W.get_config(idx, scale), 866, epochs, path, kernel)
+    assert moved > 0
