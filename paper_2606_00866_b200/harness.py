@@ -36,6 +36,7 @@ class GpuRunner:
                                  max_programs=max(1, min(binding.MAX_PROGRAMS, cfg.n_programs)),
                                  path_demote=path_demote, path_promote=path_promote,
                                  copy_kernel=copy_kernel, staging_bytes=staging_bytes)
+        self.mori_paths = (self.mori.path_demote, self.mori.path_promote)
         n = cfg.n_programs
         d = self.dev
         # device-side inputs/outputs of rank_partition + pinned mirrors for the small copies
