@@ -1,0 +1,531 @@
+#!/usr/bin/env python
+"""bench.py -- the MORI hot path on B200, measured (driver contract: one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+A *step* is one scheduling epoch: every row of SURVEY.md section 8(a) once --
+``mori_rank_partition`` (a1-a4), ``mori_demote`` / ``mori_promote`` for every program the placement
+moves (a5, a6, concurrently in both link directions) and ``mori_sync`` (a7) -- on the seeded
+synthetic workload of BASELINE.json ``configs[1]`` (cfg 2, Llama-3-8B-shaped KV, 64 programs,
+60 GiB device pool, 128 GiB pinned arena).  Everything on the path runs in
+libmori.so (CUDA, sm_100a) through its C ABI; there is no CPU fallback.
+
+Numbers on the line (DESIGN.md section 7 says how each is derived):
+  value        migrated KV bytes / time of K epochs, GB/s.  The KV pool and the rank/partition
+               inputs are resident in HBM when the timed region starts; timed on the device with
+               CUDA events (region A: rank/partition + read-back of the move lists, region B:
+               all demotes/promotes up to the join).  The page/slot allocator between A and B is
+               harness code (it stands in for the serving engine's allocator) and is not timed.
+  e2e          the same epochs' metric through the public API from HOST buffers: idleness / size /
+               previous-tier arrays copied host->device, lists device->host, host page tables
+               into mori_demote / mori_promote, the allocator included, one timed region.
+  roofline     the gather/scatter kernel of the STAGED path (the only HBM-bound kernel), timed
+               live by the library's CUDA events around every launch inside the timed steps.
+  link         measured pinned-memcpy peaks of this box (denominators) and the achieved fractions.
+  gather_scatter  the device halves alone (pool <-> contiguous device buffer), >= 4 GiB per launch.
+  cpu_baseline the CPU oracle (oracle/, as it stands) on this box's host cores, bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "kv_migration_GBps"
+UNIT = "GB/s"
+SEED = 866
+GIB = 1 << 30
+
+
+# ------------------------------------------------------------------------------------------------
+# helpers
+# ------------------------------------------------------------------------------------------------
+def _mem_available_bytes() -> int:
+    with open("/proc/meminfo") as f:
+        for line in f:
+            if line.startswith("MemAvailable:"):
+                return int(line.split()[1]) * 1024
+    return 0
+
+
+def _pick_scale(cfg_index: int, world: int, W) -> int:
+    """SURVEY 8(d) scale rule: the smallest power of two that lets the pinned arena of every
+    rank fit host RAM (80 % of MemAvailable) and the pool fit HBM."""
+    import torch
+    avail = int(_mem_available_bytes() * 0.80) // max(1, world)
+    free_hbm, _ = torch.cuda.mem_get_info()
+    scale = 1
+    while True:
+        cfg = W.get_config(cfg_index, scale)
+        sh = cfg.shape
+        if (cfg.cpu_pool_pages * sh.page_bytes <= avail
+                and cfg.gpu_pool_pages * sh.page_bytes + (3 << 30) <= free_hbm):
+            return scale
+        scale *= 2
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons every 200 ms while the timed region runs
+    (B200_PROFILING.md 'clocks line')."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for k, name in enumerate(names):
+                if f[3 + k].lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measure_link_peak(arena, nbytes=GIB, reps=5):
+    """Pinned cudaMemcpyAsync of ONE contiguous buffer: D2H alone, H2D alone, both at once on
+    two streams -- the host-link denominators (GB/s).  Uses the first bytes of the arena before
+    the workload touches it, and a scratch device buffer."""
+    import torch
+    nbytes = min(nbytes, arena.numel() // 2)
+    nbytes -= nbytes % 4096
+    h1, h2 = arena[:nbytes], arena[nbytes:2 * nbytes]
+    d1 = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    d2 = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+
+    def run(do_d2h, do_h2d):
+        best = float("inf")
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            cur = torch.cuda.current_stream()
+            e0 = torch.cuda.Event(enable_timing=True); e0.record(cur)
+            s1.wait_event(e0); s2.wait_event(e0)
+            if do_d2h:
+                with torch.cuda.stream(s1):
+                    h1.copy_(d1, non_blocking=True)
+            if do_h2d:
+                with torch.cuda.stream(s2):
+                    d2.copy_(h2, non_blocking=True)
+            cur.wait_stream(s1); cur.wait_stream(s2)
+            e1 = torch.cuda.Event(enable_timing=True); e1.record(cur)
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+            del ev
+        return best * 1e-3
+
+    out = {"bytes": nbytes,
+           "d2h": nbytes / run(True, False) / 1e9,
+           "h2d": nbytes / run(False, True) / 1e9,
+           "bidir_sum": 2 * nbytes / run(True, True) / 1e9}
+    del d1, d2
+    return out
+
+
+def ideal_seconds(dem_bytes, pro_bytes, link):
+    """Lower bound on an epoch's transfer time from the measured pinned-memcpy peaks."""
+    return max(dem_bytes / (link["d2h"] * 1e9), pro_bytes / (link["h2d"] * 1e9),
+               (dem_bytes + pro_bytes) / (link["bidir_sum"] * 1e9))
+
+
+# ------------------------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline, --impl reference): the only places bench.py touches oracle/
+# ------------------------------------------------------------------------------------------------
+class OracleEpochs:
+    """The oracle as it stands on a scaled twin of the bench workload (same L/H/D/T/n, pools and
+    contexts divided by ``scale`` so that byte mirrors of both pools fit host RAM)."""
+
+    def __init__(self, cfg_index: int, scale: int, seed: int):
+        import oracle
+        from paper_2606_00866_b200 import workload as W
+        self.oracle, self.W = oracle, W
+        oracle.build()
+        self.cfg = W.get_config(cfg_index, scale)
+        sh = self.cfg.shape
+        self.sim = W.Sim(self.cfg, seed)
+        rng = np.random.default_rng(seed)
+        self.pool = rng.integers(0, 256, sh.n_layers * self.cfg.gpu_pool_pages * sh.chunk_bytes, dtype=np.uint8)
+        self.arena = np.zeros(self.cfg.cpu_pool_pages * sh.page_bytes, np.uint8)
+        self.arena[::4096] = 1                       # touch every page before timing
+
+    def step(self):
+        """One epoch.  -> (seconds in the oracle, bytes migrated)."""
+        cfg, sh, o = self.cfg, self.cfg.shape, self.oracle
+        plan = self.sim.begin_epoch()
+        t0 = time.perf_counter()
+        res = o.rank_partition(plan.iota, plan.kv_pages, plan.prev_tier, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+        t = time.perf_counter() - t0
+        self.sim.apply_placement(res["tier"], res["lists"])
+        t0 = time.perf_counter()
+        for op in plan.ops:
+            if op[0] == "demote":
+                o.demote(sh.n_layers, sh.chunk_bytes, self.pool, self.arena, op[3], op[4])
+            elif op[0] == "promote":
+                o.promote(sh.n_layers, sh.chunk_bytes, self.pool, self.arena, op[3], op[4])
+        t += time.perf_counter() - t0
+        self.sim.end_epoch()                         # page contents are irrelevant to the timing
+        return t, (plan.demote_pages + plan.promote_pages) * sh.page_bytes
+
+
+def cpu_baseline(cfg_index: int, budget_s: float = 12.0, scale: int = 16):
+    oe = OracleEpochs(cfg_index, scale, SEED)
+    for _ in range(3):
+        oe.step()
+    t_sum, b_sum, n = 0.0, 0, 0
+    t_wall = time.perf_counter()
+    while (time.perf_counter() - t_wall < budget_s and n < oe.cfg.epochs - 3) or n < 3:
+        t, b = oe.step()
+        t_sum += t; b_sum += b; n += 1
+    return {"value": b_sum / t_sum / 1e9 if t_sum > 0 else 0.0, "unit": UNIT, "cores": 1,
+            "host_cores_available": os.cpu_count(), "kind": "oracle",
+            "sample": f"{n} epochs of {oe.cfg.name} (cfg {cfg_index} with pools and contexts / {scale}, "
+                      f"same L/H/D/T/n), {b_sum / GIB:.1f} GiB migrated host->host by oracle.c "
+                      f"(qsort + prefix loop + per-(page,layer) memcpy, single thread)"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scale = 16
+    oe = OracleEpochs(args.config, scale, SEED)
+    for _ in range(args.warmup):
+        oe.step()
+    t_sum, b_sum = 0.0, 0
+    for _ in range(args.steps):
+        t, b = oe.step()
+        t_sum += t; b_sum += b
+    v = b_sum / t_sum / 1e9 if t_sum > 0 else 0.0
+    sample = (f"{args.steps} epochs of {oe.cfg.name} (pools and contexts / {scale}), "
+              f"{b_sum / GIB:.1f} GiB migrated host->host, single thread")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_sum / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
+        "data": "synthetic", "config": {"workload": oe.cfg.name, "scale": scale},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_00866_b200 import binding, replicas, workload as W
+    from paper_2606_00866_b200.harness import GpuRunner
+
+    rank, world, local = replicas.env_rank()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    scale = args.scale or _pick_scale(args.config, world, W)
+    cfg = W.get_config(args.config, scale)
+    sh = cfg.shape
+    seed = replicas.replica_seed(SEED, rank)
+    t_setup = time.perf_counter()
+    arena = binding.Mori.mori_host_alloc(cfg.cpu_pool_pages * sh.page_bytes)
+    link = measure_link_peak(arena)
+    paths = {"auto": 0, "zerocopy": 1, "staged": 2, "copyengine": 3}
+    r = GpuRunner(cfg, seed, arena=arena, staging_bytes=args.staging_mib << 20,
+                  path_demote=paths[args.path_demote], path_promote=paths[args.path_promote],
+                  copy_kernel={"auto": 0, "ldst": 1, "tma": 2}[args.kernel])
+    kernel_name = binding.KERNEL_NAMES[r.mori.copy_kernel]
+    sim = W.Sim(cfg, seed)
+    t_setup = time.perf_counter() - t_setup
+    cur = torch.cuda.current_stream()
+    page_b = sh.page_bytes
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    def epoch(mode):
+        """One step.  mode 'dev': inputs resident, regions A+B timed; 'e2e': host buffers, one
+        region.  -> dict(ms, dem, pro, h2d, d2h)."""
+        plan = sim.begin_epoch()                                   # input generation (host)
+        n = cfg.n_programs
+        if mode == "dev":
+            r.upload_inputs(plan.iota, plan.kv_pages, plan.prev_tier)
+            torch.cuda.synchronize()
+            a0, a1, b0, b1 = ev(), ev(), ev(), ev()
+            a0.record(cur)
+            got = r.place_resident(cur)                            # kernel + D2H of lists + sync
+            a1.record(cur)
+            sim.apply_placement(got["tier"], got["lists"])         # harness allocator (untimed)
+            b0.record(cur)
+            r.mori.mori_after_stream(binding.BOTH, cur)
+            r.execute(plan, sync=False)
+            r.mori.mori_stream_wait(cur, binding.BOTH)
+            b1.record(cur)
+            r.mori.mori_sync(binding.BOTH)
+            torch.cuda.synchronize()
+            ms = a0.elapsed_time(a1) + b0.elapsed_time(b1)
+        else:
+            torch.cuda.synchronize()
+            e0, e1 = ev(), ev()
+            e0.record(cur)
+            r.mori.mori_after_stream(binding.BOTH, cur)
+            got = r.place(plan.iota, plan.kv_pages, plan.prev_tier, stream=cur)
+            sim.apply_placement(got["tier"], got["lists"])
+            r.execute(plan, sync=False)
+            r.mori.mori_stream_wait(cur, binding.BOTH)
+            e1.record(cur)
+            r.mori.mori_sync(binding.BOTH)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+        sim.end_epoch()
+        r.fill(plan.fills)                                          # stands in for prefill (untimed)
+        n_tab = 8 * (plan.demote_pages + plan.promote_pages)        # page + slot ids, int32 each
+        return dict(ms=ms, dem=plan.demote_pages * page_b, pro=plan.promote_pages * page_b,
+                    h2d=plan.promote_pages * page_b + 9 * n + n_tab,
+                    d2h=plan.demote_pages * page_b + r.h_out.numel())
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        epoch("dev")
+    # ---- timed: K steps, device-resident inputs ---------------------------------------------------
+    r.mori.mori_profile(True)
+    r.mori.mori_profile_read(binding.DEMOTE); r.mori.mori_profile_read(binding.PROMOTE)
+    clocks = ClockSampler(local)
+    barrier()
+    clocks.start()
+    l0 = r.mori.mori_launch_count()
+    steps = [epoch("dev") for _ in range(args.steps)]
+    barrier()
+    launches = r.mori.mori_launch_count() - l0
+    clk = clocks.stop()
+    prof = {"demote": r.mori.mori_profile_read(binding.DEMOTE),
+            "promote": r.mori.mori_profile_read(binding.PROMOTE)}
+    r.mori.mori_profile(False)
+    # ---- timed: K steps through the public API from host buffers -----------------------------------
+    barrier()
+    steps_e2e = [epoch("e2e") for _ in range(args.steps)]
+    barrier()
+
+    def total(st, k):
+        return float(sum(s[k] for s in st))
+
+    t_dev, t_e2e = total(steps, "ms") * 1e-3, total(steps_e2e, "ms") * 1e-3
+    b_dev = total(steps, "dem") + total(steps, "pro")
+    b_e2e = total(steps_e2e, "dem") + total(steps_e2e, "pro")
+    (t_dev, t_e2e), (b_dev, b_e2e, launches) = replicas.aggregate(
+        [t_dev, t_e2e], [b_dev, b_e2e, float(launches)], device="cuda")
+    value = b_dev / t_dev / 1e9 if t_dev > 0 else 0.0
+    value_e2e = b_e2e / t_e2e / 1e9 if t_e2e > 0 else 0.0
+
+    # ---- link fractions (rank 0's own steps against rank 0's own measured peaks) -------------------
+    def link_report(st):
+        ideal = sum(ideal_seconds(s["dem"], s["pro"], link) for s in st)
+        meas = sum(s["ms"] for s in st) * 1e-3
+        out = {"frac_of_measured_link_peak": ideal / meas if meas > 0 else None}
+        for name, sel in (("demote_only", lambda s: s["dem"] > 0 and s["pro"] == 0),
+                          ("promote_only", lambda s: s["pro"] > 0 and s["dem"] == 0),
+                          ("bidirectional", lambda s: s["pro"] > 0 and s["dem"] > 0)):
+            sub = [s for s in st if sel(s)]
+            if sub:
+                byt = sum(s["dem"] + s["pro"] for s in sub)
+                sec = sum(s["ms"] for s in sub) * 1e-3
+                peak = {"demote_only": link["d2h"], "promote_only": link["h2d"]}.get(name)
+                ent = {"steps": len(sub), "GBps": byt / sec / 1e9, "GiB": byt / GIB}
+                ent["frac"] = (ent["GBps"] / peak) if peak else \
+                    sum(ideal_seconds(s["dem"], s["pro"], link) for s in sub) / sec
+                out[name] = ent
+        return out
+
+    # ---- roofline of the HBM-bound kernel, from the library's per-launch CUDA events ---------------
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        hbm_peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    else:
+        hbm_peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
+    k_ms = prof["demote"][0] + prof["promote"][0]
+    k_n = prof["demote"][1] + prof["promote"][1]
+    k_b = prof["demote"][2] + prof["promote"][2]
+    staged = binding.PATH_STAGED in r.mori_paths
+    roofline = None
+    if staged and k_ms > 0:
+        ach = 2.0 * k_b / (k_ms * 1e-3) / 1e9                     # read + write, per DESIGN.md 5
+        roofline = {"bound": "hbm", "kernel": f"copy_pages_{binding.KERNEL_NAMES[r.mori.copy_kernel]}"
+                                              " (gather/scatter of the STAGED path, inside the timed steps)",
+                    "achieved": ach, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s",
+                    "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC.get("bytes_per_launch"),
+                    "traffic_source": NCU_TRAFFIC.get("source"),
+                    "launches": k_n, "avg_launch_us": 1e3 * k_ms / k_n,
+                    "algorithmic_bytes_per_launch": 2.0 * k_b / k_n}
+
+    # ---- the device halves alone: pool <-> contiguous device buffer, >= 4 GiB per launch ------------
+    gs = None
+    if rank == 0 and not args.no_gather_leg:
+        gs = gather_scatter_leg(r, sim, hbm_peak)
+        if roofline is None and gs:
+            roofline = {"bound": "hbm", "kernel": gs["kernel"] + " (standalone gather launches)",
+                        "achieved": gs["gather_GBps"], "peak": hbm_peak, "peak_source": peak_src,
+                        "unit": "GB/s", "frac": gs["gather_GBps"] / hbm_peak,
+                        "traffic": NCU_TRAFFIC.get("bytes_per_launch"),
+                        "traffic_source": NCU_TRAFFIC.get("source")}
+
+    r.close()
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(args.config)
+    if rank == 0:
+        K = args.steps
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_dev / K, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": cfg.name, "bj_config": f"configs[{args.config - 1}]", "scale": scale,
+                       "n_programs": cfg.n_programs, "gpu_pool_GiB": cfg.gpu_pool_pages * page_b / GIB,
+                       "host_arena_GiB": cfg.cpu_pool_pages * page_b / GIB,
+                       "page_bytes": page_b, "chunk_bytes": sh.chunk_bytes,
+                       "parallelism": f"replicas x{world} (no data-path collective)",
+                       "path_demote": binding.PATH_NAMES[r.mori_paths[0]],
+                       "path_promote": binding.PATH_NAMES[r.mori_paths[1]],
+                       "copy_kernel": kernel_name,
+                       "staging_MiB": args.staging_mib,
+                       "l2": "inputs larger than L2 (GiB per step vs 126 MB); no flush needed",
+                       "migrated_GiB": b_dev / GIB, "setup_s": t_setup},
+            "clocks": clk,
+            "e2e": {"value": value_e2e, "unit": UNIT,
+                    "h2d_bytes_per_step": total(steps_e2e, "h2d") / K,
+                    "d2h_bytes_per_step": total(steps_e2e, "d2h") / K,
+                    "ms_per_step": 1e3 * t_e2e / K, "migrated_GiB": b_e2e / GIB,
+                    "link": link_report(steps_e2e)},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "link": dict(link_report(steps), peaks_GBps=link,
+                         peak_how="pinned cudaMemcpyAsync of one contiguous 1 GiB buffer, best of 5, "
+                                  "measured in this process before the run"),
+            "gather_scatter": gs,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    binding.Mori.mori_host_free(arena)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the gather kernel from the committed
+# ncu --set full capture (profiles/); filled in once that capture exists.
+NCU_TRAFFIC: dict = {}
+
+
+def gather_scatter_leg(r, sim, hbm_peak, min_bytes=4 * GIB, reps=20, warm=3):
+    """mori_gather_pages / mori_scatter_pages on the page tables the workload has produced
+    (resident GPU-tier programs, in table order), padded with the remaining pool pages in
+    allocator order up to >= 4 GiB: one launch, CUDA events on the launching stream."""
+    import torch
+    from paper_2606_00866_b200 import binding
+    cfg, sh = r.cfg, r.cfg.shape
+    pages = [p for p in sim.gpu_pages if p.size]
+    used = np.concatenate(pages) if pages else np.zeros(0, np.int32)
+    want = -(-min_bytes // sh.page_bytes)
+    if used.size < want:
+        rest = np.setdiff1d(np.arange(cfg.gpu_pool_pages, dtype=np.int32), used)
+        used = np.concatenate([used, rest[:want - used.size]])
+    used = used[:max(want, 1)].astype(np.int32)
+    free, _ = torch.cuda.mem_get_info()
+    n = int(min(used.size, (free - GIB) // sh.page_bytes))
+    if n <= 0:
+        return None
+    used = used[:n]
+    gd = torch.from_numpy(used).cuda()
+    buf = torch.empty(n * sh.page_bytes, dtype=torch.uint8, device="cuda")
+    cur = torch.cuda.current_stream()
+    out = {"pages": n, "GiB_per_launch": n * sh.page_bytes / GIB,
+           "kernel": f"copy_pages_{binding.KERNEL_NAMES[r.mori.copy_kernel]}",
+           "contiguous_runs_mean_pages": float(n / max(1, 1 + np.count_nonzero(np.diff(used) != 1)))}
+    for name, fn in (("gather", lambda: r.mori.mori_gather_pages(gd, buf, stream=cur)),
+                     ("scatter", lambda: r.mori.mori_scatter_pages(gd, buf, stream=cur))):
+        for _ in range(warm):
+            fn()
+        ts = []
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(cur); fn(); e1.record(cur)
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        byt = 2.0 * n * sh.page_bytes
+        out[f"{name}_GBps"] = byt / float(np.median(ts)) / 1e9
+        out[f"{name}_GBps_best"] = byt / min(ts) / 1e9
+        out[f"{name}_frac_of_measured_hbm"] = out[f"{name}_GBps"] / hbm_peak
+        out[f"{name}_frac_of_8TBps_spec"] = out[f"{name}_GBps"] / 8000.0
+    del buf
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=24)
+    ap.add_argument("--warmup", type=int, default=4)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based")
+    ap.add_argument("--scale", type=int, default=0, help="0 = auto (1 when the pools fit)")
+    ap.add_argument("--path-demote", default="auto", choices=["auto", "zerocopy", "staged", "copyengine"])
+    ap.add_argument("--path-promote", default="auto", choices=["auto", "zerocopy", "staged", "copyengine"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "ldst", "tma"])
+    ap.add_argument("--staging-mib", type=int, default=0, help="0 = library default")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-gather-leg", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -177,6 +177,17 @@ int mori_profile(mori_ctx* ctx, int32_t enable);
 int mori_profile_read(mori_ctx* ctx, int32_t which, double* kernel_ms, int64_t* launches,
                       int64_t* bytes);
 
+/* Number of CUDA kernels this context has launched since mori_create (rank/partition, index
+ * upload, gather/scatter/zero-copy kernels); copy-engine DMAs are not kernels and not counted. */
+int mori_launch_count(const mori_ctx* ctx, int64_t* out);
+
+/* PINNED host memory for an arena when the caller has no allocator of its own: page-locked,
+ * mapped into the device address space, exactly `bytes` long (no rounding), 4 KiB aligned.
+ * *out is NULL on failure (MORI_ERR_CUDA; mori_last_error(NULL) says why).  Free with
+ * mori_host_free, after destroying every context that uses it. */
+int mori_host_alloc(int64_t bytes, void** out);
+int mori_host_free(void* p);
+
 /* Resolved MORI_PATH_* for a direction (after AUTO), and resolved MORI_KERNEL_*. */
 int mori_path(const mori_ctx* ctx, int32_t which);
 int mori_copy_kernel(const mori_ctx* ctx);

@@ -28,7 +28,8 @@ KERNEL_NAMES = {1: "ldst", 2: "tma"}
 EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", "mori_promote",
            "mori_sync", "mori_after_stream", "mori_stream_wait", "mori_gather_pages",
            "mori_scatter_pages", "mori_profile", "mori_profile_read", "mori_path",
-           "mori_copy_kernel", "mori_last_error"]
+           "mori_copy_kernel", "mori_last_error", "mori_launch_count", "mori_host_alloc",
+           "mori_host_free"]
 
 
 class MoriConfig(C.Structure):
@@ -74,6 +75,9 @@ def load():
         L.mori_path.argtypes = [vp, i32]
         L.mori_copy_kernel.argtypes = [vp]
         L.mori_last_error.argtypes = [vp]
+        L.mori_launch_count.argtypes = [vp, C.POINTER(i64)]
+        L.mori_host_alloc.argtypes = [i64, C.POINTER(vp)]
+        L.mori_host_free.argtypes = [vp]
         L.mori_last_error.restype = C.c_char_p
         for name in EXPORTS:
             if name != "mori_last_error":
@@ -215,7 +219,36 @@ class Mori:
         return self._ck(self._lib.mori_scatter_pages(self._h, _stream_handle(stream),
                                                      gpu_pages_dev.numel(), _ptr(gpu_pages_dev), _ptr(src)))
 
+    # -- pinned host memory ------------------------------------------------------------------
+    @staticmethod
+    def mori_host_alloc(nbytes: int):
+        """-> uint8 torch tensor over ``nbytes`` of pinned, device-mapped host memory (exact size,
+        unlike torch's pinned allocator which rounds up to a power of two).  Free it with
+        ``mori_host_free(t)`` after closing every context that uses it."""
+        import torch
+        lib = load()
+        p = C.c_void_p()
+        rc = lib.mori_host_alloc(int(nbytes), C.byref(p))
+        if rc != OK:
+            raise MoriError(rc, (lib.mori_last_error(None) or b"").decode())
+        t = torch.frombuffer((C.c_uint8 * int(nbytes)).from_address(p.value), dtype=torch.uint8)
+        t._mori_host_ptr = p.value
+        return t
+
+    @staticmethod
+    def mori_host_free(t):
+        p = getattr(t, "_mori_host_ptr", None)
+        if p:
+            t._mori_host_ptr = None
+            return load().mori_host_free(p)
+        return OK
+
     # -- profiling ---------------------------------------------------------------------------
+    def mori_launch_count(self) -> int:
+        n = C.c_int64(0)
+        self._ck(self._lib.mori_launch_count(self._h, C.byref(n)))
+        return n.value
+
     def mori_profile(self, enable: bool):
         return self._ck(self._lib.mori_profile(self._h, int(enable)))
 

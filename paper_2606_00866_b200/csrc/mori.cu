@@ -52,6 +52,7 @@ struct mori_ctx {
   Direction dir[2];                              // 0 demote, 1 promote
   std::vector<cudaEvent_t> free_events;
   bool profiling = false;
+  mutable long long launches = 0;                // kernels launched by this context
   int sticky = MORI_OK;
   mutable std::string err;
 };
@@ -101,6 +102,7 @@ template <bool kGather>
 cudaError_t launch_copy(const mori_ctx* c, const mori::CopyArgs& a, cudaStream_t s, bool link) {
   const long long n_pieces = a.n_pages * a.n_layers * a.pieces_per_chunk;
   if (n_pieces == 0) return cudaSuccess;
+  c->launches += 1;
   if (c->copy_kernel == MORI_KERNEL_TMA) {
     const long long max_grid = link ? 32 : c->sm_count;          // 1 CTA per SM (smem-bound)
     const int grid = (int)std::min<long long>(n_pieces, max_grid);
@@ -146,6 +148,7 @@ int stage_indices(mori_ctx* c, Direction& d, long long n, const int32_t* a0, con
   const int grid = (int)std::min<long long>((2 * n + 255) / 256, 64);
   upload_idx_kernel<<<grid, 256, 0, d.kern>>>(d.idx_host_dev + d.idx_used, d.idx_dev + d.idx_used, 2 * n);
   CK(c, cudaGetLastError());
+  c->launches += 1;
   *d0 = d.idx_dev + d.idx_used;
   *d1 = d.idx_dev + d.idx_used + n;
   d.idx_used += 2 * n;
@@ -347,6 +350,7 @@ int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idlen
   }
 #undef LR
   CK(c, e);
+  c->launches += 1;
   return MORI_OK;
 }
 
@@ -537,6 +541,30 @@ int mori_profile_read(mori_ctx* c, int32_t which, double* ms, int64_t* launches,
   if (bytes) *bytes = d.prof_bytes;
   d.prof_ms = 0; d.prof_launches = 0; d.prof_bytes = 0;
   return MORI_OK;
+}
+
+int mori_launch_count(const mori_ctx* c, int64_t* out) {
+  if (!c || !out) return MORI_ERR_INVALID_ARG;
+  *out = c->launches;
+  return MORI_OK;
+}
+
+int mori_host_alloc(int64_t bytes, void** out) {
+  if (out) *out = nullptr;
+  if (!out || bytes <= 0) return fail(nullptr, MORI_ERR_INVALID_ARG, "mori_host_alloc: bad arguments");
+  void* p = nullptr;
+  cudaError_t e = cudaHostAlloc(&p, (size_t)bytes, cudaHostAllocMapped | cudaHostAllocPortable);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, MORI_ERR_CUDA, std::string("cudaHostAlloc: ") + cudaGetErrorString(e));
+  }
+  *out = p;
+  return MORI_OK;
+}
+
+int mori_host_free(void* p) {
+  if (!p) return MORI_OK;
+  return cudaFreeHost(p) == cudaSuccess ? MORI_OK : MORI_ERR_CUDA;
 }
 
 int mori_path(const mori_ctx* c, int32_t which) {
