@@ -349,6 +349,11 @@ def run_ours(args):
             "promote": r.mori.mori_profile_read(binding.PROMOTE)}
     r.mori.mori_profile(False)
     # ---- timed: K steps through the public API from host buffers -----------------------------------
+    # the SAME epochs again (the trace and the placement are deterministic in the seed), so that
+    # `e2e` and `value` move identical bytes: fresh Sim, W untimed epochs, then K timed ones
+    sim = W.Sim(cfg, seed)
+    for _ in range(args.warmup):
+        epoch("e2e")
     barrier()
     steps_e2e = [epoch("e2e") for _ in range(args.steps)]
     barrier()

@@ -76,7 +76,7 @@ typedef struct {
   int32_t path_demote;       /* MORI_PATH_* */
   int32_t path_promote;      /* MORI_PATH_* */
   int32_t copy_kernel;       /* MORI_KERNEL_* */
-  int64_t staging_bytes;     /* per staging buffer (2 per direction); 0 -> 128 MiB */
+  int64_t staging_bytes;     /* per staging buffer (2 per direction); 0 -> 1 GiB */
   int64_t max_pages_per_call;/* 0 -> max(gpu_pool_pages, host_arena_slots) */
 } mori_config;
 

@@ -226,6 +226,7 @@ class Mori:
         unlike torch's pinned allocator which rounds up to a power of two).  Free it with
         ``mori_host_free(t)`` after closing every context that uses it."""
         import torch
+        torch.cuda.init()            # is_pinned() answers False before torch's lazy CUDA init
         lib = load()
         p = C.c_void_p()
         rc = lib.mori_host_alloc(int(nbytes), C.byref(p))

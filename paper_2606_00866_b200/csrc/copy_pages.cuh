@@ -15,10 +15,11 @@
 // consecutive addresses of one chunk (DRAM page locality on both sides).
 //
 // Two implementations:
-//   copy_pages_tma   one thread per CTA drives the SM's bulk-copy engine: cp.async.bulk
-//                    global->shared (mbarrier complete_tx) into a ring of stages, then
-//                    cp.async.bulk shared->global (bulk_group).  No registers, no LSU
-//                    instructions per byte; ~150 KiB of loads in flight per SM.
+//   copy_pages_tma   two threads per CTA drive the SM's bulk-copy engine: a loader issues
+//                    cp.async.bulk global->shared (mbarrier complete_tx) into a ring of stages,
+//                    a storer issues cp.async.bulk shared->global (bulk_group) and hands stages
+//                    back.  No registers, no LSU instructions per byte; up to 192 KiB of the
+//                    ring in flight per SM.
 //   copy_pages_ldst  256 threads, 4 x 16-byte ld.global.nc.L1::no_allocate per thread issued
 //                    before the 4 st.global: 16 KiB in flight per CTA, 8 CTAs per SM.
 #pragma once
@@ -139,52 +140,84 @@ __device__ __forceinline__ void bulk_wait_read() {
 }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-constexpr int kTmaThreads = 32;
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(bar)) : "memory");
+}
+
+constexpr int kTmaThreads = 64;   // warp 0 lane 0 = load issuer, warp 1 lane 0 = store issuer
 constexpr int kTmaStoreLag = 2;   // stores allowed to be still reading shared memory
 
-// Shared memory: kStages stage buffers of a.piece_bytes each, then kStages mbarriers.
-// Lane 0 runs the whole pipeline; loads run (kStages - kTmaStoreLag) pieces ahead of stores.
+// Addresses of chunk w = (page k, layer l): one page-table load and one division per CHUNK;
+// the pieces of a chunk are consecutive on both sides.
+template <bool kGather>
+__device__ __forceinline__ void chunk_addresses(const CopyArgs& a, long long w, const unsigned char*& src,
+                                                unsigned char*& dst) {
+  const long long k = w / a.n_layers;
+  const int l = (int)(w - k * a.n_layers);
+  const long long g = a.gpu_pages[k];
+  const long long e = a.lin_idx ? (long long)a.lin_idx[k] : k;
+  unsigned char* pp = a.pool + ((long long)l * a.pool_pages + g) * a.chunk_bytes;
+  unsigned char* lp = a.lin + (e * a.n_layers + l) * a.chunk_bytes;
+  if (kGather) { src = pp; dst = lp; } else { src = lp; dst = pp; }
+}
+
+// Shared memory: kStages stage buffers of a.piece_bytes each, then kStages "full" and kStages
+// "empty" mbarriers.  Two single-thread roles so that neither waits for the other's latency:
+//   loader  (warp 0): for every piece, wait until its stage is empty, expect_tx + bulk load;
+//   storer  (warp 1): wait until the stage is full, bulk store, commit; once the store issued
+//                     kTmaStoreLag groups ago has finished READING shared memory, hand its
+//                     stage back to the loader.
+// CTA b takes chunks b, b + grid, ...; every CTA walks the same piece sequence in both roles.
 template <bool kGather, int kStages>
 __global__ void __launch_bounds__(kTmaThreads, 1) copy_pages_tma(const CopyArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * a.piece_bytes);
-  if (threadIdx.x != 0) return;
-  for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-
-  const long long n_pieces = a.n_pages * a.n_layers * a.pieces_per_chunk;
-  const long long first = blockIdx.x, step = gridDim.x;
-  if (first >= n_pieces) return;
-  const long long n_mine = (n_pieces - first + step - 1) / step;
-  constexpr int kAhead = kStages - kTmaStoreLag;
-
-  long long i_load = 0;
-  auto issue_load = [&](long long i) {
-    const unsigned char* src; unsigned char* dst; int bytes;
-    piece_addresses<kGather>(a, first + i * step, src, dst, bytes);
-    const int st = (int)(i % kStages);
-    mbar_expect_tx(&full[st], (uint32_t)bytes);
-    bulk_g2s(smem + (size_t)st * a.piece_bytes, src, (uint32_t)bytes, &full[st]);
-  };
-  for (; i_load < n_mine && i_load < kAhead; ++i_load) issue_load(i_load);
-
-  for (long long i = 0; i < n_mine; ++i) {
-    const int st = (int)(i % kStages);
-    const uint32_t parity = (uint32_t)((i / kStages) & 1);
-    const unsigned char* src; unsigned char* dst; int bytes;
-    piece_addresses<kGather>(a, first + i * step, src, dst, bytes);
-    mbar_wait(&full[st], parity);
-    bulk_s2g(dst, smem + (size_t)st * a.piece_bytes, (uint32_t)bytes);
-    bulk_commit();
-    if (i_load < n_mine) {
-      // the stage piece i_load lands in was last read by the store of piece i_load - kStages
-      // = i - kTmaStoreLag: every group but the newest kTmaStoreLag must have finished reading
-      bulk_wait_read<kTmaStoreLag>();
-      issue_load(i_load);
-      ++i_load;
-    }
+  uint64_t* empty = full + kStages;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  bulk_wait_all();   // writes complete before the CTA exits
+  __syncthreads();
+  if ((threadIdx.x & 31) != 0) return;
+  const long long n_chunks = a.n_pages * a.n_layers;
+  const int ppc = a.pieces_per_chunk;
+
+  if (threadIdx.x == 0) {
+    // ---------------- loader ----------------
+    long long i = 0;
+    for (long long w = blockIdx.x; w < n_chunks; w += gridDim.x) {
+      const unsigned char* src; unsigned char* dst;
+      chunk_addresses<kGather>(a, w, src, dst);
+      for (int c = 0; c < ppc; ++c, ++i) {
+        const int off = c * a.piece_bytes;
+        const uint32_t bytes = (uint32_t)min(a.piece_bytes, a.chunk_bytes - off);
+        const int st = (int)(i % kStages);
+        if (i >= kStages) mbar_wait(&empty[st], (uint32_t)(((i / kStages) - 1) & 1));
+        mbar_expect_tx(&full[st], bytes);
+        bulk_g2s(smem + (size_t)st * a.piece_bytes, src + off, bytes, &full[st]);
+      }
+    }
+  } else {
+    // ---------------- storer ----------------
+    long long i = 0;
+    for (long long w = blockIdx.x; w < n_chunks; w += gridDim.x) {
+      const unsigned char* src; unsigned char* dst;
+      chunk_addresses<kGather>(a, w, src, dst);
+      for (int c = 0; c < ppc; ++c, ++i) {
+        const int off = c * a.piece_bytes;
+        const uint32_t bytes = (uint32_t)min(a.piece_bytes, a.chunk_bytes - off);
+        const int st = (int)(i % kStages);
+        mbar_wait(&full[st], (uint32_t)((i / kStages) & 1));
+        bulk_s2g(dst + off, smem + (size_t)st * a.piece_bytes, bytes);
+        bulk_commit();
+        if (i >= kTmaStoreLag) {
+          bulk_wait_read<kTmaStoreLag>();                       // group i - lag has left shared memory
+          mbar_arrive(&empty[(int)((i - kTmaStoreLag) % kStages)]);
+        }
+      }
+    }
+    bulk_wait_all();   // writes complete before the CTA exits
+  }
 }
 
 }  // namespace mori

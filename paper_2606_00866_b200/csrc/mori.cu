@@ -105,7 +105,7 @@ cudaError_t launch_copy(const mori_ctx* c, const mori::CopyArgs& a, cudaStream_t
   c->launches += 1;
   if (c->copy_kernel == MORI_KERNEL_TMA) {
     const long long max_grid = link ? 32 : c->sm_count;          // 1 CTA per SM (smem-bound)
-    const int grid = (int)std::min<long long>(n_pieces, max_grid);
+    const int grid = (int)std::min<long long>(a.n_pages * a.n_layers, max_grid);   // CTAs stride chunks
     mori::copy_pages_tma<kGather, kTmaStages><<<grid, mori::kTmaThreads, c->tma_smem, s>>>(a);
   } else {
     const long long max_grid = link ? 64 : (long long)c->sm_count * 8;
@@ -250,10 +250,11 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   c->piece = (int)std::min<long long>(kPieceBytes, chunk);
   c->ppc = (int)((chunk + c->piece - 1) / c->piece);
   c->copy_kernel = cfg->copy_kernel == MORI_KERNEL_AUTO ? MORI_KERNEL_TMA : cfg->copy_kernel;
-  c->tma_smem = (size_t)kTmaStages * c->piece + kTmaStages * sizeof(uint64_t);
+  c->tma_smem = (size_t)kTmaStages * c->piece + 2 * kTmaStages * sizeof(uint64_t);
   c->max_pages = cfg->max_pages_per_call ? cfg->max_pages_per_call
                                           : std::max<long long>(cfg->gpu_pool_pages, cfg->host_arena_slots);
-  c->staging_bytes = cfg->staging_bytes ? cfg->staging_bytes : (128LL << 20);
+  c->staging_bytes = cfg->staging_bytes ? cfg->staging_bytes : (1024LL << 20);
+  c->staging_bytes = std::min(c->staging_bytes, c->max_pages * c->page_bytes);   // never more than one call can fill
   c->staging_bytes = std::max(c->staging_bytes, c->page_bytes);
   c->staging_bytes -= c->staging_bytes % c->page_bytes;
   // AUTO: see DESIGN.md section 6 for the measurements behind this choice.
