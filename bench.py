@@ -406,6 +406,7 @@ def run_ours(args):
                     "achieved": ach, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s",
                     "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC.get("bytes_per_launch"),
                     "traffic_source": NCU_TRAFFIC.get("source"),
+                    "traffic_over_algorithmic_same_launch": NCU_TRAFFIC.get("ratio"),
                     "launches": k_n, "avg_launch_us": 1e3 * k_ms / k_n,
                     "algorithmic_bytes_per_launch": 2.0 * k_b / k_n}
 
@@ -421,6 +422,7 @@ def run_ours(args):
                         "traffic_source": NCU_TRAFFIC.get("source")}
 
     r.close()
+    rp = rank_partition_leg(with_oracle=(world == 1 and not args.no_cpu_baseline)) if rank == 0 else None
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(args.config)
@@ -453,6 +455,7 @@ def run_ours(args):
                          peak_how="pinned cudaMemcpyAsync of one contiguous 1 GiB buffer, best of 5, "
                                   "measured in this process before the run"),
             "gather_scatter": gs,
+            "rank_partition": rp,
             "cpu_baseline": cpu,
         }
         print(json.dumps(line))
@@ -463,7 +466,12 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the gather kernel from the committed
 # ncu --set full capture (profiles/); filled in once that capture exists.
-NCU_TRAFFIC: dict = {}
+NCU_TRAFFIC: dict = {
+    "bytes_per_launch": 1780.27e6,              # dram__bytes_read.sum 914.47 MB + write 865.81 MB
+    "algorithmic_bytes_same_launch": 1828.72e6,  # that launch gathered 436 pages of 2 MiB, x2
+    "ratio": 0.974,
+    "source": "profiles/r1_gather_ncu_full.md, launch 4 (ncu --set full, one in-step gather launch)",
+}
 
 
 def gather_scatter_leg(r, sim, hbm_peak, min_bytes=4 * GIB, reps=20, warm=3):
@@ -507,6 +515,56 @@ def gather_scatter_leg(r, sim, hbm_peak, min_bytes=4 * GIB, reps=20, warm=3):
         out[f"{name}_frac_of_measured_hbm"] = out[f"{name}_GBps"] / hbm_peak
         out[f"{name}_frac_of_8TBps_spec"] = out[f"{name}_GBps"] / 8000.0
     del buf
+    return out
+
+
+def rank_partition_leg(with_oracle: bool, reps=200):
+    """a1-a4 alone: device microseconds per call (CUDA events over `reps` back-to-back launches)
+    and host wall-clock of one launch + sync, at cfg 2's n = 64 and cfg 5's n = 4096 (scores
+    i.i.d. lognormal, sizes uniform, capacities that put the boundaries mid-ranking); the
+    oracle's microseconds beside it when allowed (rank 0, N = 1)."""
+    import torch
+    from paper_2606_00866_b200 import binding
+    pool = torch.zeros(2 * 4 * 8192, dtype=torch.uint8, device="cuda")
+    m = binding.Mori(2, 2, 64, 16, pool)
+    rng = np.random.default_rng(SEED)
+    cur = torch.cuda.current_stream()
+    out = {}
+    for n in (64, 4096):
+        iota = rng.lognormal(0.0, 1.0, n).astype(np.float32)
+        kv = rng.integers(16, 513, n).astype(np.int32)
+        prev = rng.integers(0, 3, n).astype(np.uint8)
+        cg, cc = int(kv.sum() * 0.2), int(kv.sum() * 0.4)
+        d = "cuda"
+        t_i, t_s, t_p = (torch.from_numpy(x).to(d) for x in (iota, kv, prev))
+        order = torch.empty(n, dtype=torch.int32, device=d); tier = torch.empty(n, dtype=torch.uint8, device=d)
+        bounds = torch.empty(2, dtype=torch.int32, device=d); used = torch.empty(2, dtype=torch.int64, device=d)
+        lists = torch.empty(5 * n, dtype=torch.int32, device=d); counts = torch.empty(5, dtype=torch.int32, device=d)
+
+        def call():
+            m.mori_rank_partition(n, t_i, t_s, t_p, cg, cc, order, tier, bounds, used, lists, counts, stream=cur)
+        for _ in range(10):
+            call()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(cur)
+        for _ in range(reps):
+            call()
+        e1.record(cur)
+        torch.cuda.synchronize()
+        wall = []
+        for _ in range(50):
+            t0 = time.perf_counter(); call(); torch.cuda.synchronize(); wall.append(time.perf_counter() - t0)
+        ent = {"device_us_per_call": 1e3 * e0.elapsed_time(e1) / reps,
+               "host_launch_plus_sync_us": 1e6 * float(np.median(wall))}
+        if with_oracle:
+            import oracle
+            ts = []
+            for _ in range(50):
+                t0 = time.perf_counter(); oracle.rank_partition(iota, kv, prev, cg, cc); ts.append(time.perf_counter() - t0)
+            ent["oracle_us_per_call_1core"] = 1e6 * float(np.median(ts))
+        out[f"n{n}"] = ent
+    m.close()
     return out
 
 
