@@ -58,7 +58,10 @@ enum { MORI_LIST_DEMOTE = 0, MORI_LIST_PROMOTE = 1, MORI_LIST_DROP = 2, MORI_LIS
  *              cudaMemcpyAsync DMAs staging -> arena on a copy stream, double-buffered
  *              (promote: DMA arena -> staging, then scatter kernel staging -> pool).
  *   COPYENGINE no kernel: one strided cudaMemcpy2DAsync per logical page (baseline).
- *   AUTO       the per-direction choice measured fastest on B200. */
+ *   AUTO       chosen per call from the slot table: STAGED when the runs of
+ *              consecutive host slots average >= 6 MiB (large DMAs reach 97-100 % of the measured
+ *              link peak), ZEROCOPY otherwise (a DMA per 2 MiB run reaches 89 %, SM-driven
+ *              zero-copy 92 % whatever the fragmentation).  mori_path() reports STAGED. */
 enum { MORI_PATH_AUTO = 0, MORI_PATH_ZEROCOPY = 1, MORI_PATH_STAGED = 2, MORI_PATH_COPYENGINE = 3 };
 /* Device copy kernel used by STAGED paths and by mori_gather_pages / mori_scatter_pages. */
 enum { MORI_KERNEL_AUTO = 0, MORI_KERNEL_LDST = 1, MORI_KERNEL_TMA = 2 };
@@ -78,6 +81,9 @@ typedef struct {
   int32_t copy_kernel;       /* MORI_KERNEL_* */
   int64_t staging_bytes;     /* per staging buffer (2 per direction); 0 -> 1 GiB */
   int64_t max_pages_per_call;/* 0 -> max(gpu_pool_pages, host_arena_slots) */
+  int32_t zerocopy_ctas;     /* grid of a ZEROCOPY kernel (it is link-bound, a few CTAs saturate
+                                PCIe and the rest of the SMs stay free); 0 -> library default */
+  int32_t reserved0;         /* must be 0 */
 } mori_config;
 
 /* Creates a context on the CURRENT CUDA device.  *out is NULL on failure. */

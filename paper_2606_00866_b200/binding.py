@@ -39,7 +39,8 @@ class MoriConfig(C.Structure):
                 ("host_arena", C.c_void_p), ("host_arena_slots", C.c_int64),
                 ("max_programs", C.c_int32), ("path_demote", C.c_int32),
                 ("path_promote", C.c_int32), ("copy_kernel", C.c_int32),
-                ("staging_bytes", C.c_int64), ("max_pages_per_call", C.c_int64)]
+                ("staging_bytes", C.c_int64), ("max_pages_per_call", C.c_int64),
+                ("zerocopy_ctas", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class MoriError(RuntimeError):
@@ -114,7 +115,7 @@ class Mori:
     def __init__(self, n_layers, n_kv_heads, head_dim, page_tokens, gpu_pool, host_arena=None,
                  elem_bytes=2, max_programs=MAX_PROGRAMS, path_demote=PATH_AUTO,
                  path_promote=PATH_AUTO, copy_kernel=KERNEL_AUTO, staging_bytes=0,
-                 max_pages_per_call=0):
+                 max_pages_per_call=0, zerocopy_ctas=0):
         self._lib = load()
         self.chunk_bytes = 2 * n_kv_heads * page_tokens * head_dim * elem_bytes
         self.page_bytes = self.chunk_bytes * n_layers
@@ -125,7 +126,8 @@ class Mori:
         self.gpu_pool_pages = pool_bytes // self.page_bytes
         cfg = MoriConfig(n_layers, n_kv_heads, head_dim, page_tokens, elem_bytes,
                          gpu_pool.data_ptr(), self.gpu_pool_pages, None, 0, max_programs,
-                         path_demote, path_promote, copy_kernel, staging_bytes, max_pages_per_call)
+                         path_demote, path_promote, copy_kernel, staging_bytes, max_pages_per_call,
+                         zerocopy_ctas, 0)
         self.host_arena_slots = 0
         if host_arena is not None:
             arena_bytes = host_arena.numel() * host_arena.element_size()

@@ -21,11 +21,13 @@ thread_local std::string g_create_error;
 constexpr int kTicketRing = 4096;
 constexpr int kTmaStages = 12;
 constexpr int kPieceBytes = 16 * 1024;
+constexpr long long kAutoMinRunBytes = 6LL << 20;   // AUTO: below this mean slot-run length, ZEROCOPY
 
 struct ProfSpan { cudaEvent_t a, b; long long bytes; };
 
 struct Direction {
   int path = 0;
+  bool auto_path = false;                        // AUTO: STAGED or ZEROCOPY per call, by slot-run length
   cudaStream_t kern = nullptr, copy = nullptr;   // kernel stream, DMA stream (STAGED only)
   unsigned char* staging[2] = {nullptr, nullptr};
   cudaEvent_t kern_done[2] = {nullptr, nullptr}, copy_done[2] = {nullptr, nullptr};
@@ -47,6 +49,7 @@ struct mori_ctx {
   long long chunk = 0, page_bytes = 0, staging_bytes = 0, max_pages = 0;
   int copy_kernel = MORI_KERNEL_TMA;
   int piece = kPieceBytes, ppc = 1;
+  int link_ctas = 32;
   size_t tma_smem = 0;
   unsigned char* arena_dev = nullptr;            // device-side alias of the pinned arena
   Direction dir[2];                              // 0 demote, 1 promote
@@ -104,11 +107,11 @@ cudaError_t launch_copy(const mori_ctx* c, const mori::CopyArgs& a, cudaStream_t
   if (n_pieces == 0) return cudaSuccess;
   c->launches += 1;
   if (c->copy_kernel == MORI_KERNEL_TMA) {
-    const long long max_grid = link ? 32 : c->sm_count;          // 1 CTA per SM (smem-bound)
+    const long long max_grid = link ? c->link_ctas : c->sm_count;  // 1 CTA per SM (smem-bound)
     const int grid = (int)std::min<long long>(a.n_pages * a.n_layers, max_grid);   // CTAs stride chunks
     mori::copy_pages_tma<kGather, kTmaStages><<<grid, mori::kTmaThreads, c->tma_smem, s>>>(a);
   } else {
-    const long long max_grid = link ? 64 : (long long)c->sm_count * 8;
+    const long long max_grid = link ? 2 * c->link_ctas : (long long)c->sm_count * 8;
     const int grid = (int)std::min<long long>(n_pieces, max_grid);
     mori::copy_pages_ldst<kGather><<<grid, mori::kLdstThreads, 0, s>>>(a);
   }
@@ -232,6 +235,7 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   if (cfg->copy_kernel < MORI_KERNEL_AUTO || cfg->copy_kernel > MORI_KERNEL_TMA)
     return fail(nullptr, MORI_ERR_INVALID_ARG, "bad copy_kernel");
   if (cfg->staging_bytes < 0 || cfg->max_pages_per_call < 0) return fail(nullptr, MORI_ERR_INVALID_ARG, "negative size");
+  if (cfg->zerocopy_ctas < 0 || cfg->zerocopy_ctas > 1024 || cfg->reserved0 != 0) return fail(nullptr, MORI_ERR_INVALID_ARG, "bad zerocopy_ctas / reserved0");
 
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
@@ -246,6 +250,7 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   c->device = dev;
   c->sm_count = prop.multiProcessorCount;
   c->chunk = chunk;
+  if (cfg->zerocopy_ctas > 0) c->link_ctas = cfg->zerocopy_ctas;
   c->page_bytes = chunk * cfg->n_layers;
   c->piece = (int)std::min<long long>(kPieceBytes, chunk);
   c->ppc = (int)((chunk + c->piece - 1) / c->piece);
@@ -260,6 +265,8 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   // AUTO: see DESIGN.md section 6 for the measurements behind this choice.
   c->dir[0].path = cfg->path_demote == MORI_PATH_AUTO ? MORI_PATH_STAGED : cfg->path_demote;
   c->dir[1].path = cfg->path_promote == MORI_PATH_AUTO ? MORI_PATH_STAGED : cfg->path_promote;
+  c->dir[0].auto_path = cfg->path_demote == MORI_PATH_AUTO;
+  c->dir[1].auto_path = cfg->path_promote == MORI_PATH_AUTO;
   *out = c;   // from here on mori_destroy cleans up
 
 #define CKC(call)                                                                             \
@@ -334,7 +341,7 @@ int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idlen
   if (!bounds || !used) return fail(c, MORI_ERR_INVALID_ARG, "bounds/used_pages is NULL");
   if (n > 0 && (!idleness || !kv_pages || !order || !tier)) return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
   if (prev_tier && (!lists || !counts)) return fail(c, MORI_ERR_INVALID_ARG, "prev_tier given but lists/list_counts NULL");
-  int n_pad = 32;
+  int n_pad = 64;                                  // the kernel's warp-local stages need >= 64
   while (n_pad < n) n_pad <<= 1;
   const int ipt = n_pad <= 1024 ? 1 : n_pad / 1024;
   const int threads = n_pad / ipt;
@@ -389,7 +396,17 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
   unsigned char* arena = static_cast<unsigned char*>(c->cfg.host_arena);
   const long long pb = c->page_bytes;
 
-  if (d.path == MORI_PATH_ZEROCOPY) {
+  // AUTO: a DMA per run of consecutive slots costs ~4.3 us of copy-engine
+  // set-up, so short runs (2 MiB: 89 % of the link peak, 4 MiB: 94 %) lose to SM-driven
+  // zero-copy (92 % whatever the run length); long runs (>= 8 MiB: 97-100 %) win.
+  int path = d.path;
+  if (d.auto_path && total > 0) {
+    long long runs = 1;
+    for (long long j = 1; j < total; ++j) runs += host_slots[j] != host_slots[j - 1] + 1;
+    path = (total * pb / runs < kAutoMinRunBytes) ? MORI_PATH_ZEROCOPY : MORI_PATH_STAGED;
+  }
+
+  if (path == MORI_PATH_ZEROCOPY) {
     if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc;
     if (total > 0) {
       const int32_t *dg, *dh;
@@ -402,7 +419,7 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
     return issue_ticket(c, d, d.kern, ticket_out);
   }
 
-  if (d.path == MORI_PATH_COPYENGINE) {
+  if (path == MORI_PATH_COPYENGINE) {
     if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc;
     const size_t dpitch = (size_t)c->cfg.gpu_pool_pages * c->chunk;   // layer stride in the pool
     for (long long j = 0; j < total; ++j) {

@@ -329,6 +329,22 @@ class IdAllocator:
     def n_free(self, clean_only: bool = False) -> int:
         return int((self.free & (self.tag == 0)).sum()) if clean_only else int(self.free.sum())
 
+    def alloc_run(self, k: int) -> Tuple[np.ndarray, int]:
+        """k clean ids as ONE run of consecutive ids (first fit, lowest address) -- the
+        "contiguous pinned host buffer" of a demoted program (BASELINE.json north_star; DESIGN
+        R7).  Falls back to ``alloc(k, clean_only=True)`` (fragments) when no such run is free."""
+        if k == 0:
+            return np.zeros(0, np.int32), 0
+        ok = self.free & (self.tag == 0)
+        edges = np.diff(np.concatenate(([0], ok.view(np.int8), [0])))
+        starts, ends = np.flatnonzero(edges == 1), np.flatnonzero(edges == -1)
+        fit = np.flatnonzero(ends - starts >= k)
+        if fit.size == 0:
+            return self.alloc(k, clean_only=True)
+        ids = np.arange(starts[fit[0]], starts[fit[0]] + k)
+        self.free[ids] = False
+        return ids.astype(np.int32), 0
+
     def alloc(self, k: int, clean_only: bool = False) -> Tuple[np.ndarray, int]:
         """-> (ids int32[k], max tag among them)."""
         if k == 0:
@@ -385,8 +401,8 @@ class Sim:
         self.trace = Trace(cfg, seed)
         n = cfg.n_programs
         arng = np.random.Generator(np.random.PCG64(config_seed(seed, cfg) + 7919)) if cfg.random_pages else None
-        self.gpu_alloc = IdAllocator(cfg.gpu_pool_pages, arng)
-        self.cpu_alloc = IdAllocator(cfg.cpu_pool_pages, arng)
+        self.gpu_alloc = IdAllocator(cfg.gpu_pool_pages, arng)     # cfg 5: every device page scattered
+        self.cpu_alloc = IdAllocator(cfg.cpu_pool_pages, None)     # host buffers: contiguous runs first
         self.tier = np.full(n, TIER_WAIT, np.uint8)
         self.gpu_pages: List[np.ndarray] = [np.zeros(0, np.int32) for _ in range(n)]
         self.host_slots: List[np.ndarray] = [np.zeros(0, np.int32) for _ in range(n)]
@@ -429,7 +445,7 @@ class Sim:
                 if dem_q and self.cpu_alloc.n_free(clean_only=True) >= self.gpu_pages[dem_q[0]].size:
                     p = dem_q.pop(0)
                     pages = self.gpu_pages[p]
-                    slots, _ = self.cpu_alloc.alloc(pages.size, clean_only=True)
+                    slots, _ = self.cpu_alloc.alloc_run(pages.size)
                     k += 1
                     ops.append(("demote", k, p, pages.copy(), slots))
                     self.gpu_alloc.release(pages, tag=k)     # reusable once demote #k completes

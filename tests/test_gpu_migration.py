@@ -10,7 +10,7 @@ from paper_2606_00866_b200.harness import GpuRunner
 
 pytestmark = pytest.mark.gpu
 
-PATHS = [1, 2, 3]          # zerocopy, staged, copyengine
+PATHS = [0, 1, 2, 3]       # auto (per call), zerocopy, staged, copyengine
 KERNELS = [1, 2]           # ldst, tma
 
 

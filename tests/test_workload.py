@@ -164,3 +164,22 @@ def test_cfg3_busy_fraction_moves_the_boundary():
             iota, _, _ = t.advance(tier)
         frac.append(float((iota < 0.5).mean()))
     assert frac[0] < frac[1] < frac[2]
+
+
+def test_alloc_run_gives_one_contiguous_clean_run_or_falls_back():
+    a = W.IdAllocator(32, None)
+    x, _ = a.alloc(10)                       # ids 0..9
+    a.release(x[2:5])                        # hole of 3 at 2..4
+    a.release(x[7:9], tag=3)                 # dirty hole at 7..8 (not yet reusable)
+    r, dep = a.alloc_run(3)
+    assert r.tolist() == [2, 3, 4] and dep == 0
+    r, _ = a.alloc_run(5)                    # first clean run of >= 5 starts at 10
+    assert r.tolist() == [10, 11, 12, 13, 14]
+    r, _ = a.alloc_run(17)                   # exactly the rest
+    assert r.tolist() == list(range(15, 32))
+    a.release(np.array([0, 1, 20, 21, 30]))
+    r, _ = a.alloc_run(4)                    # no run of 4: fragments, lowest clean ids
+    assert sorted(r.tolist()) == [0, 1, 20, 21]
+    with pytest.raises(MemoryError):
+        a.alloc_run(5)
+    assert a.alloc_run(0)[0].size == 0
