@@ -170,6 +170,20 @@ def ideal_seconds(dem_bytes, pro_bytes, link):
                (dem_bytes + pro_bytes) / (link["bidir_sum"] * 1e9))
 
 
+def memcpy_model_seconds(dem_bytes, pro_bytes, link):
+    """Time two plain pinned memcpys of these sizes, started together, would take at the measured
+    rates: both directions share the link at the measured simultaneous rate (split in
+    proportion to the solo rates) until the shorter one ends, the rest runs at its solo rate.
+    Tighter than ``ideal_seconds`` when the two directions carry different amounts."""
+    d_solo, p_solo = link["d2h"] * 1e9, link["h2d"] * 1e9
+    both = link["bidir_sum"] * 1e9
+    d_both, p_both = both * d_solo / (d_solo + p_solo), both * p_solo / (d_solo + p_solo)
+    if dem_bytes == 0 or pro_bytes == 0:
+        return dem_bytes / d_solo + pro_bytes / p_solo
+    t = min(dem_bytes / d_both, pro_bytes / p_both)
+    return t + (dem_bytes - t * d_both) / d_solo + (pro_bytes - t * p_both) / p_solo
+
+
 # ------------------------------------------------------------------------------------------------
 # the CPU oracle legs (cpu_baseline, --impl reference): the only places bench.py touches oracle/
 # ------------------------------------------------------------------------------------------------
@@ -322,7 +336,8 @@ def run_ours(args):
         sim.end_epoch()
         r.fill(plan.fills)                                          # stands in for prefill (untimed)
         n_tab = 8 * (plan.demote_pages + plan.promote_pages)        # page + slot ids, int32 each
-        return dict(ms=ms, dem=plan.demote_pages * page_b, pro=plan.promote_pages * page_b,
+        return dict(ms=ms, ops=[(op[0][0], len(op[3])) for op in plan.ops if op[0] != "sync_all"],
+                    dem=plan.demote_pages * page_b, pro=plan.promote_pages * page_b,
                     h2d=plan.promote_pages * page_b + 9 * n + n_tab,
                     d2h=plan.demote_pages * page_b + r.h_out.numel())
 
@@ -343,6 +358,11 @@ def run_ours(args):
     l0 = r.mori.mori_launch_count()
     steps = [epoch("dev") for _ in range(args.steps)]
     barrier()
+    if args.verbose and rank == 0:
+        for i, st in enumerate(steps):
+            gb = (st["dem"] + st["pro"]) / 1e9
+            print(f"step {i}: {st['ms']:.2f} ms  demote {st['dem'] / GIB:.2f} GiB  promote {st['pro'] / GIB:.2f} GiB  "
+                  f"{gb / (st['ms'] * 1e-3) if st['ms'] > 0 else 0:.1f} GB/s  ops {st['ops']}", file=sys.stderr)
     launches = r.mori.mori_launch_count() - l0
     clk = clocks.stop()
     prof = {"demote": r.mori.mori_profile_read(binding.DEMOTE),
@@ -373,7 +393,9 @@ def run_ours(args):
     def link_report(st):
         ideal = sum(ideal_seconds(s["dem"], s["pro"], link) for s in st)
         meas = sum(s["ms"] for s in st) * 1e-3
-        out = {"frac_of_measured_link_peak": ideal / meas if meas > 0 else None}
+        model = sum(memcpy_model_seconds(s["dem"], s["pro"], link) for s in st)
+        out = {"frac_of_measured_link_peak": ideal / meas if meas > 0 else None,
+               "frac_of_pinned_memcpy_model": model / meas if meas > 0 else None}
         for name, sel in (("demote_only", lambda s: s["dem"] > 0 and s["pro"] == 0),
                           ("promote_only", lambda s: s["pro"] > 0 and s["dem"] == 0),
                           ("bidirectional", lambda s: s["pro"] > 0 and s["dem"] > 0)):
@@ -385,6 +407,9 @@ def run_ours(args):
                 ent = {"steps": len(sub), "GBps": byt / sec / 1e9, "GiB": byt / GIB}
                 ent["frac"] = (ent["GBps"] / peak) if peak else \
                     sum(ideal_seconds(s["dem"], s["pro"], link) for s in sub) / sec
+                if not peak:
+                    ent["frac_of_pinned_memcpy_model"] = \
+                        sum(memcpy_model_seconds(s["dem"], s["pro"], link) for s in sub) / sec
                 out[name] = ent
         return out
 
@@ -580,6 +605,7 @@ def main():
     ap.add_argument("--path-promote", default="auto", choices=["auto", "zerocopy", "staged", "copyengine"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "ldst", "tma"])
     ap.add_argument("--staging-mib", type=int, default=0, help="0 = library default")
+    ap.add_argument("--verbose", action="store_true", help="per-step lines on stderr")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gather-leg", action="store_true")
     args = ap.parse_args()

@@ -188,7 +188,8 @@ int mori_profile_read(mori_ctx* ctx, int32_t which, double* kernel_ms, int64_t* 
 int mori_launch_count(const mori_ctx* ctx, int64_t* out);
 
 /* PINNED host memory for an arena when the caller has no allocator of its own: page-locked,
- * mapped into the device address space, exactly `bytes` long (no rounding), 4 KiB aligned.
+ * mapped into the device address space, exactly `bytes` long (no rounding), 2 MiB aligned,
+ * zero-filled (transparent-huge-page backed where the kernel allows).
  * *out is NULL on failure (MORI_ERR_CUDA; mori_last_error(NULL) says why).  Free with
  * mori_host_free, after destroying every context that uses it. */
 int mori_host_alloc(int64_t bytes, void** out);

@@ -54,65 +54,22 @@ __device__ __forceinline__ uint64_t block_excl_scan(uint64_t v, uint64_t* warp_t
   return warp_tot[warp] + incl - v;
 }
 
-// IPT = ranks per thread (n_pad / blockDim.x), blocked: thread t owns ranks [t*IPT, (t+1)*IPT).
+// Steps a2-a4 for one CTA whose thread t owns ranks [t*IPT, (t+1)*IPT): prog[i] is the program at
+// rank t*IPT + i (or -1 past n).  warp_tot = 33 words, bcast = 2 words of shared memory.
 template <int IPT>
-__global__ void __launch_bounds__(kRankMaxThreads, 1)
-rank_partition_kernel(int n, int n_pad, const float* __restrict__ idleness,
-                      const int32_t* __restrict__ kv_pages, const uint8_t* __restrict__ prev_tier,
-                      long long cap_gpu, long long cap_cpu, int32_t* __restrict__ order,
-                      uint8_t* __restrict__ tier, int32_t* __restrict__ bounds,
-                      long long* __restrict__ used, int32_t* __restrict__ lists,
-                      int32_t* __restrict__ list_counts) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n_pad]
-  uint64_t* warp_tot = keys + n_pad;                                 // [33]
-  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
-  const int tid = threadIdx.x, nt = blockDim.x;
-
-  // ---- a1: keys ------------------------------------------------------------------------------
-  for (int i = tid; i < n_pad; i += nt)
-    keys[i] = i < n ? ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i
-                    : 0xFFFFFFFFFFFFFFFFull;                         // padding sorts last
-  __syncthreads();
-
-  // ---- a1: bitonic sort, ascending ------------------------------------------------------------
-  // Pair q of a stage with stride j touches elements i = ((q & ~(j-1)) << 1) | (q & (j-1)) and
-  // i | j.  For j <= 32 the 32 pairs [32w, 32w+32) of one warp touch exactly the 64 elements
-  // [64w, 64w+64) whatever j is, so the stages j = 32 ... 1 of every merge run back to back
-  // inside a warp with __syncwarp only; a block barrier is needed only around strides >= 64.
-  // (n_pad = 4096: 21 block barriers instead of 78; n_pad <= 64: none.)
-  const int n_pairs = n_pad >> 1;                    // n_pad >= 64: a multiple of 32, whole warps
-  for (int k = 2; k <= n_pad; k <<= 1) {
-    int j = k >> 1;
-    for (; j >= 64; j >>= 1) {
-      for (int q = tid; q < n_pairs; q += nt) {
-        const int i = ((q & ~(j - 1)) << 1) | (q & (j - 1));
-        const int p = i | j;
-        const uint64_t a = keys[i], b = keys[p];
-        if ((a > b) == ((i & k) == 0)) { keys[i] = b; keys[p] = a; }
-      }
-      __syncthreads();
-    }
-    for (int q = tid; q < n_pairs; q += nt) {        // nt is a multiple of 32: whole warps iterate together
-      for (int jj = j; jj > 0; jj >>= 1) {
-        const int i = ((q & ~(jj - 1)) << 1) | (q & (jj - 1));
-        const int p = i | jj;
-        const uint64_t a = keys[i], b = keys[p];
-        if ((a > b) == ((i & k) == 0)) { keys[i] = b; keys[p] = a; }
-        __syncwarp();
-      }
-    }
-    if (k >= 64 || k == n_pad) __syncthreads();      // next merge (or the scan) crosses warps
-  }
-
+__device__ __forceinline__ void partition_tail(
+    int n, const int (&prog)[IPT], const int32_t* __restrict__ kv_pages,
+    const uint8_t* __restrict__ prev_tier, long long cap_gpu, long long cap_cpu,
+    int32_t* __restrict__ order, uint8_t* __restrict__ tier, int32_t* __restrict__ bounds,
+    long long* __restrict__ used, int32_t* __restrict__ lists, int32_t* __restrict__ list_counts,
+    uint64_t* warp_tot, long long* bcast) {
+  const int tid = threadIdx.x;
   // ---- a2: footprints in rank order + exclusive prefix sum (int64) ----------------------------
-  int prog[IPT];
   long long sz[IPT];
   long long tsum = 0;
 #pragma unroll
   for (int i = 0; i < IPT; ++i) {
     const int r = tid * IPT + i;
-    prog[i] = r < n ? (int)(uint32_t)keys[r] : -1;
     int s = r < n ? kv_pages[prog[i]] : 0;
     sz[i] = s > 0 ? s : 0;
     tsum += sz[i];
@@ -210,6 +167,124 @@ rank_partition_kernel(int n, int n_pad, const float* __restrict__ idleness,
   }
   if (tid < 4) list_counts[tid] = (int)((ptot >> (16 * tid)) & 0xFFFF);
   if (tid == 4) list_counts[4] = (int)rtot;
+}
+
+// IPT = ranks per thread (n_pad / blockDim.x), blocked: thread t owns ranks [t*IPT, (t+1)*IPT).
+template <int IPT>
+__global__ void __launch_bounds__(kRankMaxThreads, 1)
+rank_partition_kernel(int n, int n_pad, const float* __restrict__ idleness,
+                      const int32_t* __restrict__ kv_pages, const uint8_t* __restrict__ prev_tier,
+                      long long cap_gpu, long long cap_cpu, int32_t* __restrict__ order,
+                      uint8_t* __restrict__ tier, int32_t* __restrict__ bounds,
+                      long long* __restrict__ used, int32_t* __restrict__ lists,
+                      int32_t* __restrict__ list_counts) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n_pad]
+  uint64_t* warp_tot = keys + n_pad;                                 // [33]
+  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
+  const int tid = threadIdx.x, nt = blockDim.x;
+
+  // ---- a1: keys ------------------------------------------------------------------------------
+  for (int i = tid; i < n_pad; i += nt)
+    keys[i] = i < n ? ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i
+                    : 0xFFFFFFFFFFFFFFFFull;                         // padding sorts last
+  __syncthreads();
+
+  // ---- a1: bitonic sort, ascending ------------------------------------------------------------
+  // Pair q of a stage with stride j touches elements i = ((q & ~(j-1)) << 1) | (q & (j-1)) and
+  // i | j.  For j <= 32 the 32 pairs [32w, 32w+32) of one warp touch exactly the 64 elements
+  // [64w, 64w+64) whatever j is, so the stages j = 32 ... 1 of every merge run back to back
+  // inside a warp with __syncwarp only; a block barrier is needed only around strides >= 64.
+  // (n_pad = 4096: 21 block barriers instead of 78; n_pad <= 64: none.)
+  const int n_pairs = n_pad >> 1;                    // n_pad >= 64: a multiple of 32, whole warps
+  for (int k = 2; k <= n_pad; k <<= 1) {
+    int j = k >> 1;
+    for (; j >= 64; j >>= 1) {
+      for (int q = tid; q < n_pairs; q += nt) {
+        const int i = ((q & ~(j - 1)) << 1) | (q & (j - 1));
+        const int p = i | j;
+        const uint64_t a = keys[i], b = keys[p];
+        if ((a > b) == ((i & k) == 0)) { keys[i] = b; keys[p] = a; }
+      }
+      __syncthreads();
+    }
+    for (int q = tid; q < n_pairs; q += nt) {        // nt is a multiple of 32: whole warps iterate together
+      for (int jj = j; jj > 0; jj >>= 1) {
+        const int i = ((q & ~(jj - 1)) << 1) | (q & (jj - 1));
+        const int p = i | jj;
+        const uint64_t a = keys[i], b = keys[p];
+        if ((a > b) == ((i & k) == 0)) { keys[i] = b; keys[p] = a; }
+        __syncwarp();
+      }
+    }
+    if (k >= 64 || k == n_pad) __syncthreads();      // next merge (or the scan) crosses warps
+  }
+
+  int prog[IPT];
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    const int r = tid * IPT + i;
+    prog[i] = r < n ? (int)(uint32_t)keys[r] : -1;
+  }
+  partition_tail<IPT>(n, prog, kv_pages, prev_tier, cap_gpu, cap_cpu, order, tier, bounds, used, lists,
+                      list_counts, warp_tot, bcast);
+}
+
+// ---------------------------------------------------------------------------------------------
+// n > 1024: the sort of one CTA is bound by ONE SM's shared-memory bandwidth (78 passes over
+// 32-64 KiB).  Ranking by counting spreads a1 over the whole chip instead: the keys are unique
+// (the index is their low half), so rank(i) = #{j : key_j < key_i} is the sorted position, and
+// n^2 <= 6.7e7 compares over 148 SMs are ~1 us.  Every CTA builds all n keys in its shared
+// memory, ranks its slice of programs (one warp per program, lanes striding j) and writes
+// order[rank] = program.  The LAST CTA to finish (atomic ticket) runs a2-a4 on the completed
+// order: one launch, no grid barrier, no co-residency requirement.
+template <int IPT>
+__global__ void __launch_bounds__(kRankMaxThreads, 1)
+rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
+                            const int32_t* __restrict__ kv_pages, const uint8_t* __restrict__ prev_tier,
+                            long long cap_gpu, long long cap_cpu, int32_t* __restrict__ order,
+                            uint8_t* __restrict__ tier, int32_t* __restrict__ bounds,
+                            long long* __restrict__ used, int32_t* __restrict__ lists,
+                            int32_t* __restrict__ list_counts, unsigned int* __restrict__ ticket) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
+  uint64_t* warp_tot = keys + n;                                     // [33]
+  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
+  __shared__ unsigned int s_ticket;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+
+  for (int i = tid; i < n; i += blockDim.x)
+    keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;
+  __syncthreads();
+
+  const int per = (n + gridDim.x - 1) / gridDim.x;
+  const int lo = blockIdx.x * per, hi = min(n, lo + per);
+  for (int i = lo + warp; i < hi; i += n_warps) {
+    const uint64_t ki = keys[i];
+    int c = 0;
+    for (int j = lane; j < n; j += 32) c += keys[j] < ki;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
+    if (lane == 0) order[c] = i;
+  }
+
+  // ---- last CTA done? ---------------------------------------------------------------------------
+  __threadfence();                                   // this CTA's order[] writes are visible ...
+  __syncthreads();
+  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);    // ... before its ticket is
+  __syncthreads();
+  if (s_ticket != gridDim.x - 1) return;
+  if (tid == 0) *ticket = 0;                         // ready for the next launch that uses this counter
+  __threadfence();
+
+  int prog[IPT];
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    const int r = tid * IPT + i;
+    prog[i] = r < n ? __ldcg(order + r) : -1;        // written by other CTAs: read through L2
+  }
+  partition_tail<IPT>(n, prog, kv_pages, prev_tier, cap_gpu, cap_cpu, order, tier, bounds, used, lists,
+                      list_counts, warp_tot, bcast);
 }
 
 }  // namespace mori
