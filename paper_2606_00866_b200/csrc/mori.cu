@@ -28,8 +28,14 @@ std::map<void*, std::pair<void*, size_t>> g_host_allocs;   // mori_host_alloc: a
 
 constexpr int kTicketRing = 4096;
 constexpr int kRankTickets = 64;      // rank/partition launches that may be in flight at once
-constexpr int kTmaStages = 12;
-constexpr int kPieceBytes = 16 * 1024;
+#ifndef MORI_TMA_STAGES
+#define MORI_TMA_STAGES 12
+#endif
+#ifndef MORI_PIECE_BYTES
+#define MORI_PIECE_BYTES (16 * 1024)
+#endif
+constexpr int kTmaStages = MORI_TMA_STAGES;     // ring depth of the bulk-copy kernel
+constexpr int kPieceBytes = MORI_PIECE_BYTES;   // bytes per bulk copy (stage size)
 constexpr long long kAutoMinRunBytes = 6LL << 20;   // AUTO: below this mean slot-run length, ZEROCOPY
 
 struct ProfSpan { cudaEvent_t a, b; long long bytes; };
