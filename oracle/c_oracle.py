@@ -37,6 +37,8 @@ def _load():
         L.oracle_rank_partition.restype = C.c_int
         L.oracle_bruteforce_partition.argtypes = [i32, vp, vp, i64, i64, vp, vp, vp]
         L.oracle_bruteforce_partition.restype = C.c_int
+        L.oracle_sticky_rebalance.argtypes = [i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
+        L.oracle_sticky_rebalance.restype = C.c_int
         for f in (L.oracle_demote, L.oracle_promote):
             f.argtypes = [i32, i64, vp, i64, vp, i64, i64, vp, vp]
             f.restype = C.c_int
@@ -71,6 +73,29 @@ def rank_partition(iota, s, prev_tier, cap_gpu, cap_cpu):
     if prev is not None:
         out["lists"] = [lists[k, :counts[k]].copy() for k in range(5)]
     return out
+
+
+def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
+    """oracle_sticky_rebalance -> dict(tier, lazy, used, lists (5 arrays; reserve always empty))."""
+    iota = np.ascontiguousarray(iota, dtype=np.float32)
+    s = np.ascontiguousarray(s, dtype=np.int32)
+    prev = np.ascontiguousarray(prev_tier, dtype=np.uint8)
+    flags = np.ascontiguousarray(flags, dtype=np.uint8)
+    n = int(iota.shape[0])
+    assert s.shape == (n,) and prev.shape == (n,) and flags.shape == (n,)
+    tier = np.empty(max(n, 1), np.uint8)
+    lazy = np.zeros(max(n, 1), np.uint8)
+    used = np.zeros(2, np.int64)
+    lists = np.full((5, max(n, 1)), -1, np.int32)
+    if n:
+        lists = np.ascontiguousarray(lists[:, :n])
+    counts = np.zeros(5, np.int32)
+    rc = _load().oracle_sticky_rebalance(n, _p(iota), _p(s), _p(prev), _p(flags), int(cap_gpu),
+                                         int(cap_cpu), _p(tier), _p(lazy), _p(used), _p(lists), _p(counts))
+    if rc != 0:
+        raise ValueError(f"oracle_sticky_rebalance: bad argument (rc={rc})")
+    return dict(tier=tier[:n], lazy=lazy[:n], used=used,
+                lists=[lists[k, :counts[k]].copy() for k in range(5)])
 
 
 def bruteforce_partition(iota, s, cap_gpu, cap_cpu):

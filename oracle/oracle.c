@@ -215,3 +215,112 @@ int oracle_promote(int32_t n_layers, int64_t chunk, uint8_t *pool, int64_t pool_
   }
   return ORACLE_OK;
 }
+
+/*
+ * NEXT-1: the paper's sticky, status-aware tier management, section 4.3.1, followed
+ * step by step in the paper's order.  Nothing moves unless capacity forces or allows it
+ * ("programs are not eagerly reshuffled on every tick").
+ *
+ *   flags[p] bit 0  ACTING   the program waits on a tool call (else REASONING)
+ *            bit 1  READY    a CPU- or Waiting-queue program whose request is waiting for inference
+ *            bit 2  NEW      a Waiting-queue program that never held KV ("new arrival")
+ *
+ * Demotion from GPU: "When the aggregate KV cache of GPU-queue programs exceeds GPU
+ *   memory capacity, the scheduler demotes programs until usage fits within the budget ...
+ *   prioritizes demoting Acting programs ... over Reasoning programs ... Among programs of the
+ *   same status, it selects the one with the highest idleness first ... If only Reasoning
+ *   programs remain, the scheduler applies lazy demotion ... Demoted programs move to the CPU
+ *   queue if CPU capacity permits, or to the Waiting queue otherwise."
+ * Promotion to GPU: "When GPU capacity becomes available, the scheduler promotes
+ *   programs in a priority order: (1) CPU-queue programs that have completed their tool call and
+ *   are waiting for inference; (2) Waiting-queue programs that are waiting for inference, with
+ *   returning programs preferred over new arrivals; (3) newly arrived programs, smallest context
+ *   first.  Within each priority level ... the lowest idleness first."
+ *
+ * Readings (S1..S6): equal idleness resolves by the same total order as the ranking
+ * (the later program in that order is "more idle"); class 3 orders by (size, then that order);
+ * promotion stops at the first candidate that does not fit (head of line, like R3); a program
+ * demoted in this tick is not a promotion candidate in the same tick; the CPU queue must fit
+ * its capacity on entry (its programs are gated and do not grow) -- violated: ORACLE_ERR_ARG;
+ * no Waiting -> CPU move exists in this mode.
+ *
+ * Outputs: tier[n]; lazy[n] (1 = Reasoning victim, moves after its current step); used[2];
+ * lists[5*n] rows demote (GPU->CPU, victim order), promote (CPU->GPU, priority order),
+ * drop (GPU->WAIT, victim order), admit (WAIT->GPU, priority order), reserve (always empty);
+ * counts[5].
+ */
+enum { FLAG_ACTING = 1, FLAG_READY = 2, FLAG_NEW = 4 };
+
+int oracle_sticky_rebalance(int32_t n, const float *iota, const int32_t *s, const uint8_t *prev_tier,
+                            const uint8_t *flags, int64_t cap_gpu, int64_t cap_cpu, uint8_t *tier,
+                            uint8_t *lazy, int64_t *used, int32_t *lists, int32_t *counts) {
+  if (n < 0 || cap_gpu < 0 || cap_cpu < 0) return ORACLE_ERR_ARG;
+  if (n > 0 && (!iota || !s || !prev_tier || !flags || !tier || !lazy || !lists)) return ORACLE_ERR_ARG;
+  if (!counts || !used) return ORACLE_ERR_ARG;
+  int64_t usage_gpu = 0, usage_cpu = 0;
+  for (int32_t p = 0; p < n; ++p) {
+    if (s[p] < 0) return ORACLE_ERR_ARG;
+    tier[p] = (uint8_t)(prev_tier[p] == 0 ? TIER_GPU : (prev_tier[p] == 1 ? TIER_CPU : TIER_WAIT));
+    lazy[p] = 0;
+    if (tier[p] == TIER_GPU) usage_gpu += s[p];
+    if (tier[p] == TIER_CPU) usage_cpu += s[p];
+  }
+  if (usage_cpu > cap_cpu) return ORACLE_ERR_ARG;
+  for (int k = 0; k < 5; ++k) counts[k] = 0;
+
+  /* ---- demotion from GPU, one victim at a time ---- */
+  while (usage_gpu > cap_gpu) {
+    int32_t v = -1;
+    for (int32_t p = 0; p < n; ++p) {
+      if (tier[p] != TIER_GPU) continue;
+      if (v < 0) { v = p; continue; }
+      int ap = (flags[p] & FLAG_ACTING) != 0, av = (flags[v] & FLAG_ACTING) != 0;
+      if (ap != av) { if (ap) v = p; continue; }           /* Acting before Reasoning */
+      prog_key kp = { iota[p], p }, kv = { iota[v], v };
+      if (before(&kv, &kp)) v = p;                          /* highest idleness first */
+    }
+    if (v < 0) break;                                       /* nothing left to demote */
+    if (!(flags[v] & FLAG_ACTING)) lazy[v] = 1;             /* only Reasoning remain: lazy demotion */
+    usage_gpu -= s[v];
+    if (usage_cpu + s[v] <= cap_cpu) {                      /* CPU queue if capacity permits */
+      tier[v] = TIER_CPU; usage_cpu += s[v];
+      lists[0 * (size_t)n + counts[0]++] = v;
+    } else {                                                /* Waiting queue otherwise */
+      tier[v] = TIER_WAIT;
+      lists[2 * (size_t)n + counts[2]++] = v;
+    }
+  }
+
+  /* ---- promotion to GPU, in priority order, while it fits ---- */
+  uint8_t *seen = (uint8_t *)calloc((size_t)(n > 0 ? n : 1), 1);
+  if (!seen) return ORACLE_ERR_ARG;
+  for (;;) {
+    int32_t c = -1; int cls_c = 0;
+    for (int32_t p = 0; p < n; ++p) {
+      if (seen[p] || !(flags[p] & FLAG_READY)) continue;
+      int cls;
+      if (prev_tier[p] == 1) cls = 1;                                   /* CPU queue, ready        */
+      else if (prev_tier[p] != 0) cls = (flags[p] & FLAG_NEW) ? 3 : 2;  /* Waiting: returning, new */
+      else continue;                                                    /* was on GPU this tick    */
+      int better;
+      if (c < 0) better = 1;
+      else if (cls != cls_c) better = cls < cls_c;
+      else {
+        prog_key kp = { iota[p], p }, kc = { iota[c], c };
+        if (cls == 3 && s[p] != s[c]) better = s[p] < s[c];             /* smallest context first  */
+        else better = before(&kp, &kc);                                 /* lowest idleness first   */
+      }
+      if (better) { c = p; cls_c = cls; }
+    }
+    if (c < 0) break;
+    seen[c] = 1;
+    if (usage_gpu + s[c] > cap_gpu) break;                  /* head of line does not fit: stop */
+    usage_gpu += s[c];
+    if (cls_c == 1) { usage_cpu -= s[c]; lists[1 * (size_t)n + counts[1]++] = c; }
+    else lists[3 * (size_t)n + counts[3]++] = c;
+    tier[c] = TIER_GPU;
+  }
+  free(seen);
+  used[0] = usage_gpu; used[1] = usage_cpu;
+  return ORACLE_OK;
+}

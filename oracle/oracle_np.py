@@ -70,3 +70,60 @@ def promote(n_layers, chunk, pool, arena, host_slots, gpu_pages):
     g = np.asarray(gpu_pages, dtype=np.int64)
     h = np.asarray(host_slots, dtype=np.int64)
     pv[:, g] = av[h].transpose(1, 0, 2)
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-1: sticky, status-aware tier management restated with sorts and prefix sums
+# ------------------------------------------------------------------------------------------------
+ACTING, READY, NEW = 1, 2, 4
+
+
+def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
+    """Second statement of oracle_sticky_rebalance: instead of picking one victim / one candidate
+    at a time it sorts each group once by the paper's priority and cuts the sorted list with a
+    prefix sum (the cuts are monotone because sizes are non-negative)."""
+    s = np.asarray(s, dtype=np.int64)
+    prev = np.asarray(prev_tier, dtype=np.uint8)
+    prev = np.where(prev > 2, 2, prev)
+    flags = np.asarray(flags, dtype=np.uint8)
+    n = s.shape[0]
+    pos = np.empty(n, np.int64)
+    pos[rank(iota)] = np.arange(n)                  # position in the total order (0 = least idle)
+    tier = prev.copy()
+    lazy = np.zeros(n, np.uint8)
+    usage_gpu, usage_cpu = int(s[prev == 0].sum()), int(s[prev == 1].sum())
+    if usage_cpu > cap_cpu or (s < 0).any() or cap_gpu < 0 or cap_cpu < 0:
+        raise ValueError("bad argument")
+    # demotion: victims in order (Acting first, then most idle first) until the rest fits
+    g = np.flatnonzero(prev == 0)
+    acting = (flags[g] & ACTING) != 0
+    g = g[np.lexsort((-pos[g], ~acting))]           # primary: acting first; then descending position
+    freed = np.cumsum(s[g])                         # pages freed after demoting the first k+1 victims
+    # smallest v with usage - freed[v-1] <= cap  ==  number of k with usage - (freed before k) > cap
+    before_k = freed - s[g]
+    v = int(np.count_nonzero(usage_gpu - before_k > cap_gpu)) if usage_gpu > cap_gpu else 0
+    victims = g[:v]
+    demote, drop = [], []
+    for p in victims:                               # CPU if it fits, else Waiting: per victim, in order
+        if (flags[p] & ACTING) == 0:
+            lazy[p] = 1
+        usage_gpu -= int(s[p])
+        if usage_cpu + int(s[p]) <= cap_cpu:
+            tier[p] = 1; usage_cpu += int(s[p]); demote.append(p)
+        else:
+            tier[p] = 2; drop.append(p)
+    # promotion: candidates sorted by (class, [size for class 3], position); longest prefix that fits
+    ready = (flags & READY) != 0
+    cls = np.where(prev == 1, 1, np.where((flags & NEW) != 0, 3, 2))
+    c = np.flatnonzero(ready & (prev != 0))
+    size_key = np.where(cls[c] == 3, s[c], 0)
+    c = c[np.lexsort((pos[c], size_key, cls[c]))]
+    k = int(np.searchsorted(np.cumsum(s[c]), cap_gpu - usage_gpu, side="right"))
+    promote = [p for p in c[:k] if prev[p] == 1]
+    admit = [p for p in c[:k] if prev[p] != 1]
+    tier[c[:k]] = 0
+    usage_gpu += int(s[c[:k]].sum())
+    usage_cpu -= int(s[promote].sum()) if promote else 0
+    i32 = lambda x: np.asarray(x, dtype=np.int32)
+    return dict(tier=tier, lazy=lazy, used=np.array([usage_gpu, usage_cpu], np.int64),
+                lists=[i32(demote), i32(promote), i32(drop), i32(admit), i32([])])
