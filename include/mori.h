@@ -131,6 +131,38 @@ int mori_rank_partition(mori_ctx* ctx, void* stream, int32_t n, const float* idl
                         int64_t* used_pages, int32_t* lists, int32_t* list_counts);
 
 /*
+ * NEXT-1: the paper's sticky, status-aware tier management, section 4.3.1, as an
+ * alternative to mori_rank_partition for callers that track program status.  Nothing moves unless
+ * capacity forces or allows it.  One kernel launch on `stream`; DEVICE pointers.
+ *
+ *   Demotion   only while the GPU queue's pages exceed gpu_cap_pages: Acting programs before
+ *              Reasoning ones, the most idle first (equal scores: the later program in
+ *              the ranking order of mori_rank_partition is the more idle).  A Reasoning victim
+ *              is flagged lazy[p] = 1 ("finishes its current inference step before being
+ *              moved").  Each victim, in that order, goes to the CPU queue if its pages still
+ *              fit under cpu_cap_pages, else to Waiting.
+ *   Promotion  then, while the next candidate fits the GPU (the first that does not fit stops
+ *              it), in the priority order of P:L208: (1) CPU-queue programs that are READY,
+ *              (2) READY Waiting-queue programs that are not NEW, (3) READY NEW programs smallest
+ *              kv_pages first; the least idle first inside a class.  A program demoted by this
+ *              call is not a candidate in the same call.
+ *
+ *   flags        [n] uint8: MORI_FLAG_ACTING (waiting on a tool call; else Reasoning),
+ *                MORI_FLAG_READY (a request of it is waiting for inference), MORI_FLAG_NEW (never
+ *                held KV: a new arrival)
+ *   prev_tier    [n] required; the CPU queue must fit cpu_cap_pages on entry (its programs are
+ *                gated and do not grow) -- not checked on the device
+ *   tier         [n] out;  lazy [n] out;  used_pages [2] out (GPU queue, CPU queue)
+ *   lists        [5][n] out, rows MORI_LIST_*: demote and drop in victim order, promote and admit
+ *                in priority order, reserve always empty;  list_counts [5] out
+ */
+enum { MORI_FLAG_ACTING = 1, MORI_FLAG_READY = 2, MORI_FLAG_NEW = 4 };
+int mori_sticky_rebalance(mori_ctx* ctx, void* stream, int32_t n, const float* idleness,
+                          const int32_t* kv_pages, const uint8_t* prev_tier, const uint8_t* flags,
+                          int64_t gpu_cap_pages, int64_t cpu_cap_pages, uint8_t* tier, uint8_t* lazy,
+                          int64_t* used_pages, int32_t* lists, int32_t* list_counts);
+
+/*
  * Step a5, demotion ("offloaded to CPU DRAM on the same node"): for every
  * j in [0, total_pages) and every layer l, copy chunk (l, gpu_pages[j]) of the pool to
  * (host_slots[j], l) of the arena.  Asynchronous, on the context's demote stream(s).

@@ -22,6 +22,7 @@ DEMOTE, PROMOTE, BOTH = 1, 2, 3
 PATH_AUTO, PATH_ZEROCOPY, PATH_STAGED, PATH_COPYENGINE = 0, 1, 2, 3
 KERNEL_AUTO, KERNEL_LDST, KERNEL_TMA = 0, 1, 2
 MAX_PROGRAMS = 8192
+FLAG_ACTING, FLAG_READY, FLAG_NEW = 1, 2, 4
 PATH_NAMES = {1: "zerocopy", 2: "staged", 3: "copyengine"}
 KERNEL_NAMES = {1: "ldst", 2: "tma"}
 
@@ -29,7 +30,7 @@ EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", 
            "mori_sync", "mori_after_stream", "mori_stream_wait", "mori_gather_pages",
            "mori_scatter_pages", "mori_profile", "mori_profile_read", "mori_path",
            "mori_copy_kernel", "mori_last_error", "mori_launch_count", "mori_host_alloc",
-           "mori_host_free"]
+           "mori_host_free", "mori_sticky_rebalance"]
 
 
 class MoriConfig(C.Structure):
@@ -64,6 +65,7 @@ def load():
         L.mori_create.argtypes = [C.POINTER(MoriConfig), C.POINTER(vp)]
         L.mori_destroy.argtypes = [vp]
         L.mori_rank_partition.argtypes = [vp, vp, i32, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        L.mori_sticky_rebalance.argtypes = [vp, vp, i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
         L.mori_demote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
         L.mori_promote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
         L.mori_sync.argtypes = [vp, i32]
@@ -184,6 +186,15 @@ class Mori:
         return self._ck(self._lib.mori_rank_partition(
             self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), _ptr(prev_tier),
             int(gpu_cap_pages), int(cpu_cap_pages), _ptr(order), _ptr(tier), _ptr(bounds),
+            _ptr(used_pages), _ptr(lists), _ptr(list_counts)))
+
+    # -- NEXT-1: sticky, status-aware tier management ----------------------------------------
+    def mori_sticky_rebalance(self, n, idleness, kv_pages, prev_tier, flags, gpu_cap_pages,
+                              cpu_cap_pages, tier, lazy, used_pages, lists, list_counts, stream=None):
+        """All array arguments are CUDA tensors (see include/mori.h); asynchronous on ``stream``."""
+        return self._ck(self._lib.mori_sticky_rebalance(
+            self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), _ptr(prev_tier),
+            _ptr(flags), int(gpu_cap_pages), int(cpu_cap_pages), _ptr(tier), _ptr(lazy),
             _ptr(used_pages), _ptr(lists), _ptr(list_counts)))
 
     # -- a5-a7 -------------------------------------------------------------------------------

@@ -19,6 +19,7 @@
 
 #include "copy_pages.cuh"
 #include "rank_partition.cuh"
+#include "sticky_rebalance.cuh"
 
 namespace {
 
@@ -69,6 +70,7 @@ struct mori_ctx {
   unsigned char* arena_dev = nullptr;            // device-side alias of the pinned arena
   unsigned int* rank_tickets = nullptr;          // [kRankTickets] last-CTA counters of the multi-CTA ranker
   unsigned long long rank_seq = 0;
+  int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
   Direction dir[2];                              // 0 demote, 1 promote
   std::vector<cudaEvent_t> free_events;
   bool profiling = false;
@@ -241,6 +243,21 @@ cudaError_t launch_rank_multi(int grid, size_t smem, cudaStream_t s, int n, cons
   return cudaGetLastError();
 }
 
+template <int IPT>
+cudaError_t launch_sticky(int grid, size_t smem, cudaStream_t s, int n, const float* idl, const int32_t* kv,
+                                 const uint8_t* prev, const uint8_t* flags, long long cg, long long cc,
+                                 uint8_t* tier, uint8_t* lazy, long long* used, int32_t* lists, int32_t* counts,
+                                 int32_t* order, unsigned int* ticket) {
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(mori::sticky_rebalance_kernel<IPT>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  mori::sticky_rebalance_kernel<IPT><<<grid, mori::kRankMaxThreads, smem, s>>>(
+      n, idl, kv, prev, flags, cg, cc, tier, lazy, used, lists, counts, order, ticket);
+  return cudaGetLastError();
+}
+
 }  // namespace
 
 extern "C" {
@@ -314,6 +331,7 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   CKC(cudaFuncSetAttribute(mori::copy_pages_tma<false, kTmaStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
   CKC(cudaMalloc((void**)&c->rank_tickets, sizeof(unsigned int) * kRankTickets));
   CKC(cudaMemset(c->rank_tickets, 0, sizeof(unsigned int) * kRankTickets));
+  CKC(cudaMalloc((void**)&c->sticky_order, sizeof(int32_t) * kRankTickets * (size_t)cfg->max_programs));
   if (cfg->host_arena) {
     void* dp = nullptr;
     CKC(cudaHostGetDevicePointer(&dp, cfg->host_arena, 0));
@@ -362,6 +380,7 @@ int mori_destroy(mori_ctx* c) {
   }
   for (auto ev : c->free_events) cudaEventDestroy(ev);
   if (c->rank_tickets) cudaFree(c->rank_tickets);
+  if (c->sticky_order) cudaFree(c->sticky_order);
   delete c;
   return MORI_OK;
 }
@@ -404,6 +423,39 @@ int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idlen
   cudaError_t e;
   long long* u = reinterpret_cast<long long*>(used);
   e = launch_rank<1>(threads, smem, s, n, n_pad, idleness, kv_pages, prev_tier, gpu_cap, cpu_cap, order, tier, bounds, u, lists, counts);
+  CK(c, e);
+  c->launches += 1;
+  return MORI_OK;
+}
+
+int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idleness, const int32_t* kv_pages,
+                          const uint8_t* prev_tier, const uint8_t* flags, int64_t gpu_cap, int64_t cpu_cap,
+                          uint8_t* tier, uint8_t* lazy, int64_t* used, int32_t* lists, int32_t* counts) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (n < 0 || n > c->cfg.max_programs) return fail(c, MORI_ERR_INVALID_ARG, "n out of range (0..max_programs)");
+  if (gpu_cap < 0 || cpu_cap < 0) return fail(c, MORI_ERR_INVALID_ARG, "negative capacity");
+  if (!used || !counts) return fail(c, MORI_ERR_INVALID_ARG, "used_pages/list_counts is NULL");
+  if (n > 0 && (!idleness || !kv_pages || !prev_tier || !flags || !tier || !lazy || !lists))
+    return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
+  int n_pad = 1024;
+  while (n_pad < n) n_pad <<= 1;
+  const int grid = std::max(1, std::min(c->sm_count, (n + 31) / 32));
+  const size_t smem = sizeof(uint64_t) * (2 * (size_t)n + 33) + 4 * sizeof(long long);
+  const unsigned long long slot = c->rank_seq++ % kRankTickets;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  long long* u = reinterpret_cast<long long*>(used);
+  int32_t* ord = c->sticky_order + slot * (size_t)c->cfg.max_programs;
+  unsigned int* tk = c->rank_tickets + slot;
+  cudaError_t e;
+#define LS(I) launch_sticky<I>(grid, smem, s, n, idleness, kv_pages, prev_tier, flags, gpu_cap, cpu_cap, tier, lazy, u, lists, counts, ord, tk)
+  switch (n_pad / 1024) {
+    case 1: e = LS(1); break;
+    case 2: e = LS(2); break;
+    case 4: e = LS(4); break;
+    default: e = LS(8); break;
+  }
+#undef LS
   CK(c, e);
   c->launches += 1;
   return MORI_OK;

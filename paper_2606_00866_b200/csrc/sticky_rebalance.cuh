@@ -1,0 +1,213 @@
+// sticky_rebalance.cuh -- NEXT-1: the paper's sticky, status-aware tier management (section
+// 4.3.1) in ONE launch (sm_100a).  Declared in include/mori.h (mori_sticky_rebalance).
+//
+//   Demotion from GPU: only while the GPU queue exceeds its capacity; victims are Acting
+//     programs before Reasoning ones, the most idle first; Reasoning victims are flagged lazy;
+//     each victim goes to the CPU queue if it fits there, else to Waiting.
+//   Promotion to GPU: while it fits, in priority order (1) CPU-queue programs waiting
+//     for inference, (2) returning Waiting-queue programs, (3) new arrivals smallest context
+//     first; the least idle first inside a class.
+//   Everything else stays where it is.
+//
+// The paper's one-victim-at-a-time / one-candidate-at-a-time loops become one ordering and two
+// prefix cuts.  Every program gets a unique 128-bit key (group, status | size, idleness, index)
+// that sorts victims first (in victim order), then the promotion candidates (in priority order),
+// then everybody else.  Positions come from ranking by counting on every SM (keys in shared
+// memory, one warp per program); the last CTA to finish (atomic ticket) cuts the victim prefix
+// ("usage minus what the earlier victims free still exceeds the capacity" is monotone) and the
+// candidate prefix ("inclusive size sum fits the free capacity" is monotone) with block scans.
+// The only sequential step is the paper's per-victim "CPU if it fits, else Waiting", walked by
+// one thread over the victims' sizes in shared memory, and skipped when all of them fit.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "rank_partition.cuh"
+
+namespace mori {
+
+constexpr int kFlagActing = 1, kFlagReady = 2, kFlagNew = 4;
+
+// group: 0 GPU-queue program (victim order), 1..3 promotion classes, 7 not a candidate
+__device__ __forceinline__ int sticky_group(int prev, int fl) {
+  if (prev == 0) return 0;
+  if (!(fl & kFlagReady)) return 7;
+  if (prev == 1) return 1;
+  return (fl & kFlagNew) ? 3 : 2;
+}
+
+__device__ __forceinline__ void sticky_key(int p, float iota, int s, int prev, int fl, uint64_t& hi, uint64_t& lo) {
+  const uint32_t ik = idleness_key(iota);
+  const int g = sticky_group(prev, fl);
+  if (g == 0) {                       // Acting first, then most idle first (later in the total order)
+    hi = (uint64_t)((fl & kFlagActing) ? 0 : 1) << 32;
+    lo = ((uint64_t)(~ik) << 32) | (uint32_t)(~(uint32_t)p);
+  } else {                            // least idle first; class 3: smallest context first
+    hi = ((uint64_t)g << 33) | (g == 3 ? (uint32_t)(s > 0 ? s : 0) : 0u);
+    lo = ((uint64_t)ik << 32) | (uint32_t)p;
+  }
+}
+
+template <int IPT>
+__global__ void __launch_bounds__(kRankMaxThreads, 1)
+sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t* __restrict__ kv_pages,
+                        const uint8_t* __restrict__ prev_tier, const uint8_t* __restrict__ flags,
+                        long long cap_gpu, long long cap_cpu, uint8_t* __restrict__ tier,
+                        uint8_t* __restrict__ lazy, long long* __restrict__ used,
+                        int32_t* __restrict__ lists, int32_t* __restrict__ list_counts,
+                        int32_t* __restrict__ order, unsigned int* __restrict__ ticket) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint64_t* khi = reinterpret_cast<uint64_t*>(smem_raw);             // [n]
+  uint64_t* klo = khi + n;                                           // [n]
+  uint64_t* warp_tot = klo + n;                                      // [33]
+  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [4]
+  __shared__ unsigned int s_ticket;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+
+  for (int p = tid; p < n; p += blockDim.x) {
+    const int pv = prev_tier[p];
+    sticky_key(p, idleness[p], kv_pages[p], pv == 0 ? 0 : (pv == 1 ? 1 : 2), flags[p], khi[p], klo[p]);
+  }
+  __syncthreads();
+
+  // ---- position of every program of this CTA's slice = number of smaller keys -------------------
+  const int per = (n + gridDim.x - 1) / gridDim.x;
+  const int lo_p = blockIdx.x * per, hi_p = min(n, lo_p + per);
+  for (int p = lo_p + warp; p < hi_p; p += n_warps) {
+    const uint64_t h = khi[p], l = klo[p];
+    int c = 0;
+    for (int j = lane; j < n; j += 32) {
+      const uint64_t hj = khi[j];
+      c += (hj < h) || (hj == h && klo[j] < l);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
+    if (lane == 0) order[c] = p;
+  }
+
+  // ---- last CTA done? ---------------------------------------------------------------------------
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);
+  __syncthreads();
+  if (s_ticket != gridDim.x - 1) return;
+  if (tid == 0) *ticket = 0;
+  __threadfence();
+
+  // ---- this thread's positions ------------------------------------------------------------------
+  int32_t* vsize = reinterpret_cast<int32_t*>(khi);                  // [n] victims' sizes, by position
+  uint8_t* vdest = reinterpret_cast<uint8_t*>(klo);                  // [n] 1 = CPU queue, 2 = Waiting
+  int prog[IPT], grp[IPT], was[IPT], fl[IPT];
+  long long sz[IPT];
+  long long sum_g = 0, sum_c = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    const int r = tid * IPT + i;
+    prog[i] = -1; grp[i] = 7; was[i] = 2; fl[i] = 0; sz[i] = 0;
+    if (r < n) {
+      const int p = __ldcg(order + r);
+      const int pv = prev_tier[p];
+      prog[i] = p;
+      was[i] = pv == 0 ? 0 : (pv == 1 ? 1 : 2);
+      fl[i] = flags[p];
+      grp[i] = sticky_group(was[i], fl[i]);
+      const int s = kv_pages[p];
+      sz[i] = s > 0 ? s : 0;
+      if (was[i] == 0) sum_g += sz[i];
+      if (was[i] == 1) sum_c += sz[i];
+    }
+  }
+  __syncthreads();                                                   // keys are dead: smem is reused below
+
+  // ---- demotion: victims = the prefix of group 0 whose predecessors do not free enough ----------
+  uint64_t tot_g, tot_c, tot;
+  long long run = (long long)block_excl_scan((uint64_t)sum_g, warp_tot, &tot_g);   // freed BEFORE this thread
+  block_excl_scan((uint64_t)sum_c, warp_tot, &tot_c);
+  const long long usage_gpu0 = (long long)tot_g, usage_cpu0 = (long long)tot_c;
+  bool victim[IPT];
+  int n_v = 0;
+  long long freed_mine = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    victim[i] = grp[i] == 0 && usage_gpu0 - run > cap_gpu;           // group 0 sits at positions [0, nG)
+    if (grp[i] == 0) run += sz[i];
+    if (victim[i]) {
+      ++n_v; freed_mine += sz[i];
+      vsize[tid * IPT + i] = (int32_t)sz[i];
+    }
+  }
+  block_excl_scan((uint64_t)n_v, warp_tot, &tot);
+  const int v = (int)tot;                                            // victims are positions [0, v)
+  block_excl_scan((uint64_t)freed_mine, warp_tot, &tot);
+  const long long freed = (long long)tot;
+
+  // ---- each victim: CPU queue if it fits, else Waiting, in victim order -----------------
+  if (usage_cpu0 + freed <= cap_cpu) {                               // all of them fit
+#pragma unroll
+    for (int i = 0; i < IPT; ++i) if (victim[i]) vdest[tid * IPT + i] = 1;
+    if (tid == 0) bcast[0] = usage_cpu0 + freed;
+  } else if (tid == 0) {
+    long long cpu = usage_cpu0;
+    for (int k = 0; k < v; ++k) {
+      const bool fits = cpu + vsize[k] <= cap_cpu;
+      vdest[k] = fits ? 1 : 2;
+      if (fits) cpu += vsize[k];
+    }
+    bcast[0] = cpu;
+  }
+  __syncthreads();
+  const long long usage_cpu1 = bcast[0];
+
+  // ---- promotion: the longest prefix of the candidates (positions [nG, nG + nC)) that fits -------
+  const long long free_gpu = cap_gpu - (usage_gpu0 - freed);
+  long long cand_mine = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) if (grp[i] >= 1 && grp[i] <= 3) cand_mine += sz[i];
+  long long crun = (long long)block_excl_scan((uint64_t)cand_mine, warp_tot, &tot);
+  bool promoted[IPT];
+  long long up_g = 0, down_c = 0;
+  uint64_t packed = 0;                                               // 16-bit counters: demote | promote | drop | admit
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    promoted[i] = false;
+    if (grp[i] >= 1 && grp[i] <= 3) {
+      crun += sz[i];
+      promoted[i] = crun <= free_gpu;
+      if (promoted[i]) {
+        up_g += sz[i];
+        if (was[i] == 1) { down_c += sz[i]; packed += 1ull << 16; } else packed += 1ull << 48;
+      }
+    }
+    if (victim[i]) packed += vdest[tid * IPT + i] == 1 ? 1ull : (1ull << 32);
+  }
+  uint64_t ptot;
+  uint64_t pex = block_excl_scan(packed, warp_tot, &ptot);
+  block_excl_scan((uint64_t)up_g, warp_tot, &tot);
+  const long long promoted_pages = (long long)tot;
+  block_excl_scan((uint64_t)down_c, warp_tot, &tot);
+  const long long promoted_from_cpu = (long long)tot;
+
+  // ---- outputs ----------------------------------------------------------------------------------
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    if (prog[i] < 0) continue;
+    int now = was[i], row = -1;
+    if (victim[i]) { now = vdest[tid * IPT + i]; row = now == 1 ? 0 : 2; }
+    else if (promoted[i]) { now = 0; row = was[i] == 1 ? 1 : 3; }
+    tier[prog[i]] = (uint8_t)now;
+    lazy[prog[i]] = (uint8_t)(victim[i] && !(fl[i] & kFlagActing));
+    if (row >= 0) {
+      const int pos = (int)((pex >> (16 * row)) & 0xFFFF);
+      pex += 1ull << (16 * row);
+      lists[(size_t)row * n + pos] = prog[i];
+    }
+  }
+  if (tid < 4) list_counts[tid] = (int)((ptot >> (16 * tid)) & 0xFFFF);
+  if (tid == 4) list_counts[4] = 0;
+  if (tid == 0) {
+    used[0] = usage_gpu0 - freed + promoted_pages;
+    used[1] = usage_cpu1 - promoted_from_cpu;
+  }
+}
+
+}  // namespace mori
