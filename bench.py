@@ -582,12 +582,36 @@ def rank_partition_leg(with_oracle: bool, reps=200):
             t0 = time.perf_counter(); call(); torch.cuda.synchronize(); wall.append(time.perf_counter() - t0)
         ent = {"device_us_per_call": 1e3 * e0.elapsed_time(e1) / reps,
                "host_launch_plus_sync_us": 1e6 * float(np.median(wall))}
+        # NEXT-1: the sticky, status-aware policy mode on the same programs (GPU queue 1.5x over
+        # its capacity so that victims are cut, CPU queue with room for some of them)
+        fl = rng.integers(0, 8, n).astype(np.uint8)
+        t_f = torch.from_numpy(fl).to(d)
+        lazy = torch.empty(n, dtype=torch.uint8, device=d)
+        scg = int(kv[prev == 0].sum() / 1.5)
+        scc = int(kv[prev == 1].sum()) + int(kv[prev == 0].sum() * 0.2)
+
+        def call_sticky():
+            m.mori_sticky_rebalance(n, t_i, t_s, t_p, t_f, scg, scc, tier, lazy, used, lists, counts, stream=cur)
+        for _ in range(10):
+            call_sticky()
+        torch.cuda.synchronize()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(cur)
+        for _ in range(reps):
+            call_sticky()
+        s1.record(cur)
+        torch.cuda.synchronize()
+        ent["sticky_device_us_per_call"] = 1e3 * s0.elapsed_time(s1) / reps
         if with_oracle:
             import oracle
             ts = []
             for _ in range(50):
                 t0 = time.perf_counter(); oracle.rank_partition(iota, kv, prev, cg, cc); ts.append(time.perf_counter() - t0)
             ent["oracle_us_per_call_1core"] = 1e6 * float(np.median(ts))
+            ts = []
+            for _ in range(10):
+                t0 = time.perf_counter(); oracle.sticky_rebalance(iota, kv, prev, fl, scg, scc); ts.append(time.perf_counter() - t0)
+            ent["sticky_oracle_us_per_call_1core"] = 1e6 * float(np.median(ts))
         out[f"n{n}"] = ent
     m.close()
     return out

@@ -70,6 +70,35 @@ class GpuRunner:
         s.synchronize()
         return self._unpack(self.h_out.numpy())
 
+    # -- NEXT-1: the sticky policy mode, same host-in / host-out shape as place() ------------------
+    def place_sticky(self, iota, kv_pages, prev_tier, flags, stream=None):
+        n = self.cfg.n_programs
+        s = stream or torch.cuda.current_stream()
+        if not hasattr(self, "_st"):
+            d = self.dev
+            self._st = dict(flags=torch.empty(n, dtype=torch.uint8, device=d),
+                            lazy=torch.empty(n, dtype=torch.uint8, device=d))
+        hin = self.h_in.numpy()
+        hin[:4 * n].view(np.float32)[:] = iota
+        hin[4 * n:8 * n].view(np.int32)[:] = kv_pages
+        hin[8 * n:] = prev_tier
+        base, p = self.d_out.data_ptr(), self.d_in.data_ptr()
+        with torch.cuda.stream(s):
+            self.d_in.copy_(self.h_in, non_blocking=True)
+            self._st["flags"].copy_(torch.from_numpy(np.ascontiguousarray(flags, dtype=np.uint8)))
+            self.mori._ck(self.mori._lib.mori_sticky_rebalance(
+                self.mori._h, s.cuda_stream, n, p, p + 4 * n, p + 8 * n, self._st["flags"].data_ptr(),
+                self.cfg.cap_gpu_pages, self.cfg.cap_cpu_pages, base + self._o_tier,
+                self._st["lazy"].data_ptr(), base + self._o_used, base + self._o_lists,
+                base + self._o_counts))
+            self.h_out.copy_(self.d_out, non_blocking=True)
+            lazy = self._st["lazy"].cpu()
+        s.synchronize()
+        out = self._unpack(self.h_out.numpy())
+        out["lazy"] = lazy.numpy()
+        del out["order"], out["bounds"]
+        return out
+
     # -- the same with the inputs already resident in HBM (bench.py 'value' leg) -------------------
     def upload_inputs(self, iota, kv_pages, prev_tier):
         n = self.cfg.n_programs

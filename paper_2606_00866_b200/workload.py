@@ -19,6 +19,7 @@ from typing import List, Optional, Tuple
 import numpy as np
 
 TIER_GPU, TIER_CPU, TIER_WAIT = 0, 1, 2
+FLAG_ACTING, FLAG_READY, FLAG_NEW = 1, 2, 4     # inputs of the sticky policy mode
 K_WINDOW = 5          # P:L194 "we use k=5 in all experiments"
 TICK_S = 5.0          # P:L229 control-loop period
 
@@ -386,6 +387,7 @@ class EpochPlan:
     iota: np.ndarray
     kv_pages: np.ndarray
     prev_tier: np.ndarray
+    flags: Optional[np.ndarray] = None       # FLAG_* per program (sticky policy mode only)
     ops: list = field(default_factory=list)
     fills: list = field(default_factory=list)
     demote_pages: int = 0
@@ -406,8 +408,18 @@ class Sim:
         self.tier = np.full(n, TIER_WAIT, np.uint8)
         self.gpu_pages: List[np.ndarray] = [np.zeros(0, np.int32) for _ in range(n)]
         self.host_slots: List[np.ndarray] = [np.zeros(0, np.int32) for _ in range(n)]
+        self.ever_resident = np.zeros(n, bool)      # has held KV on this replica (else "new arrival")
         self.epoch = 0
         self._pending = None
+
+    def flags(self) -> np.ndarray:
+        """Status inputs of the sticky policy: ACTING while a tool call runs,
+        READY when the program wants inference (for a CPU/Waiting program: its request is gated
+        and waiting), NEW until it has held KV once."""
+        st = self.trace.state
+        f = np.where(st == 1, FLAG_ACTING, FLAG_READY).astype(np.uint8)
+        f[~self.ever_resident] |= FLAG_NEW
+        return f
 
     # step 1: inputs of this epoch's placement
     def begin_epoch(self) -> EpochPlan:
@@ -415,9 +427,10 @@ class Sim:
         for p in np.flatnonzero(replaced):                   # finished program: KV gone, slot reused
             self._drop(p)
             self.tier[p] = TIER_WAIT
+            self.ever_resident[p] = False
         T = self.cfg.shape.page_tokens
         kv_pages = ((tokens + T - 1) // T).astype(np.int32)
-        plan = EpochPlan(iota=iota, kv_pages=kv_pages, prev_tier=self.tier.copy())
+        plan = EpochPlan(iota=iota, kv_pages=kv_pages, prev_tier=self.tier.copy(), flags=self.flags())
         self._pending = plan
         return plan
 
@@ -481,6 +494,7 @@ class Sim:
         plan = self._pending
         self.gpu_alloc.clear_tags()
         self.cpu_alloc.clear_tags()
+        self.ever_resident |= self.tier == TIER_GPU
         for p in np.flatnonzero(self.tier == TIER_GPU):      # admit + growth: recompute prefill
             need = int(plan.kv_pages[p]) - self.gpu_pages[p].size
             if need > 0:

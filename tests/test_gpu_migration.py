@@ -121,7 +121,7 @@ def test_device_fill_matches_numpy_generator(mori):
     r.close()
 
 
-def _epochs_with_mirror(mori, cfg, seed, epochs, path, kernel):
+def _epochs_with_mirror(mori, cfg, seed, epochs, path, kernel, sticky=False):
     """Whole epochs: GPU placement must equal the oracle's; the CUDA movers and the oracle's
     memcpy movers get identical tables; both pools are compared byte for byte every epoch."""
     sh = cfg.shape
@@ -134,9 +134,16 @@ def _epochs_with_mirror(mori, cfg, seed, epochs, path, kernel):
     moved = 0
     for e in range(epochs):
         plan = sim.begin_epoch()
-        want = oracle.rank_partition(plan.iota, plan.kv_pages, plan.prev_tier, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
-        got = r.place(plan.iota, plan.kv_pages, plan.prev_tier)
-        for k in ("order", "tier", "bounds", "used"):
+        if sticky:
+            want = oracle.sticky_rebalance(plan.iota, plan.kv_pages, plan.prev_tier, plan.flags,
+                                           cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+            got = r.place_sticky(plan.iota, plan.kv_pages, plan.prev_tier, plan.flags)
+            keys = ("tier", "lazy", "used")
+        else:
+            want = oracle.rank_partition(plan.iota, plan.kv_pages, plan.prev_tier, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+            got = r.place(plan.iota, plan.kv_pages, plan.prev_tier)
+            keys = ("order", "tier", "bounds", "used")
+        for k in keys:
             assert np.array_equal(got[k], want[k]), (cfg.name, e, k)
         for k in range(5):
             assert np.array_equal(got["lists"][k], want["lists"][k]), (cfg.name, e, k)
@@ -172,4 +179,12 @@ def test_cfg1_epochs_full_mirror(mori, path):
 @pytest.mark.parametrize("path,kernel", [(1, 1), (2, 2)])
 def test_scaled_twins_epochs_full_mirror(mori, idx, scale, epochs, path, kernel):
     moved = _epochs_with_mirror(mori, W.get_config(idx, scale), 866, epochs, path, kernel)
+    assert moved > 0
+
+
+@pytest.mark.parametrize("idx,scale,epochs", [(2, 128, 30)])
+def test_sticky_policy_epochs_full_mirror(mori, idx, scale, epochs):
+    """NEXT-1 end to end: placement from mori_sticky_rebalance (== the section-4.3.1 oracle every
+    epoch), bytes moved by mori_demote / mori_promote, both pools mirrored byte for byte."""
+    moved = _epochs_with_mirror(mori, W.get_config(idx, scale), 866, epochs, 0, 2, sticky=True)
     assert moved > 0
