@@ -39,6 +39,10 @@ def _load():
         L.oracle_bruteforce_partition.restype = C.c_int
         L.oracle_sticky_rebalance.argtypes = [i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
         L.oracle_sticky_rebalance.restype = C.c_int
+        L.oracle_idleness_update.argtypes = [i32, vp, vp, vp, i32, i64, vp, vp, vp, vp]
+        L.oracle_idleness_update.restype = C.c_int
+        L.oracle_idleness_eval.argtypes = [i32, vp, vp, vp, i32, vp, vp, vp]
+        L.oracle_idleness_eval.restype = C.c_int
         for f in (L.oracle_demote, L.oracle_promote):
             f.argtypes = [i32, i64, vp, i64, vp, i64, i64, vp, vp]
             f.restype = C.c_int
@@ -96,6 +100,38 @@ def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
         raise ValueError(f"oracle_sticky_rebalance: bad argument (rc={rc})")
     return dict(tier=tier[:n], lazy=lazy[:n], used=used,
                 lists=[lists[k, :counts[k]].copy() for k in range(5)])
+
+
+class IdlenessTracker:
+    """State + the two oracle calls of Eq. (1): ``update(prog, kind, reasoning, acting)`` applies
+    completed cycles (kind 0) and slot resets (kind 1) in order; ``eval(open_r, open_a)`` -> f32[n]."""
+
+    def __init__(self, n, k=5):
+        self.n, self.k = int(n), int(k)
+        self.hist_r = np.zeros((self.n, self.k), np.float64)
+        self.hist_a = np.zeros((self.n, self.k), np.float64)
+        self.cnt = np.zeros(self.n, np.int32)
+
+    def update(self, prog, kind, reasoning, acting):
+        prog = np.ascontiguousarray(prog, dtype=np.int32)
+        kind = np.ascontiguousarray(kind, dtype=np.uint8)
+        r = np.ascontiguousarray(reasoning, dtype=np.float64)
+        a = np.ascontiguousarray(acting, dtype=np.float64)
+        assert prog.shape == kind.shape == r.shape == a.shape
+        rc = _load().oracle_idleness_update(self.k, _p(self.hist_r), _p(self.hist_a), _p(self.cnt),
+                                            self.n, prog.size, _p(prog), _p(kind), _p(r), _p(a))
+        if rc != 0:
+            raise ValueError(f"oracle_idleness_update: bad argument (rc={rc})")
+
+    def eval(self, open_r=None, open_a=None):
+        o_r = None if open_r is None else np.ascontiguousarray(open_r, dtype=np.float64)
+        o_a = None if open_a is None else np.ascontiguousarray(open_a, dtype=np.float64)
+        out = np.empty(self.n, np.float32)
+        rc = _load().oracle_idleness_eval(self.k, _p(self.hist_r), _p(self.hist_a), _p(self.cnt),
+                                          self.n, _p(o_r), _p(o_a), _p(out))
+        if rc != 0:
+            raise ValueError(f"oracle_idleness_eval: bad argument (rc={rc})")
+        return out
 
 
 def bruteforce_partition(iota, s, cap_gpu, cap_cpu):

@@ -324,3 +324,55 @@ int oracle_sticky_rebalance(int32_t n, const float *iota, const int32_t *s, cons
   used[0] = usage_gpu; used[1] = usage_cpu;
   return ORACLE_OK;
 }
+
+/*
+ * NEXT-2: the windowed idleness metric, Eq. (1), P:L190-194:
+ *     iota = T_acting^(k) / (T_reasoning^(k) + T_acting^(k))
+ * "the total time spent in each status over the last k inference--tool-call cycles (we use k=5)".
+ * Gated time never enters either sum: the caller simply does not report it.
+ * The unfinished cycle counts with its elapsed time ("the ongoing tool call's elapsed time keeps
+ * increasing and soon dominates the other terms in the window"): when it has any elapsed
+ * time it is the newest of the k cycles (R19).
+ *
+ * State per program, kept here in the plainest form: hist_r / hist_a [n][k] hold the completed
+ * cycles oldest first, cnt[n] how many (<= k).  A push on a full window drops the oldest.
+ * Precision (the paper is silent; R20): sums in double, oldest cycle first, the open
+ * cycle last; one division; one rounding to float.  No completed and no open time -> NaN.
+ */
+int oracle_idleness_update(int32_t k, double *hist_r, double *hist_a, int32_t *cnt, int32_t n,
+                           int64_t m, const int32_t *prog, const uint8_t *kind,
+                           const double *reasoning, const double *acting) {
+  if (k <= 0 || n < 0 || m < 0) return ORACLE_ERR_ARG;
+  for (int64_t e = 0; e < m; ++e) {
+    int32_t p = prog[e];
+    if (p < 0 || p >= n) return ORACLE_ERR_ARG;
+    double *hr = hist_r + (size_t)p * k, *ha = hist_a + (size_t)p * k;
+    if (kind[e] == 1) { cnt[p] = 0; continue; }             /* a fresh program took this slot */
+    if (cnt[p] == k) {                                      /* window slides: oldest cycle leaves */
+      memmove(hr, hr + 1, sizeof(double) * (size_t)(k - 1));
+      memmove(ha, ha + 1, sizeof(double) * (size_t)(k - 1));
+      cnt[p] = k - 1;
+    }
+    hr[cnt[p]] = reasoning[e]; ha[cnt[p]] = acting[e]; cnt[p] += 1;
+  }
+  return ORACLE_OK;
+}
+
+int oracle_idleness_eval(int32_t k, const double *hist_r, const double *hist_a, const int32_t *cnt,
+                         int32_t n, const double *open_r, const double *open_a, float *iota) {
+  if (k <= 0 || n < 0) return ORACLE_ERR_ARG;
+  for (int32_t p = 0; p < n; ++p) {
+    double orr = open_r ? open_r[p] : 0.0, oa = open_a ? open_a[p] : 0.0;
+    int open = (orr + oa) > 0.0;
+    int take = open ? k - 1 : k;                            /* the open cycle is one of the k */
+    if (take > cnt[p]) take = cnt[p];
+    double tr = 0.0, ta = 0.0;
+    for (int32_t i = cnt[p] - take; i < cnt[p]; ++i) {
+      tr += hist_r[(size_t)p * k + i];
+      ta += hist_a[(size_t)p * k + i];
+    }
+    if (open) { tr += orr; ta += oa; }
+    iota[p] = (tr + ta == 0.0) ? (float)(0.0 / 0.0) : (float)(ta / (tr + ta));
+  }
+  return ORACLE_OK;
+}

@@ -177,6 +177,9 @@ class Trace:
         self.hist_reason = [[] for _ in range(n)]   # completed cycles, most recent last
         self.hist_act = [[] for _ in range(n)]
         self.steps_left = np.zeros(n, np.int64)
+        # what a router would report to a device-side idleness tracker, in order:
+        # (program, kind, reasoning s, acting s) with kind 0 = completed cycle, 1 = slot reset
+        self.events: List[Tuple[int, int, float, float]] = []
         for p in range(n):
             self._spawn(p, new_uid=False)
 
@@ -204,6 +207,8 @@ class Trace:
         # one synthetic completed cycle from the initial phase, so iota is never 0/0 (DESIGN R10)
         self.hist_reason[p] = [self._draw_reason()]
         self.hist_act[p] = [self._draw_tool(p)]
+        self.events.append((p, 1, 0.0, 0.0))
+        self.events.append((p, 0, self.hist_reason[p][0], self.hist_act[p][0]))
         self.cur_reason[p] = 0.0
         self.cur_act[p] = 0.0
         self.state[p] = 0
@@ -211,6 +216,14 @@ class Trace:
         self.steps_left[p] = int(self.rng.integers(20, 61))
 
     # -- one tick ----------------------------------------------------------------------------
+    def take_events(self):
+        """-> (prog i32[m], kind u8[m], reasoning f64[m], acting f64[m]) since the last call, plus
+        the open cycle's elapsed (reasoning f64[n], acting f64[n]) -- the inputs of Eq. (1)."""
+        ev, self.events = self.events, []
+        cols = list(zip(*ev)) if ev else [(), (), (), ()]
+        return (np.array(cols[0], np.int32), np.array(cols[1], np.uint8), np.array(cols[2], np.float64),
+                np.array(cols[3], np.float64), self.cur_reason.copy(), self.cur_act.copy())
+
     def advance(self, tier: np.ndarray) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
         cfg = self.cfg
         n = cfg.n_programs
@@ -247,6 +260,7 @@ class Trace:
                     self.remaining[p] -= use
                     dt -= use
                     if self.remaining[p] <= 0.0:             # cycle closes
+                        self.events.append((p, 0, float(self.cur_reason[p]), float(self.cur_act[p])))
                         self.hist_reason[p] = (self.hist_reason[p] + [self.cur_reason[p]])[-K_WINDOW:]
                         self.hist_act[p] = (self.hist_act[p] + [self.cur_act[p]])[-K_WINDOW:]
                         self.cur_reason[p] = 0.0
