@@ -551,7 +551,7 @@ def rank_partition_leg(with_oracle: bool, reps=200):
     import torch
     from paper_2606_00866_b200 import binding
     pool = torch.zeros(2 * 4 * 8192, dtype=torch.uint8, device="cuda")
-    m = binding.Mori(2, 2, 64, 16, pool)
+    m = binding.Mori(2, 2, 64, 16, pool, max_programs=4096)
     rng = np.random.default_rng(SEED)
     cur = torch.cuda.current_stream()
     out = {}
@@ -602,8 +602,36 @@ def rank_partition_leg(with_oracle: bool, reps=200):
         s1.record(cur)
         torch.cuda.synchronize()
         ent["sticky_device_us_per_call"] = 1e3 * s0.elapsed_time(s1) / reps
+        # NEXT-2: Eq. (1) on the device: one tick's events (one completed cycle for a quarter of
+        # the programs) + evaluation of all n scores
+        me = max(1, n // 4)
+        e_prog = rng.permutation(n)[:me].astype(np.int32)
+        e_r, e_a = rng.lognormal(1.4, 0.5, me), rng.lognormal(1.0, 1.5, me)
+        o_r, o_a = rng.lognormal(1.0, 0.5, n), rng.lognormal(2.0, 1.5, n)
+        te = [torch.from_numpy(x).to(d) for x in (e_prog, np.zeros(me, np.uint8), e_r, e_a, o_r, o_a)]
+        iota_d = torch.empty(n, dtype=torch.float32, device=d)
+
+        def call_idl():
+            m.mori_idleness_update(te[0], te[1], te[2], te[3], stream=cur)
+            m.mori_idleness_eval(n, te[4], te[5], iota_d, stream=cur)
+        for _ in range(10):
+            call_idl()
+        torch.cuda.synchronize()
+        i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        i0.record(cur)
+        for _ in range(reps):
+            call_idl()
+        i1.record(cur)
+        torch.cuda.synchronize()
+        ent["idleness_update_eval_device_us"] = 1e3 * i0.elapsed_time(i1) / reps
         if with_oracle:
             import oracle
+            trk = oracle.IdlenessTracker(n)
+            ts = []
+            for _ in range(20):
+                t0 = time.perf_counter(); trk.update(e_prog, np.zeros(me, np.uint8), e_r, e_a); trk.eval(o_r, o_a)
+                ts.append(time.perf_counter() - t0)
+            ent["idleness_oracle_us_1core"] = 1e6 * float(np.median(ts))
             ts = []
             for _ in range(50):
                 t0 = time.perf_counter(); oracle.rank_partition(iota, kv, prev, cg, cc); ts.append(time.perf_counter() - t0)

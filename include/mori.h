@@ -83,7 +83,7 @@ typedef struct {
   int64_t max_pages_per_call;/* 0 -> max(gpu_pool_pages, host_arena_slots) */
   int32_t zerocopy_ctas;     /* grid of a ZEROCOPY kernel (it is link-bound, a few CTAs saturate
                                 PCIe and the rest of the SMs stay free); 0 -> library default */
-  int32_t reserved0;         /* must be 0 */
+  int32_t idleness_window;   /* k of Eq. (1); 0 -> 5 ("we use k=5 in all experiments"); <= 64 */
 } mori_config;
 
 /* Creates a context on the CURRENT CUDA device.  *out is NULL on failure. */
@@ -161,6 +161,29 @@ int mori_sticky_rebalance(mori_ctx* ctx, void* stream, int32_t n, const float* i
                           const int32_t* kv_pages, const uint8_t* prev_tier, const uint8_t* flags,
                           int64_t gpu_cap_pages, int64_t cpu_cap_pages, uint8_t* tier, uint8_t* lazy,
                           int64_t* used_pages, int32_t* lists, int32_t* list_counts);
+
+/*
+ * NEXT-2: the windowed idleness metric, Eq. (1), tracked on the device:
+ *     iota = T_acting^(k) / (T_reasoning^(k) + T_acting^(k))   over the last k cycles.
+ * The context keeps, per program slot 0 .. max_programs-1, the last k completed
+ * (reasoning, acting) duration pairs.  Time a program spent gated by the scheduler is simply never
+ * reported.  DEVICE pointers; one launch each on `stream`; asynchronous.
+ *
+ * mori_idleness_update applies m events in list order (events of one program keep their order):
+ *   prog [m] int32 slot;  kind [m] uint8: 0 = a cycle completed with durations
+ *   reasoning[e], acting[e] (seconds, double), 1 = the slot was taken by a new program (window
+ *   cleared; durations ignored).  Slots out of 0 .. max_programs-1 are ignored.
+ * mori_idleness_eval writes idleness_out[p] for p < n: the window is the last k cycles, the
+ *   unfinished one -- elapsed open_reasoning[p] + open_acting[p] > 0 -- counted as the newest of
+ *   them ("the ongoing tool call's elapsed time keeps increasing and soon dominates");
+ *   either open array may be NULL (all zero).  Sums in double, oldest first, open cycle last, one
+ *   division, one rounding to float; no time at all -> NaN (which the rankers place last).
+ *   idleness_out can be handed to mori_rank_partition / mori_sticky_rebalance on the same stream.
+ */
+int mori_idleness_update(mori_ctx* ctx, void* stream, int64_t m, const int32_t* prog,
+                         const uint8_t* kind, const double* reasoning, const double* acting);
+int mori_idleness_eval(mori_ctx* ctx, void* stream, int32_t n, const double* open_reasoning,
+                       const double* open_acting, float* idleness_out);
 
 /*
  * Step a5, demotion ("offloaded to CPU DRAM on the same node"): for every

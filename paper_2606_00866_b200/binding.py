@@ -30,7 +30,8 @@ EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", 
            "mori_sync", "mori_after_stream", "mori_stream_wait", "mori_gather_pages",
            "mori_scatter_pages", "mori_profile", "mori_profile_read", "mori_path",
            "mori_copy_kernel", "mori_last_error", "mori_launch_count", "mori_host_alloc",
-           "mori_host_free", "mori_sticky_rebalance"]
+           "mori_host_free", "mori_sticky_rebalance", "mori_idleness_update",
+           "mori_idleness_eval"]
 
 
 class MoriConfig(C.Structure):
@@ -41,7 +42,7 @@ class MoriConfig(C.Structure):
                 ("max_programs", C.c_int32), ("path_demote", C.c_int32),
                 ("path_promote", C.c_int32), ("copy_kernel", C.c_int32),
                 ("staging_bytes", C.c_int64), ("max_pages_per_call", C.c_int64),
-                ("zerocopy_ctas", C.c_int32), ("reserved0", C.c_int32)]
+                ("zerocopy_ctas", C.c_int32), ("idleness_window", C.c_int32)]
 
 
 class MoriError(RuntimeError):
@@ -66,6 +67,8 @@ def load():
         L.mori_destroy.argtypes = [vp]
         L.mori_rank_partition.argtypes = [vp, vp, i32, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
         L.mori_sticky_rebalance.argtypes = [vp, vp, i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
+        L.mori_idleness_update.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+        L.mori_idleness_eval.argtypes = [vp, vp, i32, vp, vp, vp]
         L.mori_demote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
         L.mori_promote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
         L.mori_sync.argtypes = [vp, i32]
@@ -117,7 +120,7 @@ class Mori:
     def __init__(self, n_layers, n_kv_heads, head_dim, page_tokens, gpu_pool, host_arena=None,
                  elem_bytes=2, max_programs=MAX_PROGRAMS, path_demote=PATH_AUTO,
                  path_promote=PATH_AUTO, copy_kernel=KERNEL_AUTO, staging_bytes=0,
-                 max_pages_per_call=0, zerocopy_ctas=0):
+                 max_pages_per_call=0, zerocopy_ctas=0, idleness_window=0):
         self._lib = load()
         self.chunk_bytes = 2 * n_kv_heads * page_tokens * head_dim * elem_bytes
         self.page_bytes = self.chunk_bytes * n_layers
@@ -129,7 +132,7 @@ class Mori:
         cfg = MoriConfig(n_layers, n_kv_heads, head_dim, page_tokens, elem_bytes,
                          gpu_pool.data_ptr(), self.gpu_pool_pages, None, 0, max_programs,
                          path_demote, path_promote, copy_kernel, staging_bytes, max_pages_per_call,
-                         zerocopy_ctas, 0)
+                         zerocopy_ctas, idleness_window)
         self.host_arena_slots = 0
         if host_arena is not None:
             arena_bytes = host_arena.numel() * host_arena.element_size()
@@ -196,6 +199,18 @@ class Mori:
             self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), _ptr(prev_tier),
             _ptr(flags), int(gpu_cap_pages), int(cpu_cap_pages), _ptr(tier), _ptr(lazy),
             _ptr(used_pages), _ptr(lists), _ptr(list_counts)))
+
+    # -- NEXT-2: Eq. (1) on the device -------------------------------------------------------
+    def mori_idleness_update(self, prog, kind, reasoning, acting, stream=None):
+        """CUDA tensors int32[m], uint8[m], float64[m], float64[m]; applied in list order."""
+        return self._ck(self._lib.mori_idleness_update(
+            self._h, _stream_handle(stream), int(prog.numel()), _ptr(prog), _ptr(kind), _ptr(reasoning),
+            _ptr(acting)))
+
+    def mori_idleness_eval(self, n, open_reasoning, open_acting, idleness_out, stream=None):
+        return self._ck(self._lib.mori_idleness_eval(
+            self._h, _stream_handle(stream), int(n), _ptr(open_reasoning), _ptr(open_acting),
+            _ptr(idleness_out)))
 
     # -- a5-a7 -------------------------------------------------------------------------------
     def mori_demote(self, gpu_pages, host_slots, wait_promote_ticket=0) -> int:

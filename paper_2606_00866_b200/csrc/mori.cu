@@ -20,6 +20,7 @@
 #include "copy_pages.cuh"
 #include "rank_partition.cuh"
 #include "sticky_rebalance.cuh"
+#include "idleness.cuh"
 
 namespace {
 
@@ -70,6 +71,8 @@ struct mori_ctx {
   unsigned char* arena_dev = nullptr;            // device-side alias of the pinned arena
   unsigned int* rank_tickets = nullptr;          // [kRankTickets] last-CTA counters of the multi-CTA ranker
   unsigned long long rank_seq = 0;
+  int idl_k = 5;                                 // window of Eq. (1)
+  double* idl_r = nullptr; double* idl_a = nullptr; int32_t* idl_pushed = nullptr;   // [max_programs][k], [max_programs]
   int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
   Direction dir[2];                              // 0 demote, 1 promote
   std::vector<cudaEvent_t> free_events;
@@ -284,7 +287,7 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   if (cfg->copy_kernel < MORI_KERNEL_AUTO || cfg->copy_kernel > MORI_KERNEL_TMA)
     return fail(nullptr, MORI_ERR_INVALID_ARG, "bad copy_kernel");
   if (cfg->staging_bytes < 0 || cfg->max_pages_per_call < 0) return fail(nullptr, MORI_ERR_INVALID_ARG, "negative size");
-  if (cfg->zerocopy_ctas < 0 || cfg->zerocopy_ctas > 1024 || cfg->reserved0 != 0) return fail(nullptr, MORI_ERR_INVALID_ARG, "bad zerocopy_ctas / reserved0");
+  if (cfg->zerocopy_ctas < 0 || cfg->zerocopy_ctas > 1024 || cfg->idleness_window < 0 || cfg->idleness_window > 64) return fail(nullptr, MORI_ERR_INVALID_ARG, "bad zerocopy_ctas / idleness_window");
 
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
@@ -331,6 +334,11 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   CKC(cudaFuncSetAttribute(mori::copy_pages_tma<false, kTmaStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
   CKC(cudaMalloc((void**)&c->rank_tickets, sizeof(unsigned int) * kRankTickets));
   CKC(cudaMemset(c->rank_tickets, 0, sizeof(unsigned int) * kRankTickets));
+  c->idl_k = cfg->idleness_window ? cfg->idleness_window : 5;
+  CKC(cudaMalloc((void**)&c->idl_r, sizeof(double) * (size_t)cfg->max_programs * c->idl_k));
+  CKC(cudaMalloc((void**)&c->idl_a, sizeof(double) * (size_t)cfg->max_programs * c->idl_k));
+  CKC(cudaMalloc((void**)&c->idl_pushed, sizeof(int32_t) * (size_t)cfg->max_programs));
+  CKC(cudaMemset(c->idl_pushed, 0, sizeof(int32_t) * (size_t)cfg->max_programs));
   CKC(cudaMalloc((void**)&c->sticky_order, sizeof(int32_t) * kRankTickets * (size_t)cfg->max_programs));
   if (cfg->host_arena) {
     void* dp = nullptr;
@@ -381,6 +389,9 @@ int mori_destroy(mori_ctx* c) {
   for (auto ev : c->free_events) cudaEventDestroy(ev);
   if (c->rank_tickets) cudaFree(c->rank_tickets);
   if (c->sticky_order) cudaFree(c->sticky_order);
+  if (c->idl_r) cudaFree(c->idl_r);
+  if (c->idl_a) cudaFree(c->idl_a);
+  if (c->idl_pushed) cudaFree(c->idl_pushed);
   delete c;
   return MORI_OK;
 }
@@ -457,6 +468,35 @@ int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idl
   }
 #undef LS
   CK(c, e);
+  c->launches += 1;
+  return MORI_OK;
+}
+
+int mori_idleness_update(mori_ctx* c, void* stream, int64_t m, const int32_t* prog, const uint8_t* kind,
+                         const double* reasoning, const double* acting) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (m < 0 || (m > 0 && (!prog || !kind || !reasoning || !acting))) return fail(c, MORI_ERR_INVALID_ARG, "bad event list");
+  if (m == 0) return MORI_OK;
+  const int n = c->cfg.max_programs;
+  mori::idleness_update_kernel<<<(n + mori::kIdlenessThreads - 1) / mori::kIdlenessThreads, mori::kIdlenessThreads, 0,
+                                 static_cast<cudaStream_t>(stream)>>>(n, c->idl_k, c->idl_r, c->idl_a, c->idl_pushed, m,
+                                                                      prog, kind, reasoning, acting);
+  CK(c, cudaGetLastError());
+  c->launches += 1;
+  return MORI_OK;
+}
+
+int mori_idleness_eval(mori_ctx* c, void* stream, int32_t n, const double* open_r, const double* open_a, float* out) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (n < 0 || n > c->cfg.max_programs) return fail(c, MORI_ERR_INVALID_ARG, "n out of range (0..max_programs)");
+  if (n > 0 && !out) return fail(c, MORI_ERR_INVALID_ARG, "idleness_out is NULL");
+  if (n == 0) return MORI_OK;
+  mori::idleness_eval_kernel<<<(n + mori::kIdlenessThreads - 1) / mori::kIdlenessThreads, mori::kIdlenessThreads, 0,
+                               static_cast<cudaStream_t>(stream)>>>(n, c->idl_k, c->idl_r, c->idl_a, c->idl_pushed,
+                                                                    open_r, open_a, out);
+  CK(c, cudaGetLastError());
   c->launches += 1;
   return MORI_OK;
 }
