@@ -39,6 +39,8 @@ def _load():
         L.oracle_bruteforce_partition.restype = C.c_int
         L.oracle_sticky_rebalance.argtypes = [i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
         L.oracle_sticky_rebalance.restype = C.c_int
+        L.oracle_eviction_order.argtypes = [i32, i64, vp, i32, vp, vp, vp, C.POINTER(i64)]
+        L.oracle_eviction_order.restype = C.c_int
         L.oracle_idleness_update.argtypes = [i32, vp, vp, vp, i32, i64, vp, vp, vp, vp]
         L.oracle_idleness_update.restype = C.c_int
         L.oracle_idleness_eval.argtypes = [i32, vp, vp, vp, i32, vp, vp, vp]
@@ -100,6 +102,21 @@ def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
         raise ValueError(f"oracle_sticky_rebalance: bad argument (rc={rc})")
     return dict(tier=tier[:n], lazy=lazy[:n], used=used,
                 lists=[lists[k, :counts[k]].copy() for k in range(5)])
+
+
+def eviction_order(which_tier, page_owner, program_tier, last_access):
+    """oracle_eviction_order -> int32 array of resident pages, first to evict first."""
+    owner = np.ascontiguousarray(page_owner, dtype=np.int32)
+    ptier = np.ascontiguousarray(program_tier, dtype=np.uint8)
+    last = np.ascontiguousarray(last_access, dtype=np.uint32)
+    assert owner.shape == last.shape
+    out = np.empty(max(owner.size, 1), np.int32)
+    nres = C.c_int64(0)
+    rc = _load().oracle_eviction_order(int(which_tier), owner.size, _p(owner), ptier.size, _p(ptier),
+                                       _p(last), _p(out), C.byref(nres))
+    if rc != 0:
+        raise ValueError(f"oracle_eviction_order: bad argument (rc={rc})")
+    return out[:nres.value].copy()
 
 
 class IdlenessTracker:

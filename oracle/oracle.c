@@ -376,3 +376,54 @@ int oracle_idleness_eval(int32_t k, const double *hist_r, const double *hist_a, 
   }
   return ORACLE_OK;
 }
+
+/*
+ * NEXT-3: typed eviction order.  "The engine's eviction policy remains
+ * LRU at its core, but uses the type label as a higher-priority sort key.  Crucially, the type
+ * priority order is reversed between the two tiers":
+ *     GPU HBM : evicts inactive first, then idle, then busy
+ *     CPU DRAM: evicts inactive first, then busy, then idle
+ * "Within each type, LRU breaks ties."  The label of a page is its program's placement
+ * (P:L214): GPU queue -> busy, CPU queue -> idle, Waiting queue -> inactive.
+ *
+ *   which_tier     0: order the pages of the GPU pool, 1: of the CPU pool
+ *   page_owner[j]  program that owns physical page j, or -1 if the page is free (not listed)
+ *   program_tier   [n_programs] 0 GPU / 1 CPU / anything else Waiting
+ *   last_access[j] time of last use (any monotone counter); smaller = less recently used
+ *   victims        out: the resident pages, first to evict first; *n_resident their number
+ * Reading (E1): equal last_access inside a type -> lower page id first.
+ */
+typedef struct { int32_t prio; uint32_t last; int32_t page; } evict_key;
+
+static int cmp_evict(const void *pa, const void *pb) {
+  const evict_key *a = (const evict_key *)pa, *b = (const evict_key *)pb;
+  if (a->prio != b->prio) return a->prio < b->prio ? -1 : 1;
+  if (a->last != b->last) return a->last < b->last ? -1 : 1;
+  return a->page < b->page ? -1 : (a->page > b->page ? 1 : 0);
+}
+
+int oracle_eviction_order(int32_t which_tier, int64_t n_pages, const int32_t *page_owner,
+                          int32_t n_programs, const uint8_t *program_tier, const uint32_t *last_access,
+                          int32_t *victims, int64_t *n_resident) {
+  if ((which_tier != 0 && which_tier != 1) || n_pages < 0 || n_programs < 0 || !n_resident) return ORACLE_ERR_ARG;
+  evict_key *keys = (evict_key *)malloc(sizeof(evict_key) * (size_t)(n_pages > 0 ? n_pages : 1));
+  if (!keys) return ORACLE_ERR_ARG;
+  int64_t r = 0;
+  for (int64_t j = 0; j < n_pages; ++j) {
+    int32_t o = page_owner[j];
+    if (o < 0) continue;                                       /* free page */
+    if (o >= n_programs) { free(keys); return ORACLE_ERR_ARG; }
+    int t = program_tier[o];
+    int busy = t == 0, idle = t == 1;                          /* else inactive */
+    int prio;
+    if (!busy && !idle) prio = 0;                              /* inactive goes first in both tiers */
+    else if (which_tier == 0) prio = idle ? 1 : 2;             /* GPU HBM : idle, then busy */
+    else prio = busy ? 1 : 2;                                  /* CPU DRAM: busy, then idle */
+    keys[r].prio = prio; keys[r].last = last_access[j]; keys[r].page = (int32_t)j; ++r;
+  }
+  qsort(keys, (size_t)r, sizeof(evict_key), cmp_evict);
+  for (int64_t i = 0; i < r; ++i) victims[i] = keys[i].page;
+  free(keys);
+  *n_resident = r;
+  return ORACLE_OK;
+}

@@ -127,3 +127,20 @@ def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
     i32 = lambda x: np.asarray(x, dtype=np.int32)
     return dict(tier=tier, lazy=lazy, used=np.array([usage_gpu, usage_cpu], np.int64),
                 lists=[i32(demote), i32(promote), i32(drop), i32(admit), i32([])])
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-3: typed eviction order as one lexsort
+# ------------------------------------------------------------------------------------------------
+def eviction_order(which_tier, page_owner, program_tier, last_access):
+    """Resident pages, first to evict first: type priority (reversed between the tiers), then LRU,
+    then page id."""
+    owner = np.asarray(page_owner, dtype=np.int64)
+    ptier = np.asarray(program_tier, dtype=np.int64)
+    last = np.asarray(last_access, dtype=np.int64)
+    pages = np.flatnonzero(owner >= 0)
+    t = ptier[owner[pages]]
+    # GPU HBM: inactive, idle, busy.  CPU DRAM: inactive, busy, idle.
+    table = np.array([2, 1], np.int64) if which_tier == 0 else np.array([1, 2], np.int64)
+    prio = np.where(t <= 1, table[np.minimum(t, 1)], 0)
+    return pages[np.lexsort((pages, last[pages], prio))].astype(np.int32)
