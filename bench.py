@@ -58,6 +58,14 @@ def _mem_available_bytes() -> int:
     return 0
 
 
+def _meminfo_kb(key: str) -> int:
+    with open("/proc/meminfo") as f:
+        for line in f:
+            if line.startswith(key + ":"):
+                return int(line.split()[1])
+    return 0
+
+
 def _pick_scale(cfg_index: int, world: int, W) -> int:
     """SURVEY 8(d) scale rule: the smallest power of two that lets the pinned arena of every
     rank fit host RAM (80 % of MemAvailable) and the pool fit HBM."""
@@ -284,7 +292,9 @@ def run_ours(args):
     sh = cfg.shape
     seed = replicas.replica_seed(SEED, rank)
     t_setup = time.perf_counter()
+    thp0 = _meminfo_kb("AnonHugePages")
     arena = binding.Mori.mori_host_alloc(cfg.cpu_pool_pages * sh.page_bytes)
+    arena_thp_gib = (_meminfo_kb("AnonHugePages") - thp0) / (1 << 20)
     link = measure_link_peak(arena)
     paths = {"auto": 0, "zerocopy": 1, "staged": 2, "copyengine": 3}
     r = GpuRunner(cfg, seed, arena=arena, staging_bytes=args.staging_mib << 20,
@@ -467,7 +477,8 @@ def run_ours(args):
                        "copy_kernel": kernel_name,
                        "staging_MiB": args.staging_mib,
                        "l2": "inputs larger than L2 (GiB per step vs 126 MB); no flush needed",
-                       "migrated_GiB": b_dev / GIB, "setup_s": t_setup},
+                       "migrated_GiB": b_dev / GIB, "setup_s": t_setup,
+                       "host_arena_on_huge_pages_GiB": arena_thp_gib},
             "clocks": clk,
             "e2e": {"value": value_e2e, "unit": UNIT,
                     "h2d_bytes_per_step": total(steps_e2e, "h2d") / K,

@@ -186,6 +186,27 @@ int mori_idleness_eval(mori_ctx* ctx, void* stream, int32_t n, const double* ope
                        const double* open_acting, float* idleness_out);
 
 /*
+ * NEXT-3: typed eviction order: "The engine's eviction policy remains LRU
+ * at its core, but uses the type label as a higher-priority sort key ... the type priority order
+ * is reversed between the two tiers":  GPU HBM evicts inactive first, then idle, then busy;
+ * CPU DRAM evicts inactive first, then busy, then idle; "within each type, LRU breaks ties".
+ * A page's type is its owner's placement: MORI_TIER_GPU busy, MORI_TIER_CPU idle,
+ * anything else inactive.  Equal last_access inside a type: lower page id first.
+ * DEVICE pointers; a fixed sequence of kernels on `stream`; asynchronous.
+ *
+ *   which_tier    MORI_TIER_GPU: n_pages <= gpu_pool_pages;  MORI_TIER_CPU: n_pages <= host_arena_slots
+ *   page_owner    [n_pages] int32 program slot, or < 0 for a free page (free pages are not listed)
+ *   program_tier  [n_programs] uint8 (e.g. the tier array mori_rank_partition wrote)
+ *   last_access   [n_pages] uint32, any monotone counter; smaller = less recently used
+ *   victims       [n_pages] out: the resident pages, first to evict first, in [0, *n_resident);
+ *                 entries past that are the free pages (unspecified order)
+ *   n_resident    [1] int32 out
+ */
+int mori_eviction_order(mori_ctx* ctx, void* stream, int32_t which_tier, int64_t n_pages,
+                        const int32_t* page_owner, int32_t n_programs, const uint8_t* program_tier,
+                        const uint32_t* last_access, int32_t* victims, int32_t* n_resident);
+
+/*
  * Step a5, demotion ("offloaded to CPU DRAM on the same node"): for every
  * j in [0, total_pages) and every layer l, copy chunk (l, gpu_pages[j]) of the pool to
  * (host_slots[j], l) of the arena.  Asynchronous, on the context's demote stream(s).

@@ -31,7 +31,7 @@ EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", 
            "mori_scatter_pages", "mori_profile", "mori_profile_read", "mori_path",
            "mori_copy_kernel", "mori_last_error", "mori_launch_count", "mori_host_alloc",
            "mori_host_free", "mori_sticky_rebalance", "mori_idleness_update",
-           "mori_idleness_eval"]
+           "mori_idleness_eval", "mori_eviction_order"]
 
 
 class MoriConfig(C.Structure):
@@ -67,6 +67,7 @@ def load():
         L.mori_destroy.argtypes = [vp]
         L.mori_rank_partition.argtypes = [vp, vp, i32, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
         L.mori_sticky_rebalance.argtypes = [vp, vp, i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
+        L.mori_eviction_order.argtypes = [vp, vp, i32, i64, vp, i32, vp, vp, vp, vp]
         L.mori_idleness_update.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         L.mori_idleness_eval.argtypes = [vp, vp, i32, vp, vp, vp]
         L.mori_demote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
@@ -199,6 +200,16 @@ class Mori:
             self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), _ptr(prev_tier),
             _ptr(flags), int(gpu_cap_pages), int(cpu_cap_pages), _ptr(tier), _ptr(lazy),
             _ptr(used_pages), _ptr(lists), _ptr(list_counts)))
+
+    # -- NEXT-3: typed eviction order -----------------------------------------------------------
+    def mori_eviction_order(self, which_tier, page_owner, program_tier, last_access, victims,
+                            n_resident, stream=None):
+        """CUDA tensors: int32[n_pages], uint8[n_programs], uint32-as-int32[n_pages]; outputs
+        int32[n_pages], int32[1]."""
+        return self._ck(self._lib.mori_eviction_order(
+            self._h, _stream_handle(stream), int(which_tier), int(page_owner.numel()), _ptr(page_owner),
+            int(program_tier.numel()), _ptr(program_tier), _ptr(last_access), _ptr(victims),
+            _ptr(n_resident)))
 
     # -- NEXT-2: Eq. (1) on the device -------------------------------------------------------
     def mori_idleness_update(self, prog, kind, reasoning, acting, stream=None):

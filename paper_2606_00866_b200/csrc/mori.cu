@@ -21,6 +21,7 @@
 #include "rank_partition.cuh"
 #include "sticky_rebalance.cuh"
 #include "idleness.cuh"
+#include "eviction_order.cuh"
 
 namespace {
 
@@ -73,6 +74,7 @@ struct mori_ctx {
   unsigned long long rank_seq = 0;
   int idl_k = 5;                                 // window of Eq. (1)
   double* idl_r = nullptr; double* idl_a = nullptr; int32_t* idl_pushed = nullptr;   // [max_programs][k], [max_programs]
+  int32_t* evict_perm[2] = {nullptr, nullptr}; int32_t* evict_table = nullptr; long long evict_cap = 0;   // scratch, grown on demand
   int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
   Direction dir[2];                              // 0 demote, 1 promote
   std::vector<cudaEvent_t> free_events;
@@ -389,6 +391,8 @@ int mori_destroy(mori_ctx* c) {
   for (auto ev : c->free_events) cudaEventDestroy(ev);
   if (c->rank_tickets) cudaFree(c->rank_tickets);
   if (c->sticky_order) cudaFree(c->sticky_order);
+  for (int b = 0; b < 2; ++b) if (c->evict_perm[b]) cudaFree(c->evict_perm[b]);
+  if (c->evict_table) cudaFree(c->evict_table);
   if (c->idl_r) cudaFree(c->idl_r);
   if (c->idl_a) cudaFree(c->idl_a);
   if (c->idl_pushed) cudaFree(c->idl_pushed);
@@ -469,6 +473,44 @@ int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idl
 #undef LS
   CK(c, e);
   c->launches += 1;
+  return MORI_OK;
+}
+
+int mori_eviction_order(mori_ctx* c, void* stream, int32_t which_tier, int64_t n_pages, const int32_t* page_owner,
+                        int32_t n_programs, const uint8_t* program_tier, const uint32_t* last_access,
+                        int32_t* victims, int32_t* n_resident) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (which_tier != MORI_TIER_GPU && which_tier != MORI_TIER_CPU) return fail(c, MORI_ERR_INVALID_ARG, "which_tier must be GPU or CPU");
+  const long long limit = which_tier == MORI_TIER_GPU ? c->cfg.gpu_pool_pages : c->cfg.host_arena_slots;
+  if (n_pages < 0 || n_pages > limit) return fail(c, MORI_ERR_INVALID_ARG, "n_pages exceeds the pool");
+  if (n_programs < 0 || !n_resident) return fail(c, MORI_ERR_INVALID_ARG, "bad n_programs / n_resident");
+  if (n_pages > 0 && (!page_owner || !last_access || !victims || (n_programs > 0 && !program_tier)))
+    return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  CK(c, cudaMemsetAsync(n_resident, 0, sizeof(int32_t), s));
+  if (n_pages == 0) return MORI_OK;
+  const int tiles = (int)((n_pages + mori::kEvictTile - 1) / mori::kEvictTile);
+  if (n_pages > c->evict_cap) {                    // first use / larger pool: (re)allocate scratch
+    CK(c, cudaStreamSynchronize(s));
+    for (int b = 0; b < 2; ++b) { if (c->evict_perm[b]) cudaFree(c->evict_perm[b]); c->evict_perm[b] = nullptr; }
+    if (c->evict_table) cudaFree(c->evict_table);
+    c->evict_table = nullptr; c->evict_cap = 0;
+    for (int b = 0; b < 2; ++b) CK(c, cudaMalloc((void**)&c->evict_perm[b], sizeof(int32_t) * (size_t)n_pages));
+    CK(c, cudaMalloc((void**)&c->evict_table, sizeof(int32_t) * 256 * (size_t)tiles));
+    c->evict_cap = n_pages;
+  }
+  mori::EvictArgs a{n_pages, n_programs, which_tier == MORI_TIER_GPU ? 0 : 1, tiles, page_owner, program_tier, last_access};
+  const int32_t* in = nullptr;                     // pass 0 reads the pages in id order
+  for (int pass = 0; pass < mori::kEvictPasses; ++pass) {
+    int32_t* out = pass == mori::kEvictPasses - 1 ? victims : c->evict_perm[pass & 1];
+    mori::evict_hist_kernel<<<tiles, mori::kEvictTile, 0, s>>>(a, pass, in, c->evict_table, n_resident);
+    mori::evict_scan_kernel<<<1, mori::kRankMaxThreads, 0, s>>>(c->evict_table, 256 * tiles);
+    mori::evict_scatter_kernel<<<tiles, mori::kEvictTile, 0, s>>>(a, pass, in, c->evict_table, out);
+    CK(c, cudaGetLastError());
+    c->launches += 3;
+    in = out;
+  }
   return MORI_OK;
 }
 
