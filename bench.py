@@ -458,6 +458,7 @@ def run_ours(args):
 
     r.close()
     rp = rank_partition_leg(with_oracle=(world == 1 and not args.no_cpu_baseline)) if rank == 0 else None
+    evl = eviction_leg(with_oracle=(world == 1 and not args.no_cpu_baseline)) if rank == 0 else None
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(args.config)
@@ -492,6 +493,7 @@ def run_ours(args):
                                   "measured in this process before the run"),
             "gather_scatter": gs,
             "rank_partition": rp,
+            "eviction_order": evl,
             "cpu_baseline": cpu,
         }
         print(json.dumps(line))
@@ -652,6 +654,42 @@ def rank_partition_leg(with_oracle: bool, reps=200):
                 t0 = time.perf_counter(); oracle.sticky_rebalance(iota, kv, prev, fl, scg, scc); ts.append(time.perf_counter() - t0)
             ent["sticky_oracle_us_per_call_1core"] = 1e6 * float(np.median(ts))
         out[f"n{n}"] = ent
+    m.close()
+    return out
+
+
+def eviction_leg(with_oracle: bool, n_pages=65536, n_programs=64, reps=50):
+    """NEXT-3: typed eviction order of a 65 536-page pool (cfg 2's arena): device microseconds per
+    call (15 kernels), and the oracle's qsort beside it."""
+    import torch
+    from paper_2606_00866_b200 import binding
+    pool = torch.zeros(n_pages * 32, dtype=torch.uint8, device="cuda")       # 32-byte pages
+    m = binding.Mori(1, 1, 8, 1, pool)
+    rng = np.random.default_rng(SEED)
+    owner = rng.integers(-1, n_programs, n_pages).astype(np.int32)
+    ptier = rng.integers(0, 3, n_programs).astype(np.uint8)
+    last = rng.integers(0, 200, n_pages).astype(np.uint32)                   # ticks
+    d = "cuda"
+    t_o, t_t = torch.from_numpy(owner).to(d), torch.from_numpy(ptier).to(d)
+    t_l = torch.from_numpy(last.view(np.int32)).to(d)
+    vic = torch.empty(n_pages, dtype=torch.int32, device=d); nres = torch.empty(1, dtype=torch.int32, device=d)
+    cur = torch.cuda.current_stream()
+    for _ in range(5):
+        m.mori_eviction_order(binding.TIER_GPU, t_o, t_t, t_l, vic, nres, stream=cur)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(cur)
+    for _ in range(reps):
+        m.mori_eviction_order(binding.TIER_GPU, t_o, t_t, t_l, vic, nres, stream=cur)
+    e1.record(cur)
+    torch.cuda.synchronize()
+    out = {"n_pages": n_pages, "device_us_per_call": 1e3 * e0.elapsed_time(e1) / reps}
+    if with_oracle:
+        import oracle
+        ts = []
+        for _ in range(5):
+            t0 = time.perf_counter(); oracle.eviction_order(0, owner, ptier, last); ts.append(time.perf_counter() - t0)
+        out["oracle_us_per_call_1core"] = 1e6 * float(np.median(ts))
     m.close()
     return out
 
