@@ -39,6 +39,8 @@ def _load():
         L.oracle_bruteforce_partition.restype = C.c_int
         L.oracle_sticky_rebalance.argtypes = [i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
         L.oracle_sticky_rebalance.restype = C.c_int
+        L.oracle_bfd_assign.argtypes = [i32, vp, vp, vp, i32, vp, vp, vp]
+        L.oracle_bfd_assign.restype = C.c_int
         L.oracle_eviction_order.argtypes = [i32, i64, vp, i32, vp, vp, vp, C.POINTER(i64)]
         L.oracle_eviction_order.restype = C.c_int
         L.oracle_idleness_update.argtypes = [i32, vp, vp, vp, i32, i64, vp, vp, vp, vp]
@@ -102,6 +104,22 @@ def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
         raise ValueError(f"oracle_sticky_rebalance: bad argument (rc={rc})")
     return dict(tier=tier[:n], lazy=lazy[:n], used=used,
                 lists=[lists[k, :counts[k]].copy() for k in range(5)])
+
+
+def bfd_assign(size, iota, flags, free_pages):
+    """oracle_bfd_assign -> (replica int32[m] with -1 = stays waiting, free_out int64[R])."""
+    size = np.ascontiguousarray(size, dtype=np.int32)
+    iota = np.ascontiguousarray(iota, dtype=np.float32)
+    flags = np.ascontiguousarray(flags, dtype=np.uint8)
+    free = np.ascontiguousarray(free_pages, dtype=np.int64)
+    m = size.size
+    assert iota.shape == (m,) and flags.shape == (m,)
+    rep = np.full(max(m, 1), -9, np.int32)
+    out = np.zeros(max(free.size, 1), np.int64)
+    rc = _load().oracle_bfd_assign(m, _p(size), _p(iota), _p(flags), free.size, _p(free), _p(rep), _p(out))
+    if rc != 0:
+        raise ValueError(f"oracle_bfd_assign: bad argument (rc={rc})")
+    return rep[:m].copy(), out[:free.size]
 
 
 def eviction_order(which_tier, page_owner, program_tier, last_access):

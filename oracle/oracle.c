@@ -427,3 +427,54 @@ int oracle_eviction_order(int32_t which_tier, int64_t n_pages, const int32_t *pa
   *n_resident = r;
   return ORACLE_OK;
 }
+
+/*
+ * NEXT-4(i): placement of Waiting-queue promotions across replicas, P:L208-210:
+ * "For multi-replica deployments, Waiting-queue promotions use Best-Fit-Decreasing bin packing
+ * across replicas, selecting the replica with the most available capacity first, while
+ * CPU-queue promotions preserve replica affinity" (so only Waiting-queue programs are packed;
+ * the single Waiting queue is shared by all replicas).
+ *
+ *   size[m], iota[m], flags[m]   the READY Waiting-queue candidates (FLAG_NEW marks new arrivals)
+ *   free_pages[R]                GPU pages each replica has free after its own demotions and
+ *                                CPU-queue promotions (all-gathered from the replicas)
+ *   replica[m] out               the replica that admits the candidate, or -1: stays in Waiting
+ *   free_out[R] out              what is left
+ * Readings (B1..B3): "decreasing" = by size, largest first; equal sizes keep the
+ * promotion priority of P:L208 (returning before new, then the least idle, then the index);
+ * the chosen replica is the one with the MOST free pages (ties: lowest replica index); a
+ * candidate that does not fit there fits nowhere and stays in Waiting, and the packing goes on
+ * with the next (smaller) candidate.
+ */
+typedef struct { int32_t size; int cls; float iota; int32_t idx; } bfd_key;
+
+static int cmp_bfd(const void *pa, const void *pb) {
+  const bfd_key *a = (const bfd_key *)pa, *b = (const bfd_key *)pb;
+  if (a->size != b->size) return a->size > b->size ? -1 : 1;        /* decreasing size */
+  if (a->cls != b->cls) return a->cls < b->cls ? -1 : 1;            /* returning before new */
+  prog_key ka = { a->iota, a->idx }, kb = { b->iota, b->idx };
+  if (before(&ka, &kb)) return -1;
+  if (before(&kb, &ka)) return 1;
+  return 0;
+}
+
+int oracle_bfd_assign(int32_t m, const int32_t *size, const float *iota, const uint8_t *flags,
+                      int32_t n_replicas, const int64_t *free_pages, int32_t *replica, int64_t *free_out) {
+  if (m < 0 || n_replicas < 1 || !free_pages || !free_out) return ORACLE_ERR_ARG;
+  for (int32_t r = 0; r < n_replicas; ++r) { if (free_pages[r] < 0) return ORACLE_ERR_ARG; free_out[r] = free_pages[r]; }
+  bfd_key *keys = (bfd_key *)malloc(sizeof(bfd_key) * (size_t)(m > 0 ? m : 1));
+  if (!keys) return ORACLE_ERR_ARG;
+  for (int32_t i = 0; i < m; ++i) {
+    if (size[i] < 0) { free(keys); return ORACLE_ERR_ARG; }
+    keys[i].size = size[i]; keys[i].cls = (flags[i] & FLAG_NEW) ? 1 : 0; keys[i].iota = iota[i]; keys[i].idx = i;
+  }
+  qsort(keys, (size_t)m, sizeof(bfd_key), cmp_bfd);
+  for (int32_t k = 0; k < m; ++k) {
+    int32_t best = 0;
+    for (int32_t r = 1; r < n_replicas; ++r) if (free_out[r] > free_out[best]) best = r;   /* most available */
+    if (keys[k].size <= free_out[best]) { replica[keys[k].idx] = best; free_out[best] -= keys[k].size; }
+    else replica[keys[k].idx] = -1;
+  }
+  free(keys);
+  return ORACLE_OK;
+}

@@ -144,3 +144,25 @@ def eviction_order(which_tier, page_owner, program_tier, last_access):
     table = np.array([2, 1], np.int64) if which_tier == 0 else np.array([1, 2], np.int64)
     prio = np.where(t <= 1, table[np.minimum(t, 1)], 0)
     return pages[np.lexsort((pages, last[pages], prio))].astype(np.int32)
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4(i): Best-Fit-Decreasing of Waiting-queue promotions across replicas
+# ------------------------------------------------------------------------------------------------
+def bfd_assign(size, iota, flags, free_pages):
+    """Largest candidate first (ties: returning before new, least idle, index); each goes to the
+    replica with the most free pages if it fits there, else stays in Waiting (-1)."""
+    size = np.asarray(size, dtype=np.int64)
+    flags = np.asarray(flags, dtype=np.uint8)
+    free = np.asarray(free_pages, dtype=np.int64).copy()
+    m = size.shape[0]
+    pos = np.empty(m, np.int64)
+    pos[rank(iota)] = np.arange(m)
+    order = np.lexsort((pos, (flags & NEW) != 0, -size))
+    rep = np.full(m, -1, np.int32)
+    for i in order:
+        r = int(np.argmax(free))                      # first maximum = lowest replica index
+        if size[i] <= free[r]:
+            rep[i] = r
+            free[r] -= size[i]
+    return rep, free
