@@ -456,6 +456,22 @@ def run_ours(args):
                         "traffic": NCU_TRAFFIC.get("bytes_per_launch"),
                         "traffic_source": NCU_TRAFFIC.get("source")}
 
+    # ---- the shared Waiting queue across replicas: all-gather every replica's
+    #      free GPU pages (NCCL; stays on the device) and pack the same queue on every rank ---------
+    free_all = replicas.gather_free_capacity(max(0, cfg.cap_gpu_pages - int(sum(p.size for p in sim.gpu_pages))),
+                                             device="cuda")
+    wq_rng = np.random.default_rng(SEED)                             # one queue, identical on every rank
+    wq_n = cfg.n_programs                                            # (the context is sized for n programs)
+    wq = [torch.from_numpy(x).cuda() for x in (
+        wq_rng.integers(1, max(2, cfg.max_program_pages // 4), wq_n).astype(np.int32),
+        wq_rng.random(wq_n).astype(np.float32), (2 | (wq_rng.integers(0, 2, wq_n) * 4)).astype(np.uint8))]
+    wq_rep = torch.empty(wq_n, dtype=torch.int32, device="cuda")
+    wq_left = torch.empty_like(free_all)
+    r.mori.mori_bfd_assign(wq[0], wq[1], wq[2], free_all, wq_rep, wq_left)
+    torch.cuda.synchronize()
+    waiting_queue = {"replicas": int(free_all.numel()), "free_pages": free_all.tolist(), "candidates": wq_n,
+                     "admitted_here": int((wq_rep == rank).sum().item()),
+                     "admitted_total": int((wq_rep >= 0).sum().item()), "free_pages_left": wq_left.tolist()}
     r.close()
     rp = rank_partition_leg(with_oracle=(world == 1 and not args.no_cpu_baseline)) if rank == 0 else None
     evl = eviction_leg(with_oracle=(world == 1 and not args.no_cpu_baseline)) if rank == 0 else None
@@ -494,6 +510,7 @@ def run_ours(args):
             "gather_scatter": gs,
             "rank_partition": rp,
             "eviction_order": evl,
+            "waiting_queue_bfd": waiting_queue,
             "cpu_baseline": cpu,
         }
         print(json.dumps(line))
@@ -637,8 +654,28 @@ def rank_partition_leg(with_oracle: bool, reps=200):
         i1.record(cur)
         torch.cuda.synchronize()
         ent["idleness_update_eval_device_us"] = 1e3 * i0.elapsed_time(i1) / reps
+        # NEXT-4(i): Best-Fit-Decreasing of n Waiting-queue candidates across 8 replicas
+        b_free = torch.from_numpy(np.full(8, int(kv.sum()) // 12, np.int64)).to(d)
+        b_rep = torch.empty(n, dtype=torch.int32, device=d); b_left = torch.empty(8, dtype=torch.int64, device=d)
+
+        def call_bfd():
+            m.mori_bfd_assign(t_s, t_i, t_f, b_free, b_rep, b_left, stream=cur)
+        for _ in range(5):
+            call_bfd()
+        torch.cuda.synchronize()
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b0.record(cur)
+        for _ in range(50):
+            call_bfd()
+        b1.record(cur)
+        torch.cuda.synchronize()
+        ent["bfd_device_us_per_call"] = 1e3 * b0.elapsed_time(b1) / 50
         if with_oracle:
             import oracle
+            ts = []
+            for _ in range(10):
+                t0 = time.perf_counter(); oracle.bfd_assign(kv, iota, fl, np.full(8, int(kv.sum()) // 12)); ts.append(time.perf_counter() - t0)
+            ent["bfd_oracle_us_1core"] = 1e6 * float(np.median(ts))
             trk = oracle.IdlenessTracker(n)
             ts = []
             for _ in range(20):

@@ -207,6 +207,26 @@ int mori_eviction_order(mori_ctx* ctx, void* stream, int32_t which_tier, int64_t
                         const uint32_t* last_access, int32_t* victims, int32_t* n_resident);
 
 /*
+ * NEXT-4(i): which replica admits each Waiting-queue promotion: "Waiting-
+ * queue promotions use Best-Fit-Decreasing bin packing across replicas, selecting the replica
+ * with the most available capacity first" (CPU-queue promotions keep their replica and are not
+ * packed).  Every replica runs this on the same inputs -- the shared Waiting queue and
+ * the all-gathered free capacities -- and gets the same answer.  DEVICE pointers, one launch.
+ *
+ *   m            candidates, 0 .. max_programs
+ *   size         [m] int32 KV pages;  idleness [m] float;  flags [m] uint8 (MORI_FLAG_NEW used)
+ *   n_replicas   1 .. 32;  free_pages [n_replicas] int64 >= 0
+ *   replica      [m] out: admitting replica, or -1 = stays in Waiting
+ *   free_out     [n_replicas] out: free pages left (may alias free_pages)
+ * Order: largest first; equal sizes: returning before new, then least idle, then index.  Each
+ * candidate goes to the replica with the most free pages (ties: lowest index) if it fits there,
+ * else nowhere; the packing continues with the next candidate.
+ */
+int mori_bfd_assign(mori_ctx* ctx, void* stream, int32_t m, const int32_t* size, const float* idleness,
+                    const uint8_t* flags, int32_t n_replicas, const int64_t* free_pages,
+                    int32_t* replica, int64_t* free_out);
+
+/*
  * Step a5, demotion ("offloaded to CPU DRAM on the same node"): for every
  * j in [0, total_pages) and every layer l, copy chunk (l, gpu_pages[j]) of the pool to
  * (host_slots[j], l) of the arena.  Asynchronous, on the context's demote stream(s).

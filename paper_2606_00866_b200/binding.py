@@ -31,7 +31,7 @@ EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", 
            "mori_scatter_pages", "mori_profile", "mori_profile_read", "mori_path",
            "mori_copy_kernel", "mori_last_error", "mori_launch_count", "mori_host_alloc",
            "mori_host_free", "mori_sticky_rebalance", "mori_idleness_update",
-           "mori_idleness_eval", "mori_eviction_order"]
+           "mori_idleness_eval", "mori_eviction_order", "mori_bfd_assign"]
 
 
 class MoriConfig(C.Structure):
@@ -67,6 +67,7 @@ def load():
         L.mori_destroy.argtypes = [vp]
         L.mori_rank_partition.argtypes = [vp, vp, i32, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
         L.mori_sticky_rebalance.argtypes = [vp, vp, i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
+        L.mori_bfd_assign.argtypes = [vp, vp, i32, vp, vp, vp, i32, vp, vp, vp]
         L.mori_eviction_order.argtypes = [vp, vp, i32, i64, vp, i32, vp, vp, vp, vp]
         L.mori_idleness_update.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         L.mori_idleness_eval.argtypes = [vp, vp, i32, vp, vp, vp]
@@ -200,6 +201,13 @@ class Mori:
             self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), _ptr(prev_tier),
             _ptr(flags), int(gpu_cap_pages), int(cpu_cap_pages), _ptr(tier), _ptr(lazy),
             _ptr(used_pages), _ptr(lists), _ptr(list_counts)))
+
+    # -- NEXT-4(i): Best-Fit-Decreasing across replicas ------------------------------------------
+    def mori_bfd_assign(self, size, idleness, flags, free_pages, replica, free_out, stream=None):
+        """CUDA tensors int32[m], float32[m], uint8[m], int64[R]; outputs int32[m], int64[R]."""
+        return self._ck(self._lib.mori_bfd_assign(
+            self._h, _stream_handle(stream), int(size.numel()), _ptr(size), _ptr(idleness), _ptr(flags),
+            int(free_pages.numel()), _ptr(free_pages), _ptr(replica), _ptr(free_out)))
 
     # -- NEXT-3: typed eviction order -----------------------------------------------------------
     def mori_eviction_order(self, which_tier, page_owner, program_tier, last_access, victims,

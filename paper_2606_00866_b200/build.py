@@ -14,7 +14,8 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std
          "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 TARGETS = {
-    "libmori.so": (["mori.cu"], ["copy_pages.cuh", "rank_partition.cuh", os.path.join(ROOT, "include", "mori.h")]),
+    "libmori.so": (["mori.cu"], sorted(f for f in os.listdir(CSRC) if f.endswith(".cuh"))
+                   + [os.path.join(ROOT, "include", "mori.h")]),
     "libmori_workload.so": (["workload_fill.cu"], []),
 }
 

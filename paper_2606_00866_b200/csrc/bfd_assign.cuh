@@ -1,0 +1,109 @@
+// bfd_assign.cuh -- NEXT-4(i): Waiting-queue promotions packed across replicas:
+// "Best-Fit-Decreasing bin packing across replicas, selecting the replica with the most available
+// capacity first".  Declared in include/mori.h (mori_bfd_assign).
+//
+// Order: largest candidate first; equal sizes keep the promotion priority (returning before new,
+// least idle, index).  The order comes from ranking unique 128-bit keys by counting on every SM
+// (as in sticky_rebalance.cuh); the last CTA then walks the candidates in that order: one thread
+// keeps every replica's free pages in registers, picks the replica with the most (ties: lowest
+// index) and admits the candidate there if it fits.  The walk is the one inherently sequential
+// step of the rule (every admission changes the next arg-max); a warp-wide shuffle arg-max per
+// candidate measured 3x slower than this single thread (shuffle latency on the critical path).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "rank_partition.cuh"
+
+namespace mori {
+
+constexpr int kBfdMaxReplicas = 32;
+
+// The walk, by ONE thread with every replica's free pages in registers (RP = 8, 16 or 32 slots,
+// unused ones hold -1 and never win): arg-max by an unrolled scan (first maximum = lowest index),
+// recomputed only after an admission -- a candidate that does not fit leaves it unchanged.
+template <int RP>
+__device__ __forceinline__ void bfd_walk(int m, const int32_t* ssize, int32_t* sdest, int n_replicas,
+                                         const long long* __restrict__ free_pages, long long* __restrict__ free_out) {
+  long long fr[RP];
+#pragma unroll
+  for (int r = 0; r < RP; ++r) fr[r] = r < n_replicas ? free_pages[r] : -1;
+  long long best = fr[0]; int who = 0;
+#pragma unroll
+  for (int r = 1; r < RP; ++r) if (fr[r] > best) { best = fr[r]; who = r; }
+  int s_next = m > 0 ? ssize[0] : 0;
+  for (int k = 0; k < m; ++k) {
+    const int s = s_next;
+    if (k + 1 < m) s_next = ssize[k + 1];
+    if ((long long)s <= best) {
+      sdest[k] = who;
+#pragma unroll
+      for (int r = 0; r < RP; ++r) fr[r] -= r == who ? (long long)s : 0;
+      best = fr[0]; who = 0;
+#pragma unroll
+      for (int r = 1; r < RP; ++r) if (fr[r] > best) { best = fr[r]; who = r; }
+    } else {
+      sdest[k] = -1;
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < RP; ++r) if (r < n_replicas) free_out[r] = fr[r];
+}
+
+__global__ void __launch_bounds__(kRankMaxThreads, 1)
+bfd_assign_kernel(int m, const int32_t* __restrict__ size, const float* __restrict__ idleness,
+                  const uint8_t* __restrict__ flags, int n_replicas, const long long* __restrict__ free_pages,
+                  int32_t* __restrict__ replica, long long* __restrict__ free_out,
+                  int32_t* __restrict__ order, unsigned int* __restrict__ ticket) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint64_t* khi = reinterpret_cast<uint64_t*>(smem_raw);             // [m]
+  uint64_t* klo = khi + m;                                           // [m]
+  __shared__ unsigned int s_ticket;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+
+  for (int i = tid; i < m; i += blockDim.x) {
+    const int s = size[i] > 0 ? size[i] : 0;
+    khi[i] = ((uint64_t)(~(uint32_t)s) << 1) | ((flags[i] & 4) ? 1u : 0u);   // size descending, then class
+    klo[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;       // least idle, then index
+  }
+  __syncthreads();
+  const int per = (m + gridDim.x - 1) / gridDim.x;
+  const int lo_i = blockIdx.x * per, hi_i = min(m, lo_i + per);
+  for (int i = lo_i + warp; i < hi_i; i += n_warps) {
+    const uint64_t h = khi[i], l = klo[i];
+    int c = 0;
+    for (int j = lane; j < m; j += 32) {
+      const uint64_t hj = khi[j];
+      c += (hj < h) || (hj == h && klo[j] < l);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
+    if (lane == 0) order[c] = i;
+  }
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);
+  __syncthreads();
+  if (s_ticket != gridDim.x - 1) return;
+  if (tid == 0) *ticket = 0;
+  __threadfence();
+
+  // ---- last CTA: sizes in packing order into shared memory, then the one-warp walk ---------------
+  int32_t* ssize = reinterpret_cast<int32_t*>(khi);                  // [m] (keys are dead)
+  int32_t* sdest = reinterpret_cast<int32_t*>(klo);                  // [m]
+  __syncthreads();
+  for (int k = tid; k < m; k += blockDim.x) {
+    const int s = size[__ldcg(order + k)];
+    ssize[k] = s > 0 ? s : 0;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    if (n_replicas <= 8) bfd_walk<8>(m, ssize, sdest, n_replicas, free_pages, free_out);
+    else if (n_replicas <= 16) bfd_walk<16>(m, ssize, sdest, n_replicas, free_pages, free_out);
+    else bfd_walk<32>(m, ssize, sdest, n_replicas, free_pages, free_out);
+  }
+  __syncthreads();
+  for (int k = tid; k < m; k += blockDim.x) replica[__ldcg(order + k)] = sdest[k];
+}
+
+}  // namespace mori

@@ -22,6 +22,7 @@
 #include "sticky_rebalance.cuh"
 #include "idleness.cuh"
 #include "eviction_order.cuh"
+#include "bfd_assign.cuh"
 
 namespace {
 
@@ -472,6 +473,29 @@ int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idl
   }
 #undef LS
   CK(c, e);
+  c->launches += 1;
+  return MORI_OK;
+}
+
+int mori_bfd_assign(mori_ctx* c, void* stream, int32_t m, const int32_t* size, const float* idleness,
+                    const uint8_t* flags, int32_t n_replicas, const int64_t* free_pages, int32_t* replica,
+                    int64_t* free_out) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (m < 0 || m > c->cfg.max_programs) return fail(c, MORI_ERR_INVALID_ARG, "m out of range (0..max_programs)");
+  if (n_replicas < 1 || n_replicas > mori::kBfdMaxReplicas) return fail(c, MORI_ERR_UNSUPPORTED, "n_replicas must be 1..32");
+  if (!free_pages || !free_out || (m > 0 && (!size || !idleness || !flags || !replica)))
+    return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
+  const int grid = std::max(1, std::min(c->sm_count, (m + 31) / 32));
+  const size_t smem = sizeof(uint64_t) * 2 * (size_t)std::max(m, 1);
+  const unsigned long long slot = c->rank_seq++ % kRankTickets;
+  if (smem > 48 * 1024)
+    CK(c, cudaFuncSetAttribute(mori::bfd_assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  mori::bfd_assign_kernel<<<grid, mori::kRankMaxThreads, smem, static_cast<cudaStream_t>(stream)>>>(
+      m, size, idleness, flags, n_replicas, reinterpret_cast<const long long*>(free_pages), replica,
+      reinterpret_cast<long long*>(free_out), c->sticky_order + slot * (size_t)c->cfg.max_programs,
+      c->rank_tickets + slot);
+  CK(c, cudaGetLastError());
   c->launches += 1;
   return MORI_OK;
 }

@@ -4,8 +4,9 @@ The paper's placement is per replica: "Each inference engine replica maintains i
 queues" and every replica "appl[ies] the same rule of filling from the busiest end of the
 ranking until local capacity is reached".  So rank r runs the whole hot path on its own
 programs (its own seeded trace), its own pool and its own pinned arena over its own host link;
-nothing of the KV path crosses NVLink.  The only cross-rank step is the bookkeeping below: the
-job's time is the slowest rank's, its work the sum -- one all-reduce of a few float64 through
+nothing of the KV path crosses NVLink.  The cross-rank steps are bookkeeping: the job's time is
+the slowest rank's, its work the sum (one all-reduce of a few float64), and -- for the shared
+Waiting queue of P:L180 -- an all-gather of each replica's free capacity, through
 ``torch.distributed`` (NCCL on GPUs, gloo in the CPU tests).
 """
 from __future__ import annotations
@@ -37,6 +38,21 @@ def aggregate(times_s: Sequence[float], sums: Sequence[float], device="cpu"):
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     dist.all_reduce(s, op=dist.ReduceOp.SUM)
     return t.tolist(), s.tolist()
+
+
+def gather_free_capacity(free_local_pages: int, device="cpu"):
+    """The one piece of cross-replica data of the paper's design: every replica's free GPU pages,
+    all-gathered so that each replica can run the same Best-Fit-Decreasing packing of the shared
+    Waiting queue (``mori_bfd_assign``).  -> int64 tensor [world] on ``device``
+    (stays on the GPU under NCCL, so it feeds the kernel without a host round trip)."""
+    import torch
+    import torch.distributed as dist
+    mine = torch.tensor([int(free_local_pages)], dtype=torch.int64, device=device)
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return mine
+    parts = [torch.empty_like(mine) for _ in range(dist.get_world_size())]
+    dist.all_gather(parts, mine)
+    return torch.cat(parts)
 
 
 def throughput_gbps(times_s: Sequence[float], bytes_moved: Sequence[float], device="cpu") -> float:

@@ -47,7 +47,15 @@ def _worker(rank, world, port, q):
     t_local = 0.25 * (rank + 1)                      # rank 1 is the slow one
     (t,), (b, n) = replicas.aggregate([t_local], [moved, 1.0])
     gbps = replicas.throughput_gbps([t_local], [moved])
-    q.put((rank, t, b, n, gbps, moved, [x.tolist() for x in tiers]))
+    # shared Waiting queue: all-gather the replicas' free capacity, pack with the oracle's BFD
+    import numpy as np, oracle
+    free = replicas.gather_free_capacity(100 * (rank + 1) + 7).numpy()
+    rng = np.random.default_rng(12)                                   # the same queue on every rank
+    size = rng.integers(1, 60, 25).astype(np.int32)
+    iota = rng.random(25).astype(np.float32)
+    flags = (2 | (rng.integers(0, 2, 25) * 4)).astype(np.uint8)
+    rep, left = oracle.bfd_assign(size, iota, flags, free)
+    q.put((rank, t, b, n, gbps, moved, [x.tolist() for x in tiers], free.tolist(), rep.tolist(), left.tolist()))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -65,7 +73,10 @@ def test_two_replicas_aggregate_like_the_bench():
         assert p.exitcode == 0
     sys.path.insert(0, ROOT)
     want = [_replica_epochs(r) for r in range(2)]
-    for r, (rank, t, b, n, gbps, moved, tiers) in enumerate(got):
+    assert got[0][7] == got[1][7] == [107, 207]                      # every rank sees every capacity
+    assert got[0][8] == got[1][8] and got[0][9] == got[1][9]          # ... and packs identically
+    assert {0, 1} <= set(got[0][8])                                   # both replicas admit someone
+    for r, (rank, t, b, n, gbps, moved, tiers, *_rest) in enumerate(got):
         assert rank == r
         assert moved == want[r][0]                                  # replicas are deterministic
         assert tiers == [x.tolist() for x in want[r][1]]
@@ -81,3 +92,4 @@ def test_single_replica_aggregate_is_identity():
     assert replicas.aggregate([1.5, 2.0], [3.0]) == ([1.5, 2.0], [3.0])
     assert replicas.throughput_gbps([1.0, 1.0], [4e9]) == 2.0
     assert replicas.replica_seed(866, 3) == 869
+    assert replicas.gather_free_capacity(42).tolist() == [42]
