@@ -50,14 +50,6 @@ GIB = 1 << 30
 # ------------------------------------------------------------------------------------------------
 # helpers
 # ------------------------------------------------------------------------------------------------
-def _mem_available_bytes() -> int:
-    with open("/proc/meminfo") as f:
-        for line in f:
-            if line.startswith("MemAvailable:"):
-                return int(line.split()[1]) * 1024
-    return 0
-
-
 def _meminfo_kb(key: str) -> int:
     with open("/proc/meminfo") as f:
         for line in f:
@@ -68,9 +60,10 @@ def _meminfo_kb(key: str) -> int:
 
 def _pick_scale(cfg_index: int, world: int, W) -> int:
     """SURVEY 8(d) scale rule: the smallest power of two that lets the pinned arena of every
-    rank fit host RAM (80 % of MemAvailable) and the pool fit HBM."""
+    rank fit host RAM (70 % of MemTotal, shared by the ranks of the node -- MemTotal, not
+    MemAvailable, so that every rank of a job picks the same scale) and the pool fit HBM."""
     import torch
-    avail = int(_mem_available_bytes() * 0.80) // max(1, world)
+    avail = int(_meminfo_kb("MemTotal") * 1024 * 0.70) // max(1, world)
     free_hbm, _ = torch.cuda.mem_get_info()
     scale = 1
     while True:
@@ -516,6 +509,7 @@ def run_ours(args):
         print(json.dumps(line))
     binding.Mori.mori_host_free(arena)
     if world > 1:
+        dist.barrier()                      # rank 0 is still running its single-rank legs
         dist.destroy_process_group()
 
 
