@@ -75,6 +75,9 @@ struct mori_ctx {
   unsigned long long rank_seq = 0;
   int idl_k = 5;                                 // window of Eq. (1)
   double* idl_r = nullptr; double* idl_a = nullptr; int32_t* idl_pushed = nullptr;   // [max_programs][k], [max_programs]
+  // the 16-node sequence of mori_eviction_order, captured once per argument set and replayed
+  cudaGraphExec_t evict_exec = nullptr; cudaStream_t evict_cap_stream = nullptr;
+  struct { int tier, n_programs; long long n_pages; const void *owner, *ptier, *last; void *victims, *nres; } evict_key{};
   int32_t* evict_perm[2] = {nullptr, nullptr}; int32_t* evict_table = nullptr; long long evict_cap = 0;   // scratch, grown on demand
   int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
   Direction dir[2];                              // 0 demote, 1 promote
@@ -392,6 +395,8 @@ int mori_destroy(mori_ctx* c) {
   for (auto ev : c->free_events) cudaEventDestroy(ev);
   if (c->rank_tickets) cudaFree(c->rank_tickets);
   if (c->sticky_order) cudaFree(c->sticky_order);
+  if (c->evict_exec) cudaGraphExecDestroy(c->evict_exec);
+  if (c->evict_cap_stream) cudaStreamDestroy(c->evict_cap_stream);
   for (int b = 0; b < 2; ++b) if (c->evict_perm[b]) cudaFree(c->evict_perm[b]);
   if (c->evict_table) cudaFree(c->evict_table);
   if (c->idl_r) cudaFree(c->idl_r);
@@ -512,11 +517,11 @@ int mori_eviction_order(mori_ctx* c, void* stream, int32_t which_tier, int64_t n
   if (n_pages > 0 && (!page_owner || !last_access || !victims || (n_programs > 0 && !program_tier)))
     return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  CK(c, cudaMemsetAsync(n_resident, 0, sizeof(int32_t), s));
-  if (n_pages == 0) return MORI_OK;
+  if (n_pages == 0) { CK(c, cudaMemsetAsync(n_resident, 0, sizeof(int32_t), s)); return MORI_OK; }
   const int tiles = (int)((n_pages + mori::kEvictTile - 1) / mori::kEvictTile);
   if (n_pages > c->evict_cap) {                    // first use / larger pool: (re)allocate scratch
     CK(c, cudaStreamSynchronize(s));
+    if (c->evict_exec) { cudaGraphExecDestroy(c->evict_exec); c->evict_exec = nullptr; }
     for (int b = 0; b < 2; ++b) { if (c->evict_perm[b]) cudaFree(c->evict_perm[b]); c->evict_perm[b] = nullptr; }
     if (c->evict_table) cudaFree(c->evict_table);
     c->evict_table = nullptr; c->evict_cap = 0;
@@ -525,16 +530,45 @@ int mori_eviction_order(mori_ctx* c, void* stream, int32_t which_tier, int64_t n
     c->evict_cap = n_pages;
   }
   mori::EvictArgs a{n_pages, n_programs, which_tier == MORI_TIER_GPU ? 0 : 1, tiles, page_owner, program_tier, last_access};
-  const int32_t* in = nullptr;                     // pass 0 reads the pages in id order
-  for (int pass = 0; pass < mori::kEvictPasses; ++pass) {
-    int32_t* out = pass == mori::kEvictPasses - 1 ? victims : c->evict_perm[pass & 1];
-    mori::evict_hist_kernel<<<tiles, mori::kEvictTile, 0, s>>>(a, pass, in, c->evict_table, n_resident);
-    mori::evict_scan_kernel<<<1, mori::kRankMaxThreads, 0, s>>>(c->evict_table, 256 * tiles);
-    mori::evict_scatter_kernel<<<tiles, mori::kEvictTile, 0, s>>>(a, pass, in, c->evict_table, out);
-    CK(c, cudaGetLastError());
-    c->launches += 3;
-    in = out;
+  auto enqueue = [&](cudaStream_t q) -> cudaError_t {
+    cudaError_t e = cudaMemsetAsync(n_resident, 0, sizeof(int32_t), q);
+    if (e != cudaSuccess) return e;
+    const int32_t* in = nullptr;                   // pass 0 reads the pages in id order
+    for (int pass = 0; pass < mori::kEvictPasses; ++pass) {
+      int32_t* out = pass == mori::kEvictPasses - 1 ? victims : c->evict_perm[pass & 1];
+      mori::evict_hist_kernel<<<tiles, mori::kEvictTile, 0, q>>>(a, pass, in, c->evict_table, n_resident);
+      mori::evict_scan_kernel<<<1, mori::kRankMaxThreads, 0, q>>>(c->evict_table, 256 * tiles);
+      mori::evict_scatter_kernel<<<tiles, mori::kEvictTile, 0, q>>>(a, pass, in, c->evict_table, out);
+      in = out;
+    }
+    return cudaGetLastError();
+  };
+  // Launch-bound (15 small kernels + a memset): captured once into a CUDA graph per argument set
+  // -- an engine passes the same tables every time -- and replayed with one cudaGraphLaunch.
+  const bool same = c->evict_exec && c->evict_key.tier == which_tier && c->evict_key.n_programs == n_programs &&
+                    c->evict_key.n_pages == n_pages && c->evict_key.owner == page_owner &&
+                    c->evict_key.ptier == program_tier && c->evict_key.last == last_access &&
+                    c->evict_key.victims == victims && c->evict_key.nres == n_resident;
+  if (!same) {
+    if (c->evict_exec) { cudaGraphExecDestroy(c->evict_exec); c->evict_exec = nullptr; }
+    if (!c->evict_cap_stream) cudaStreamCreateWithFlags(&c->evict_cap_stream, cudaStreamNonBlocking);
+    cudaGraph_t g = nullptr;
+    if (c->evict_cap_stream &&
+        cudaStreamBeginCapture(c->evict_cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      const cudaError_t e1 = enqueue(c->evict_cap_stream);
+      const cudaError_t e2 = cudaStreamEndCapture(c->evict_cap_stream, &g);
+      if (e1 == cudaSuccess && e2 == cudaSuccess && g &&
+          cudaGraphInstantiate(&c->evict_exec, g, 0) != cudaSuccess)
+        c->evict_exec = nullptr;
+      if (e1 != cudaSuccess || e2 != cudaSuccess) c->evict_exec = nullptr;
+      if (g) cudaGraphDestroy(g);
+    }
+    cudaGetLastError();                            // a failed capture falls back to plain launches
+    c->evict_key = {which_tier, n_programs, n_pages, page_owner, program_tier, last_access, victims, n_resident};
   }
+  if (c->evict_exec) CK(c, cudaGraphLaunch(c->evict_exec, s));
+  else CK(c, enqueue(s));
+  c->launches += 3 * mori::kEvictPasses;
   return MORI_OK;
 }
 
