@@ -188,3 +188,27 @@ def test_sticky_policy_epochs_full_mirror(mori, idx, scale, epochs):
     epoch), bytes moved by mori_demote / mori_promote, both pools mirrored byte for byte."""
     moved = _epochs_with_mirror(mori, W.get_config(idx, scale), 866, epochs, 0, 2, sticky=True)
     assert moved > 0
+
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_many_calls_without_a_join_wrap_the_index_ring(mori, path):
+    """The library stages page/slot ids in a pinned ring (64 Ki entries at least); 700 calls of 60
+    pages with no mori_sync in between overflow it, which must drain the streams and carry on."""
+    L, H, D, T, P, S = 1, 1, 8, 1, 4096, 4096            # 32-byte pages
+    m, pool, arena, pool_m, arena_m, chunk = _mk_ctx(mori, L, H, D, T, P, S, path, 2, staging=64 * 32)
+    rng = np.random.default_rng(11)
+    for call in range(700):
+        g = rng.integers(0, P, 60).astype(np.int32)
+        h = rng.permutation(S)[:60].astype(np.int32)
+        m.mori_demote(g, h)
+        oracle.demote(L, chunk, pool_m, arena_m, g, h)       # later calls overwrite earlier slots: order matters
+    m.mori_sync(mori.BOTH)
+    assert np.array_equal(arena.numpy(), arena_m)
+    for call in range(700):
+        h = rng.integers(0, S, 60).astype(np.int32)
+        g = rng.permutation(P)[:60].astype(np.int32)
+        m.mori_promote(h, g)
+        oracle.promote(L, chunk, pool_m, arena_m, h, g)
+    m.mori_sync(mori.BOTH)
+    assert np.array_equal(pool.cpu().numpy(), pool_m)
+    m.close()
