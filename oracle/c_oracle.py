@@ -39,6 +39,8 @@ def _load():
         L.oracle_bruteforce_partition.restype = C.c_int
         L.oracle_sticky_rebalance.argtypes = [i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
         L.oracle_sticky_rebalance.restype = C.c_int
+        L.oracle_rank_partition_tiers.argtypes = [i32, vp, vp, i32, vp, vp, vp, vp, vp]
+        L.oracle_rank_partition_tiers.restype = C.c_int
         L.oracle_bfd_assign.argtypes = [i32, vp, vp, vp, i32, vp, vp, vp]
         L.oracle_bfd_assign.restype = C.c_int
         L.oracle_eviction_order.argtypes = [i32, i64, vp, i32, vp, vp, vp, C.POINTER(i64)]
@@ -104,6 +106,20 @@ def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
         raise ValueError(f"oracle_sticky_rebalance: bad argument (rc={rc})")
     return dict(tier=tier[:n], lazy=lazy[:n], used=used,
                 lists=[lists[k, :counts[k]].copy() for k in range(5)])
+
+
+def rank_partition_tiers(iota, s, caps):
+    """oracle_rank_partition_tiers -> dict(order, tier (T = waiting), bounds[T], used[T])."""
+    iota = np.ascontiguousarray(iota, dtype=np.float32)
+    s = np.ascontiguousarray(s, dtype=np.int32)
+    caps = np.ascontiguousarray(caps, dtype=np.int64)
+    n, T = iota.size, caps.size
+    order = np.empty(max(n, 1), np.int32); tier = np.empty(max(n, 1), np.uint8)
+    bounds = np.zeros(max(T, 1), np.int32); used = np.zeros(max(T, 1), np.int64)
+    rc = _load().oracle_rank_partition_tiers(n, _p(iota), _p(s), T, _p(caps), _p(order), _p(tier), _p(bounds), _p(used))
+    if rc != 0:
+        raise ValueError(f"oracle_rank_partition_tiers: bad argument (rc={rc})")
+    return dict(order=order[:n], tier=tier[:n], bounds=bounds[:T], used=used[:T])
 
 
 def bfd_assign(size, iota, flags, free_pages):

@@ -478,3 +478,34 @@ int oracle_bfd_assign(int32_t m, const int32_t *size, const float *iota, const u
   free(keys);
   return ORACLE_OK;
 }
+
+/*
+ * NEXT-4(ii): more offloading tiers: "the design generalizes naturally to
+ * more hierarchies ... introducing a second idleness threshold: programs with iota between the
+ * two thresholds would be offloaded to [the next tier] ... treating remote DRAM as an
+ * intermediate tier".  The same rule as oracle_rank_partition with T capacities instead of two:
+ * tier t takes the longest run of the ranking, right after tier t-1, that fits cap[t]
+ * ("filling from the busiest end of the ranking until local capacity is reached");
+ * what is left is Waiting (tier value T).
+ */
+int oracle_rank_partition_tiers(int32_t n, const float *iota, const int32_t *s, int32_t n_tiers,
+                                const int64_t *cap, int32_t *order, uint8_t *tier, int32_t *bounds,
+                                int64_t *used) {
+  if (n < 0 || n_tiers < 1 || n_tiers > 8 || !cap) return ORACLE_ERR_ARG;
+  for (int t = 0; t < n_tiers; ++t) if (cap[t] < 0) return ORACLE_ERR_ARG;
+  for (int32_t p = 0; p < n; ++p) if (s[p] < 0) return ORACLE_ERR_ARG;
+  prog_key *keys = (prog_key *)malloc(sizeof(prog_key) * (size_t)(n > 0 ? n : 1));
+  if (!keys) return ORACLE_ERR_ARG;
+  for (int32_t p = 0; p < n; ++p) { keys[p].iota = iota[p]; keys[p].idx = p; }
+  qsort(keys, (size_t)n, sizeof(prog_key), cmp_keys);
+  for (int32_t r = 0; r < n; ++r) order[r] = keys[r].idx;
+  free(keys);
+  int32_t b = 0;
+  for (int t = 0; t < n_tiers; ++t) {
+    int64_t sum = 0;
+    while (b < n && sum + s[order[b]] <= cap[t]) { sum += s[order[b]]; tier[order[b]] = (uint8_t)t; ++b; }
+    bounds[t] = b; used[t] = sum;
+  }
+  for (int32_t r = b; r < n; ++r) tier[order[r]] = (uint8_t)n_tiers;
+  return ORACLE_OK;
+}

@@ -166,3 +166,24 @@ def bfd_assign(size, iota, flags, free_pages):
             rep[i] = r
             free[r] -= size[i]
     return rep, free
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4(ii): the partition with T capacities
+# ------------------------------------------------------------------------------------------------
+def rank_partition_tiers(iota, s, caps):
+    s = np.asarray(s, dtype=np.int64)
+    n = s.shape[0]
+    order = rank(iota)
+    incl = np.cumsum(s[order])
+    tier = np.full(n, len(caps), np.uint8)
+    bounds, used, b, base = [], [], 0, 0
+    for t, c in enumerate(caps):
+        nb = max(b, int(np.searchsorted(incl, base + int(c), side="right")))
+        tier[order[b:nb]] = t
+        top = int(incl[nb - 1]) if nb > 0 else 0
+        used.append(top - base if nb > b else 0)
+        base = top if nb > b else base
+        b = nb
+        bounds.append(b)
+    return dict(order=order, tier=tier, bounds=np.array(bounds, np.int32), used=np.array(used, np.int64))
