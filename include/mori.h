@@ -73,7 +73,10 @@ typedef struct {
   void*   gpu_pool;          /* DEVICE, caller-owned, 16-byte aligned */
   int64_t gpu_pool_pages;
   void*   host_arena;        /* PINNED, caller-owned, 16-byte aligned; may be NULL if neither
-                                mori_demote nor mori_promote is used */
+                                mori_demote nor mori_promote is used.  May instead be DEVICE
+                                memory (this GPU's, or a peer GPU's with peer access enabled:
+                                the intermediate tier of P:L347): both directions then run as
+                                one full-grid kernel, path_* are ignored */
   int64_t host_arena_slots;
   int32_t max_programs;      /* 1 .. MORI_MAX_PROGRAMS */
   int32_t path_demote;       /* MORI_PATH_* */
@@ -225,6 +228,22 @@ int mori_eviction_order(mori_ctx* ctx, void* stream, int32_t which_tier, int64_t
 int mori_bfd_assign(mori_ctx* ctx, void* stream, int32_t m, const int32_t* size, const float* idleness,
                     const uint8_t* flags, int32_t n_replicas, const int64_t* free_pages,
                     int32_t* replica, int64_t* free_out);
+
+/*
+ * NEXT-4(ii): the ranking cut by n_tiers capacities instead of two, P:L339-351 ("the
+ * design generalizes naturally to more hierarchies ... a second idleness threshold ... an
+ * intermediate tier"; "filling from the busiest end of the ranking until local capacity is
+ * reached").  Tier t (0 = GPU HBM, then e.g. peer HBM over NVLink, host DRAM, SSD ...) takes the
+ * longest run of the ranking right after tier t-1 whose kv_pages fit cap_pages[t]; the rest is
+ * Waiting, written as tier value n_tiers.  With n_tiers = 2 this is mori_rank_partition without
+ * the move lists.  One launch on `stream`; array pointers are DEVICE pointers.
+ *
+ *   n_tiers      1 .. 8;  cap_pages  HOST int64[n_tiers], >= 0, read before the call returns
+ *   order [n], tier [n], bounds [n_tiers] (end rank of every tier), used_pages [n_tiers]: out
+ */
+int mori_rank_partition_tiers(mori_ctx* ctx, void* stream, int32_t n, const float* idleness,
+                              const int32_t* kv_pages, int32_t n_tiers, const int64_t* cap_pages,
+                              int32_t* order, uint8_t* tier, int32_t* bounds, int64_t* used_pages);
 
 /*
  * Step a5, demotion ("offloaded to CPU DRAM on the same node"): for every

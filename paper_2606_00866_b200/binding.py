@@ -31,7 +31,8 @@ EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", 
            "mori_scatter_pages", "mori_profile", "mori_profile_read", "mori_path",
            "mori_copy_kernel", "mori_last_error", "mori_launch_count", "mori_host_alloc",
            "mori_host_free", "mori_sticky_rebalance", "mori_idleness_update",
-           "mori_idleness_eval", "mori_eviction_order", "mori_bfd_assign"]
+           "mori_idleness_eval", "mori_eviction_order", "mori_bfd_assign",
+           "mori_rank_partition_tiers"]
 
 
 class MoriConfig(C.Structure):
@@ -67,6 +68,7 @@ def load():
         L.mori_destroy.argtypes = [vp]
         L.mori_rank_partition.argtypes = [vp, vp, i32, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
         L.mori_sticky_rebalance.argtypes = [vp, vp, i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
+        L.mori_rank_partition_tiers.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp, vp, vp]
         L.mori_bfd_assign.argtypes = [vp, vp, i32, vp, vp, vp, i32, vp, vp, vp]
         L.mori_eviction_order.argtypes = [vp, vp, i32, i64, vp, i32, vp, vp, vp, vp]
         L.mori_idleness_update.argtypes = [vp, vp, i64, vp, vp, vp, vp]
@@ -138,7 +140,7 @@ class Mori:
         self.host_arena_slots = 0
         if host_arena is not None:
             arena_bytes = host_arena.numel() * host_arena.element_size()
-            assert (not host_arena.is_cuda) and host_arena.is_pinned() and host_arena.is_contiguous()
+            assert (host_arena.is_cuda or host_arena.is_pinned()) and host_arena.is_contiguous()
             assert arena_bytes % self.page_bytes == 0
             self.host_arena_slots = arena_bytes // self.page_bytes
             cfg.host_arena, cfg.host_arena_slots = host_arena.data_ptr(), self.host_arena_slots
@@ -201,6 +203,15 @@ class Mori:
             self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), _ptr(prev_tier),
             _ptr(flags), int(gpu_cap_pages), int(cpu_cap_pages), _ptr(tier), _ptr(lazy),
             _ptr(used_pages), _ptr(lists), _ptr(list_counts)))
+
+    # -- NEXT-4(ii): the partition with T capacities --------------------------------------------
+    def mori_rank_partition_tiers(self, n, idleness, kv_pages, cap_pages, order, tier, bounds,
+                                  used_pages, stream=None):
+        """``cap_pages``: host sequence of 1..8 capacities; the rest are CUDA tensors."""
+        caps = np.ascontiguousarray(cap_pages, dtype=np.int64)
+        return self._ck(self._lib.mori_rank_partition_tiers(
+            self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), int(caps.size),
+            caps.ctypes.data, _ptr(order), _ptr(tier), _ptr(bounds), _ptr(used_pages)))
 
     # -- NEXT-4(i): Best-Fit-Decreasing across replicas ------------------------------------------
     def mori_bfd_assign(self, size, idleness, flags, free_pages, replica, free_out, stream=None):

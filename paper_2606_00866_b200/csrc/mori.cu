@@ -71,6 +71,7 @@ struct mori_ctx {
   int link_ctas = 32;
   size_t tma_smem = 0;
   unsigned char* arena_dev = nullptr;            // device-side alias of the pinned arena
+  bool arena_is_device = false;                  // arena lives in (this or a peer GPU's) HBM
   unsigned int* rank_tickets = nullptr;          // [kRankTickets] last-CTA counters of the multi-CTA ranker
   unsigned long long rank_seq = 0;
   int idl_k = 5;                                 // window of Eq. (1)
@@ -253,6 +254,20 @@ cudaError_t launch_rank_multi(int grid, size_t smem, cudaStream_t s, int n, cons
 }
 
 template <int IPT>
+cudaError_t launch_tiers(int grid, size_t smem, cudaStream_t s, int n, const float* idl, const int32_t* kv,
+                         const mori::TierCaps& caps, int32_t* order, uint8_t* tier, int32_t* bounds,
+                         long long* used, unsigned int* ticket) {
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(mori::rank_tiers_kernel<IPT>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  mori::rank_tiers_kernel<IPT><<<grid, mori::kRankMaxThreads, smem, s>>>(n, idl, kv, caps, order, tier, bounds,
+                                                                        used, ticket);
+  return cudaGetLastError();
+}
+
+template <int IPT>
 cudaError_t launch_sticky(int grid, size_t smem, cudaStream_t s, int n, const float* idl, const int32_t* kv,
                                  const uint8_t* prev, const uint8_t* flags, long long cg, long long cc,
                                  uint8_t* tier, uint8_t* lazy, long long* used, int32_t* lists, int32_t* counts,
@@ -347,9 +362,20 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   CKC(cudaMemset(c->idl_pushed, 0, sizeof(int32_t) * (size_t)cfg->max_programs));
   CKC(cudaMalloc((void**)&c->sticky_order, sizeof(int32_t) * kRankTickets * (size_t)cfg->max_programs));
   if (cfg->host_arena) {
-    void* dp = nullptr;
-    CKC(cudaHostGetDevicePointer(&dp, cfg->host_arena, 0));
-    c->arena_dev = static_cast<unsigned char*>(dp);
+    // The arena may also be DEVICE memory -- a second pool in this GPU's HBM, or a peer GPU's HBM
+    // mapped over NVLink (the intermediate tier of P:L347): then there is no host link to stage
+    // for, and both directions are the one-kernel path at full grid.
+    cudaPointerAttributes at{};
+    if (cudaPointerGetAttributes(&at, cfg->host_arena) == cudaSuccess && at.type == cudaMemoryTypeDevice) {
+      c->arena_is_device = true;
+      c->arena_dev = static_cast<unsigned char*>(cfg->host_arena);
+      for (int i = 0; i < 2; ++i) { c->dir[i].path = MORI_PATH_ZEROCOPY; c->dir[i].auto_path = false; }
+    } else {
+      cudaGetLastError();
+      void* dp = nullptr;
+      CKC(cudaHostGetDevicePointer(&dp, cfg->host_arena, 0));
+      c->arena_dev = static_cast<unsigned char*>(dp);
+    }
   }
   for (int i = 0; i < 2; ++i) {
     Direction& d = c->dir[i];
@@ -477,6 +503,41 @@ int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idl
     default: e = LS(8); break;
   }
 #undef LS
+  CK(c, e);
+  c->launches += 1;
+  return MORI_OK;
+}
+
+int mori_rank_partition_tiers(mori_ctx* c, void* stream, int32_t n, const float* idleness, const int32_t* kv_pages,
+                              int32_t n_tiers, const int64_t* cap_pages, int32_t* order, uint8_t* tier,
+                              int32_t* bounds, int64_t* used) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  if (n < 0 || n > c->cfg.max_programs) return fail(c, MORI_ERR_INVALID_ARG, "n out of range (0..max_programs)");
+  if (n_tiers < 1 || n_tiers > mori::kMaxTiers || !cap_pages) return fail(c, MORI_ERR_INVALID_ARG, "n_tiers must be 1..8");
+  if (!bounds || !used || (n > 0 && (!idleness || !kv_pages || !order || !tier))) return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
+  mori::TierCaps caps{};
+  caps.n_tiers = n_tiers;
+  for (int t = 0; t < n_tiers; ++t) {
+    if (cap_pages[t] < 0) return fail(c, MORI_ERR_INVALID_ARG, "negative capacity");
+    caps.cap[t] = cap_pages[t];
+  }
+  int n_pad = 1024;
+  while (n_pad < n) n_pad <<= 1;
+  const int grid = std::max(1, std::min(c->sm_count, (n + 31) / 32));
+  const size_t smem = sizeof(uint64_t) * ((size_t)n + 33) + 2 * sizeof(long long);
+  unsigned int* tk = c->rank_tickets + (c->rank_seq++ % kRankTickets);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  long long* u = reinterpret_cast<long long*>(used);
+  cudaError_t e;
+#define LT(I) launch_tiers<I>(grid, smem, s, n, idleness, kv_pages, caps, order, tier, bounds, u, tk)
+  switch (n_pad / 1024) {
+    case 1: e = LT(1); break;
+    case 2: e = LT(2); break;
+    case 4: e = LT(4); break;
+    default: e = LT(8); break;
+  }
+#undef LT
   CK(c, e);
   c->launches += 1;
   return MORI_OK;
@@ -652,7 +713,7 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
       if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;
       mori::CopyArgs a = make_args(c, c->arena_dev, dg, dh, total);
       prof_begin(c, d, d.kern, total * pb);
-      CK(c, demote ? launch_copy<true>(c, a, d.kern, true) : launch_copy<false>(c, a, d.kern, true));
+      CK(c, demote ? launch_copy<true>(c, a, d.kern, !c->arena_is_device) : launch_copy<false>(c, a, d.kern, !c->arena_is_device));
       prof_end(c, d, d.kern);
     }
     return issue_ticket(c, d, d.kern, ticket_out);

@@ -287,4 +287,94 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
                       list_counts, warp_tot, bcast);
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT-4(ii): the same ranking cut by T capacities instead of two ("a second idleness
+// threshold", "an intermediate tier"): tier t = the longest run of the ranking right after tier
+// t-1 whose pages fit cap[t]; the rest is Waiting (tier value T).  Declared in include/mori.h
+// (mori_rank_partition_tiers).  Ranking by counting on every SM for every n, last CTA cuts.
+constexpr int kMaxTiers = 8;
+struct TierCaps { long long cap[kMaxTiers]; int n_tiers; };
+
+template <int IPT>
+__global__ void __launch_bounds__(kRankMaxThreads, 1)
+rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __restrict__ kv_pages,
+                  const TierCaps caps, int32_t* __restrict__ order, uint8_t* __restrict__ tier,
+                  int32_t* __restrict__ bounds, long long* __restrict__ used,
+                  unsigned int* __restrict__ ticket) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
+  uint64_t* warp_tot = keys + n;                                     // [33]
+  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
+  __shared__ unsigned int s_ticket;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+  for (int i = tid; i < n; i += blockDim.x)
+    keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;
+  __syncthreads();
+  const int per = (n + gridDim.x - 1) / gridDim.x;
+  const int lo = blockIdx.x * per, hi = min(n, lo + per);
+  for (int i = lo + warp; i < hi; i += n_warps) {
+    const uint64_t ki = keys[i];
+    int c = 0;
+    for (int j = lane; j < n; j += 32) c += keys[j] < ki;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
+    if (lane == 0) order[c] = i;
+  }
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);
+  __syncthreads();
+  if (s_ticket != gridDim.x - 1) return;
+  if (tid == 0) *ticket = 0;
+  __threadfence();
+
+  int prog[IPT];
+  long long incl[IPT];
+  long long tsum = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    const int r = tid * IPT + i;
+    prog[i] = r < n ? __ldcg(order + r) : -1;
+    const int s = r < n ? kv_pages[prog[i]] : 0;
+    incl[i] = s > 0 ? s : 0;
+    tsum += incl[i];
+  }
+  uint64_t tot;
+  long long run = (long long)block_excl_scan((uint64_t)tsum, warp_tot, &tot);
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) { run += incl[i]; incl[i] = run; }   // inclusive sums in rank order
+
+  int my_tier[IPT];
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) my_tier[i] = caps.n_tiers;           // Waiting unless a tier takes it
+  int b_prev = 0;
+  long long base = 0;
+  for (int t = 0; t < caps.n_tiers; ++t) {
+    int c = 0;
+#pragma unroll
+    for (int i = 0; i < IPT; ++i) {
+      const int r = tid * IPT + i;
+      c += (r < n) && (r >= b_prev) && (incl[i] - base <= caps.cap[t]);
+    }
+    block_excl_scan((uint64_t)c, warp_tot, &tot);
+    const int b = b_prev + (int)tot;
+    if (tid == 0) bcast[0] = base;
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < IPT; ++i) {
+      const int r = tid * IPT + i;
+      if (r >= b_prev && r < b) my_tier[i] = t;
+      if (r == b - 1 && b > b_prev) bcast[0] = incl[i];
+    }
+    __syncthreads();
+    const long long top = bcast[0];
+    if (tid == 0) { bounds[t] = b; used[t] = top - base; }
+    base = top;
+    b_prev = b;
+    __syncthreads();                                                 // bcast is rewritten next round
+  }
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) if (prog[i] >= 0) tier[prog[i]] = (uint8_t)my_tier[i];
+}
+
 }  // namespace mori

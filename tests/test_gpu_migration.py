@@ -212,3 +212,32 @@ def test_many_calls_without_a_join_wrap_the_index_ring(mori, path):
     m.mori_sync(mori.BOTH)
     assert np.array_equal(pool.cpu().numpy(), pool_m)
     m.close()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_device_resident_arena_is_a_third_tier(mori, kernel):
+    """The arena may be device memory (a peer GPU's HBM over NVLink in production; a second
+    buffer of the same GPU here): demote / promote byte-exact against the oracle, one kernel each."""
+    L, H, D, T, P, S = 4, 8, 128, 16, 300, 260
+    chunk = 2 * H * T * D * 2
+    g0 = torch.Generator(device="cpu").manual_seed(5)
+    pool_h = torch.randint(0, 256, (L * P * chunk,), dtype=torch.uint8, generator=g0)
+    arena_h = torch.randint(0, 256, (S * L * chunk,), dtype=torch.uint8, generator=g0)
+    pool, arena = pool_h.cuda(), arena_h.cuda()
+    m = mori.Mori(L, H, D, T, pool, arena, copy_kernel=kernel)
+    assert m.path_demote == mori.PATH_ZEROCOPY and m.path_promote == mori.PATH_ZEROCOPY
+    pool_m, arena_m = pool_h.numpy().copy(), arena_h.numpy().copy()
+    rng = np.random.default_rng(2)
+    g = rng.permutation(P)[:200].astype(np.int32); h = rng.permutation(S)[:200].astype(np.int32)
+    l0 = m.mori_launch_count()
+    t = m.mori_demote(g, h)
+    m.mori_sync(mori.BOTH)
+    assert m.mori_launch_count() - l0 == 2                    # index upload + one copy kernel
+    oracle.demote(L, chunk, pool_m, arena_m, g, h)
+    assert np.array_equal(arena.cpu().numpy(), arena_m) and np.array_equal(pool.cpu().numpy(), pool_m)
+    g2 = rng.permutation(P)[:200].astype(np.int32)
+    m.mori_promote(h, g2, wait_demote_ticket=t)
+    m.mori_sync(mori.BOTH)
+    oracle.promote(L, chunk, pool_m, arena_m, h, g2)
+    assert np.array_equal(pool.cpu().numpy(), pool_m) and np.array_equal(arena.cpu().numpy(), arena_m)
+    m.close()
