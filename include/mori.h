@@ -66,7 +66,7 @@ enum { MORI_PATH_AUTO = 0, MORI_PATH_ZEROCOPY = 1, MORI_PATH_STAGED = 2, MORI_PA
 /* Device copy kernel used by STAGED paths and by mori_gather_pages / mori_scatter_pages. */
 enum { MORI_KERNEL_AUTO = 0, MORI_KERNEL_LDST = 1, MORI_KERNEL_TMA = 2 };
 
-#define MORI_MAX_PROGRAMS 8192 /* rank_partition sorts in one CTA's shared memory */
+#define MORI_MAX_PROGRAMS 8192 /* the keys of all programs fit one CTA's shared memory */
 
 typedef struct {
   int32_t n_layers, n_kv_heads, head_dim, page_tokens, elem_bytes; /* bf16 -> elem_bytes 2 */
@@ -132,6 +132,56 @@ int mori_rank_partition(mori_ctx* ctx, void* stream, int32_t n, const float* idl
                         const int32_t* kv_pages, const uint8_t* prev_tier, int64_t gpu_cap_pages,
                         int64_t cpu_cap_pages, int32_t* order, uint8_t* tier, int32_t* bounds,
                         int64_t* used_pages, int32_t* lists, int32_t* list_counts);
+
+/*
+ * Step a5, demotion (P:L177 "offloaded to CPU DRAM on the same node"; P:L202, L206): for every
+ * j in [0, total_pages) and every layer l, copy chunk (l, gpu_pages[j]) of the pool to
+ * (host_slots[j], l) of the arena.  Asynchronous, on the context's demote stream(s).
+ *
+ *   gpu_pages, host_slots  HOST int32[total_pages]; ids out of range -> MORI_ERR_INVALID_ARG.
+ *                          Duplicate destination slots are undefined behaviour.
+ *   wait_promote_ticket    0, or a ticket returned by mori_promote: no byte of this call is
+ *                          written before that promote call has completed (device-side wait).
+ *   ticket_out             NULL, or receives this call's ticket (> 0, increasing).
+ * total_pages == 0 is a valid no-op that still yields a ticket.
+ */
+int mori_demote(mori_ctx* ctx, int64_t total_pages, const int32_t* gpu_pages,
+                const int32_t* host_slots, int64_t wait_promote_ticket, int64_t* ticket_out);
+
+/*
+ * Step a6, promotion (P:L182 "CPU-to-GPU transfer over PCIe"; P:L184, L208): the mirror image,
+ * arena (host_slots[j], l) -> pool (l, gpu_pages[j]), on the promote stream(s), concurrently
+ * with demotions.  wait_demote_ticket orders the pool writes after the demotion that vacated
+ * the destination pages (the host->device DMA of a STAGED promote may start earlier).
+ */
+int mori_promote(mori_ctx* ctx, int64_t total_pages, const int32_t* host_slots,
+                 const int32_t* gpu_pages, int64_t wait_demote_ticket, int64_t* ticket_out);
+
+/* Step a7: block the host until every demote (1), promote (2) or both (3) call has finished;
+ * returns the first asynchronous error if there was one. */
+int mori_sync(mori_ctx* ctx, int32_t which);
+
+/* Device-side ordering against a caller stream (cudaStream_t), no host blocking:
+ *   mori_after_stream   work enqueued later in direction(s) `which` starts after everything
+ *                       now in `stream` (e.g. the inference step that last touched the pages);
+ *   mori_stream_wait    work enqueued later in `stream` starts after everything now enqueued
+ *                       in direction(s) `which`. */
+int mori_after_stream(mori_ctx* ctx, int32_t which, void* stream);
+int mori_stream_wait(mori_ctx* ctx, void* stream, int32_t which);
+
+/*
+ * The on-device halves of the STAGED paths, exposed because they are what the HBM roofline is
+ * measured on: pool pages <-> a contiguous DEVICE buffer laid out [n_pages][n_layers][chunk].
+ * gpu_pages is a DEVICE int32[n_pages].  One launch on `stream`; asynchronous.
+ */
+int mori_gather_pages(mori_ctx* ctx, void* stream, int64_t n_pages, const int32_t* gpu_pages,
+                      void* dst);
+int mori_scatter_pages(mori_ctx* ctx, void* stream, int64_t n_pages, const int32_t* gpu_pages,
+                       const void* src);
+
+/* ------------------------------------------------------------------------------------------------
+ * Beyond the hot path: the steps around it, each with its own oracle.
+ * ---------------------------------------------------------------------------------------------- */
 
 /*
  * NEXT-1: the paper's sticky, status-aware tier management, section 4.3.1, as an
@@ -244,52 +294,6 @@ int mori_bfd_assign(mori_ctx* ctx, void* stream, int32_t m, const int32_t* size,
 int mori_rank_partition_tiers(mori_ctx* ctx, void* stream, int32_t n, const float* idleness,
                               const int32_t* kv_pages, int32_t n_tiers, const int64_t* cap_pages,
                               int32_t* order, uint8_t* tier, int32_t* bounds, int64_t* used_pages);
-
-/*
- * Step a5, demotion (P:L177 "offloaded to CPU DRAM on the same node"; P:L202, L206): for every
- * j in [0, total_pages) and every layer l, copy chunk (l, gpu_pages[j]) of the pool to
- * (host_slots[j], l) of the arena.  Asynchronous, on the context's demote stream(s).
- *
- *   gpu_pages, host_slots  HOST int32[total_pages]; ids out of range -> MORI_ERR_INVALID_ARG.
- *                          Duplicate destination slots are undefined behaviour.
- *   wait_promote_ticket    0, or a ticket returned by mori_promote: no byte of this call is
- *                          written before that promote call has completed (device-side wait).
- *   ticket_out             NULL, or receives this call's ticket (> 0, increasing).
- * total_pages == 0 is a valid no-op that still yields a ticket.
- */
-int mori_demote(mori_ctx* ctx, int64_t total_pages, const int32_t* gpu_pages,
-                const int32_t* host_slots, int64_t wait_promote_ticket, int64_t* ticket_out);
-
-/*
- * Step a6, promotion (P:L182 "CPU-to-GPU transfer over PCIe"; P:L184, L208): the mirror image,
- * arena (host_slots[j], l) -> pool (l, gpu_pages[j]), on the promote stream(s), concurrently
- * with demotions.  wait_demote_ticket orders the pool writes after the demotion that vacated
- * the destination pages (the host->device DMA of a STAGED promote may start earlier).
- */
-int mori_promote(mori_ctx* ctx, int64_t total_pages, const int32_t* host_slots,
-                 const int32_t* gpu_pages, int64_t wait_demote_ticket, int64_t* ticket_out);
-
-/* Step a7: block the host until every demote (1), promote (2) or both (3) call has finished;
- * returns the first asynchronous error if there was one. */
-int mori_sync(mori_ctx* ctx, int32_t which);
-
-/* Device-side ordering against a caller stream (cudaStream_t), no host blocking:
- *   mori_after_stream   work enqueued later in direction(s) `which` starts after everything
- *                       now in `stream` (e.g. the inference step that last touched the pages);
- *   mori_stream_wait    work enqueued later in `stream` starts after everything now enqueued
- *                       in direction(s) `which`. */
-int mori_after_stream(mori_ctx* ctx, int32_t which, void* stream);
-int mori_stream_wait(mori_ctx* ctx, void* stream, int32_t which);
-
-/*
- * The on-device halves of the STAGED paths, exposed because they are what the HBM roofline is
- * measured on: pool pages <-> a contiguous DEVICE buffer laid out [n_pages][n_layers][chunk].
- * gpu_pages is a DEVICE int32[n_pages].  One launch on `stream`; asynchronous.
- */
-int mori_gather_pages(mori_ctx* ctx, void* stream, int64_t n_pages, const int32_t* gpu_pages,
-                      void* dst);
-int mori_scatter_pages(mori_ctx* ctx, void* stream, int64_t n_pages, const int32_t* gpu_pages,
-                       const void* src);
 
 /* Kernel timing for the roofline: while enabled, every gather/scatter kernel launched by
  * mori_demote / mori_promote is bracketed by CUDA events on its stream.  mori_profile_read
