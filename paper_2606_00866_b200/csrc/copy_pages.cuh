@@ -10,9 +10,8 @@
 //
 // Pure data movement: the bound is HBM (device staging) or the host link (mapped arena), so the
 // design goal is bytes in flight, not arithmetic.  Work is cut into "pieces": a contiguous run
-// of <= kPieceBytes inside one chunk, contiguous on BOTH sides.  Piece w maps to
-// (k, l, c) = (w / (L*ppc), (w / ppc) % L, w % ppc) so consecutive CTAs stream through
-// consecutive addresses of one chunk (DRAM page locality on both sides).
+// of <= piece_bytes inside one chunk, contiguous on BOTH sides (the bulk-copy kernel uses whole
+// 64 KiB chunks as pieces; the LD/ST kernel 16 KiB).
 //
 // Two implementations:
 //   copy_pages_tma   two threads per CTA drive the SM's bulk-copy engine: a loader issues
@@ -20,8 +19,10 @@
 //                    a storer issues cp.async.bulk shared->global (bulk_group) and hands stages
 //                    back.  No registers, no LSU instructions per byte; up to 192 KiB of the
 //                    ring in flight per SM.
+//                    CTA b takes chunks b, b + grid, ...: one page-table load per chunk.
 //   copy_pages_ldst  256 threads, 4 x 16-byte ld.global.nc.L1::no_allocate per thread issued
-//                    before the 4 st.global: 16 KiB in flight per CTA, 8 CTAs per SM.
+//                    before the 4 st.global: 16 KiB in flight per CTA, 8 CTAs per SM; piece w
+//                    maps to (k, l, c) = (w / (L*ppc), (w / ppc) % L, w % ppc).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -39,6 +40,8 @@ struct CopyArgs {
   int chunk_bytes;            // multiple of 16
   int piece_bytes;            // multiple of 16, <= chunk_bytes
   int pieces_per_chunk;       // ceil(chunk / piece)
+  int stages;                 // bulk-copy kernel: ring depth (2 .. 24)
+  int store_lag;              // bulk-copy kernel: 1 or 2 (< stages)
 };
 
 template <bool kGather>
@@ -145,7 +148,6 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 }
 
 constexpr int kTmaThreads = 64;   // warp 0 lane 0 = load issuer, warp 1 lane 0 = store issuer
-constexpr int kTmaStoreLag = 2;   // stores allowed to be still reading shared memory
 
 // Addresses of chunk w = (page k, layer l): one page-table load and one division per CHUNK;
 // the pieces of a chunk are consecutive on both sides.
@@ -166,20 +168,22 @@ __device__ __forceinline__ void chunk_addresses(const CopyArgs& a, long long w, 
   if (kGather) { src = pp; dst = lp; } else { src = lp; dst = pp; }
 }
 
-// Shared memory: kStages stage buffers of a.piece_bytes each, then kStages "full" and kStages
+// Shared memory: a.stages stage buffers of a.piece_bytes each, then a.stages "full" and a.stages
 // "empty" mbarriers.  Two single-thread roles so that neither waits for the other's latency:
 //   loader  (warp 0): for every piece, wait until its stage is empty, expect_tx + bulk load;
 //   storer  (warp 1): wait until the stage is full, bulk store, commit; once the store issued
-//                     kTmaStoreLag groups ago has finished READING shared memory, hand its
-//                     stage back to the loader.
+//                     `lag` groups ago has finished READING shared memory, hand its stage back
+//                     to the loader (lag = 2 on a deep ring, 1 on a ring of a few large stages).
 // CTA b takes chunks b, b + grid, ...; every CTA walks the same piece sequence in both roles.
-template <bool kGather, int kStages>
+// Stage index and mbarrier phase are carried incrementally (no division per piece).
+template <bool kGather>
 __global__ void __launch_bounds__(kTmaThreads, 1) copy_pages_tma(const CopyArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * a.piece_bytes);
-  uint64_t* empty = full + kStages;
+  const int stages = a.stages;
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)stages * a.piece_bytes);
+  uint64_t* empty = full + stages;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -189,35 +193,38 @@ __global__ void __launch_bounds__(kTmaThreads, 1) copy_pages_tma(const CopyArgs 
 
   if (threadIdx.x == 0) {
     // ---------------- loader ----------------
-    long long i = 0;
+    int st = 0; uint32_t phase = 0; bool wrapped = false;          // phase of the NEXT wait on empty[st]
     for (long long w = blockIdx.x; w < n_chunks; w += gridDim.x) {
       const unsigned char* src; unsigned char* dst;
       chunk_addresses<kGather>(a, w, src, dst);
-      for (int c = 0; c < ppc; ++c, ++i) {
+      for (int c = 0; c < ppc; ++c) {
         const int off = c * a.piece_bytes;
         const uint32_t bytes = (uint32_t)min(a.piece_bytes, a.chunk_bytes - off);
-        const int st = (int)(i % kStages);
-        if (i >= kStages) mbar_wait(&empty[st], (uint32_t)(((i / kStages) - 1) & 1));
+        if (wrapped) mbar_wait(&empty[st], phase);
         mbar_expect_tx(&full[st], bytes);
         bulk_g2s(smem + (size_t)st * a.piece_bytes, src + off, bytes, &full[st]);
+        if (++st == stages) { st = 0; if (wrapped) phase ^= 1; wrapped = true; }
       }
     }
   } else {
     // ---------------- storer ----------------
-    long long i = 0;
+    const int lag = a.store_lag;
+    int st = 0; uint32_t phase = 0;                                 // stage / phase of the piece being stored
+    int rel = 0; long long issued = 0;                              // next stage to hand back
     for (long long w = blockIdx.x; w < n_chunks; w += gridDim.x) {
       const unsigned char* src; unsigned char* dst;
       chunk_addresses<kGather>(a, w, src, dst);
-      for (int c = 0; c < ppc; ++c, ++i) {
+      for (int c = 0; c < ppc; ++c) {
         const int off = c * a.piece_bytes;
         const uint32_t bytes = (uint32_t)min(a.piece_bytes, a.chunk_bytes - off);
-        const int st = (int)(i % kStages);
-        mbar_wait(&full[st], (uint32_t)((i / kStages) & 1));
+        mbar_wait(&full[st], phase);
         bulk_s2g(dst + off, smem + (size_t)st * a.piece_bytes, bytes);
         bulk_commit();
-        if (i >= kTmaStoreLag) {
-          bulk_wait_read<kTmaStoreLag>();                       // group i - lag has left shared memory
-          mbar_arrive(&empty[(int)((i - kTmaStoreLag) % kStages)]);
+        if (++st == stages) { st = 0; phase ^= 1; }
+        if (++issued > lag) {                                       // the group issued `lag` ago has left smem
+          if (lag == 1) bulk_wait_read<1>(); else bulk_wait_read<2>();
+          mbar_arrive(&empty[rel]);
+          if (++rel == stages) rel = 0;
         }
       }
     }

@@ -32,14 +32,15 @@ std::map<void*, std::pair<void*, size_t>> g_host_allocs;   // mori_host_alloc: a
 
 constexpr int kTicketRing = 4096;
 constexpr int kRankTickets = 64;      // rank/partition launches that may be in flight at once
-#ifndef MORI_TMA_STAGES
-#define MORI_TMA_STAGES 12
-#endif
 #ifndef MORI_PIECE_BYTES
-#define MORI_PIECE_BYTES (16 * 1024)
+#define MORI_PIECE_BYTES (64 * 1024)
 #endif
-constexpr int kTmaStages = MORI_TMA_STAGES;     // ring depth of the bulk-copy kernel
-constexpr int kPieceBytes = MORI_PIECE_BYTES;   // bytes per bulk copy (stage size)
+#ifndef MORI_RING_BYTES
+#define MORI_RING_BYTES (192 * 1024)
+#endif
+constexpr int kPieceBytes = MORI_PIECE_BYTES;   // bytes per bulk copy = stage size (whole 64 KiB chunks)
+constexpr int kRingBytes = MORI_RING_BYTES;     // shared memory the ring of stages may take per CTA
+constexpr int kMaxTmaStages = 24;
 constexpr long long kAutoMinRunBytes = 6LL << 20;   // AUTO: below this mean slot-run length, ZEROCOPY
 
 struct ProfSpan { cudaEvent_t a, b; long long bytes; };
@@ -67,7 +68,7 @@ struct mori_ctx {
   int device = 0, sm_count = 148;
   long long chunk = 0, page_bytes = 0, staging_bytes = 0, max_pages = 0;
   int copy_kernel = MORI_KERNEL_TMA;
-  int piece = kPieceBytes, ppc = 1;
+  int piece = kPieceBytes, ppc = 1, tma_stages = 3, tma_lag = 1;
   int link_ctas = 32;
   size_t tma_smem = 0;
   unsigned char* arena_dev = nullptr;            // device-side alias of the pinned arena
@@ -125,6 +126,8 @@ mori::CopyArgs make_args(const mori_ctx* c, unsigned char* lin, const int32_t* g
   a.chunk_bytes = (int)c->chunk;
   a.piece_bytes = c->piece;
   a.pieces_per_chunk = c->ppc;
+  a.stages = c->tma_stages;
+  a.store_lag = c->tma_lag;
   return a;
 }
 
@@ -138,11 +141,15 @@ cudaError_t launch_copy(const mori_ctx* c, const mori::CopyArgs& a, cudaStream_t
   if (c->copy_kernel == MORI_KERNEL_TMA) {
     const long long max_grid = link ? c->link_ctas : c->sm_count;  // 1 CTA per SM (smem-bound)
     const int grid = (int)std::min<long long>(a.n_pages * a.n_layers, max_grid);   // CTAs stride chunks
-    mori::copy_pages_tma<kGather, kTmaStages><<<grid, mori::kTmaThreads, c->tma_smem, s>>>(a);
+    mori::copy_pages_tma<kGather><<<grid, mori::kTmaThreads, c->tma_smem, s>>>(a);
   } else {
+    mori::CopyArgs b = a;                                        // LD/ST works in 16 KiB pieces
+    b.piece_bytes = (int)std::min<long long>(16 * 1024, a.chunk_bytes);
+    b.pieces_per_chunk = (a.chunk_bytes + b.piece_bytes - 1) / b.piece_bytes;
+    const long long n_ldst = a.n_pages * a.n_layers * b.pieces_per_chunk;
     const long long max_grid = link ? 2 * c->link_ctas : (long long)c->sm_count * 8;
-    const int grid = (int)std::min<long long>(n_pieces, max_grid);
-    mori::copy_pages_ldst<kGather><<<grid, mori::kLdstThreads, 0, s>>>(a);
+    const int grid = (int)std::min<long long>(n_ldst, max_grid);
+    mori::copy_pages_ldst<kGather><<<grid, mori::kLdstThreads, 0, s>>>(b);
   }
   return cudaGetLastError();
 }
@@ -328,7 +335,9 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   c->piece = (int)std::min<long long>(kPieceBytes, chunk);
   c->ppc = (int)((chunk + c->piece - 1) / c->piece);
   c->copy_kernel = cfg->copy_kernel == MORI_KERNEL_AUTO ? MORI_KERNEL_TMA : cfg->copy_kernel;
-  c->tma_smem = (size_t)kTmaStages * c->piece + 2 * kTmaStages * sizeof(uint64_t);
+  c->tma_stages = std::max(2, std::min(kMaxTmaStages, kRingBytes / c->piece));
+  c->tma_lag = c->tma_stages >= 6 ? 2 : 1;
+  c->tma_smem = (size_t)c->tma_stages * c->piece + 2 * c->tma_stages * sizeof(uint64_t);
   c->max_pages = cfg->max_pages_per_call ? cfg->max_pages_per_call
                                           : std::max<long long>(cfg->gpu_pool_pages, cfg->host_arena_slots);
   c->staging_bytes = cfg->staging_bytes ? cfg->staging_bytes : (1024LL << 20);
@@ -351,8 +360,8 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
     }                                                                                         \
   } while (0)
 
-  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<true, kTmaStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
-  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<false, kTmaStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
+  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
+  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
   CKC(cudaMalloc((void**)&c->rank_tickets, sizeof(unsigned int) * kRankTickets));
   CKC(cudaMemset(c->rank_tickets, 0, sizeof(unsigned int) * kRankTickets));
   c->idl_k = cfg->idleness_window ? cfg->idleness_window : 5;
