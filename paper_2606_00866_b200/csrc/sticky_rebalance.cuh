@@ -16,9 +16,8 @@
 // memory, one warp per program); the last CTA to finish (atomic ticket) cuts the victim prefix
 // ("usage minus what the earlier victims free still exceeds the capacity" is monotone) and the
 // candidate prefix ("inclusive size sum fits the free capacity" is monotone) with block scans.
-// The only sequential step is the paper's per-victim "CPU if it fits, else Waiting": one warp
-// walks the victims' sizes in shared memory 32 at a time (a ballot per admission, one per chunk
-// in which nothing fits), and the walk is skipped when all of them fit.
+// The only sequential step is the paper's per-victim "CPU if it fits, else Waiting", walked by
+// one thread over the victims' sizes in shared memory, and skipped when all of them fit.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -147,25 +146,14 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
 #pragma unroll
     for (int i = 0; i < IPT; ++i) if (victim[i]) vdest[tid * IPT + i] = 1;
     if (tid == 0) bcast[0] = usage_cpu0 + freed;
-  } else if (warp == 0) {
-    // One warp, 32 victims at a time: a ballot finds the first victim that still fits the room
-    // left, it is admitted, and the victims after it are re-tested against the smaller room; a
-    // chunk in which nothing fits costs one ballot.  Same decisions as the one-at-a-time walk.
-    long long room = cap_cpu - usage_cpu0;
-    for (int k0 = 0; k0 < v; k0 += 32) {
-      const int k = k0 + lane;
-      const long long s = k < v ? (long long)vsize[k] : 0;
-      int dest = 2;
-      unsigned cand = __ballot_sync(0xFFFFFFFFu, k < v && s <= room);
-      while (cand) {
-        const int f = __ffs(cand) - 1;
-        room -= __shfl_sync(0xFFFFFFFFu, s, f);
-        if (lane == f) dest = 1;
-        cand = __ballot_sync(0xFFFFFFFFu, k < v && lane > f && s <= room);
-      }
-      if (k < v) vdest[k] = (uint8_t)dest;
+  } else if (tid == 0) {
+    long long cpu = usage_cpu0;
+    for (int k = 0; k < v; ++k) {
+      const bool fits = cpu + vsize[k] <= cap_cpu;
+      vdest[k] = fits ? 1 : 2;
+      if (fits) cpu += vsize[k];
     }
-    if (lane == 0) bcast[0] = cap_cpu - room;
+    bcast[0] = cpu;
   }
   __syncthreads();
   const long long usage_cpu1 = bcast[0];
