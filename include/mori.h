@@ -144,6 +144,8 @@ int mori_rank_partition(mori_ctx* ctx, void* stream, int32_t n, const float* idl
  *                          written before that promote call has completed (device-side wait).
  *   ticket_out             NULL, or receives this call's ticket (> 0, increasing).
  * total_pages == 0 is a valid no-op that still yields a ticket.
+ * Calls of one direction take effect in issue order (a later call that writes the same slots or
+ * pages wins), whichever path each of them takes; the two directions are ordered only by tickets.
  */
 int mori_demote(mori_ctx* ctx, int64_t total_pages, const int32_t* gpu_pages,
                 const int32_t* host_slots, int64_t wait_promote_ticket, int64_t* ticket_out);

@@ -717,6 +717,12 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
 
   if (path == MORI_PATH_ZEROCOPY) {
     if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc;
+    // Calls of one direction take effect in issue order.  An earlier STAGED demote of this
+    // direction may still have DMAs in flight on the copy stream: this kernel must not overtake
+    // them (same-stream order covers every other combination of paths).
+    if (demote)
+      for (int b = 0; b < 2; ++b)
+        if (d.copy_done[b]) CK(c, cudaStreamWaitEvent(d.kern, d.copy_done[b], 0));
     if (total > 0) {
       const int32_t *dg, *dh;
       if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;

@@ -241,3 +241,23 @@ def test_device_resident_arena_is_a_third_tier(mori, kernel):
     oracle.promote(L, chunk, pool_m, arena_m, h, g2)
     assert np.array_equal(pool.cpu().numpy(), pool_m) and np.array_equal(arena.cpu().numpy(), arena_m)
     m.close()
+
+
+def test_auto_keeps_issue_order_when_consecutive_calls_take_different_paths(mori):
+    """AUTO picks STAGED for a long run of slots and ZEROCOPY for scattered ones; two demotes in a
+    row that write the same slots must still land in issue order (the second one wins)."""
+    L, H, D, T, P, S = 4, 8, 128, 16, 2048, 2048               # 256 KiB pages
+    m, pool, arena, pool_m, arena_m, chunk = _mk_ctx(mori, L, H, D, T, P, S, 0, 2)
+    rng = np.random.default_rng(4)
+    for rep in range(3):
+        g_a = rng.permutation(P)[:1500].astype(np.int32)
+        h_a = np.arange(1500, dtype=np.int32)                  # one run of 375 MiB -> STAGED (a long DMA)
+        g_b = rng.permutation(P)[:300].astype(np.int32)
+        h_b = (rng.permutation(750)[:300] * 2).astype(np.int32)   # isolated slots inside that run -> ZEROCOPY
+        m.mori_demote(g_a, h_a)
+        m.mori_demote(g_b, h_b)
+        m.mori_sync(mori.BOTH)
+        oracle.demote(L, chunk, pool_m, arena_m, g_a, h_a)
+        oracle.demote(L, chunk, pool_m, arena_m, g_b, h_b)
+        assert np.array_equal(arena.numpy(), arena_m), rep
+    m.close()
