@@ -302,6 +302,8 @@ def run_ours(args):
     def ev():
         return torch.cuda.Event(enable_timing=True)
 
+    sticky = args.policy == "sticky"
+
     def epoch(mode):
         """One step.  mode 'dev': inputs resident, regions A+B timed; 'e2e': host buffers, one
         region.  -> dict(ms, dem, pro, h2d, d2h)."""
@@ -312,7 +314,10 @@ def run_ours(args):
             torch.cuda.synchronize()
             a0, a1, b0, b1 = ev(), ev(), ev(), ev()
             a0.record(cur)
-            got = r.place_resident(cur)                            # kernel + D2H of lists + sync
+            if sticky:                                             # NEXT-1 policy: status flags ride along
+                got = r.place_sticky(plan.iota, plan.kv_pages, plan.prev_tier, plan.flags, stream=cur)
+            else:
+                got = r.place_resident(cur)                        # kernel + D2H of lists + sync
             a1.record(cur)
             sim.apply_placement(got["tier"], got["lists"])         # harness allocator (untimed)
             b0.record(cur)
@@ -328,7 +333,8 @@ def run_ours(args):
             e0, e1 = ev(), ev()
             e0.record(cur)
             r.mori.mori_after_stream(binding.BOTH, cur)
-            got = r.place(plan.iota, plan.kv_pages, plan.prev_tier, stream=cur)
+            got = (r.place_sticky(plan.iota, plan.kv_pages, plan.prev_tier, plan.flags, stream=cur) if sticky
+                   else r.place(plan.iota, plan.kv_pages, plan.prev_tier, stream=cur))
             sim.apply_placement(got["tier"], got["lists"])
             r.execute(plan, sync=False)
             r.mori.mori_stream_wait(cur, binding.BOTH)
@@ -485,7 +491,7 @@ def run_ours(args):
                        "path_demote": binding.PATH_NAMES[r.mori_paths[0]],
                        "path_promote": binding.PATH_NAMES[r.mori_paths[1]],
                        "copy_kernel": kernel_name,
-                       "staging_MiB": args.staging_mib,
+                       "staging_MiB": args.staging_mib, "policy": args.policy,
                        "l2": "inputs larger than L2 (GiB per step vs 126 MB); no flush needed",
                        "migrated_GiB": b_dev / GIB, "setup_s": t_setup,
                        "host_arena_on_huge_pages_GiB": arena_thp_gib},
@@ -737,6 +743,9 @@ def main():
     ap.add_argument("--path-promote", default="auto", choices=["auto", "zerocopy", "staged", "copyengine"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "ldst", "tma"])
     ap.add_argument("--staging-mib", type=int, default=0, help="0 = library default")
+    ap.add_argument("--policy", default="partition", choices=["partition", "sticky"],
+                    help="partition: re-partition every epoch (the hot path, default); sticky: the paper's "
+                         "section-4.3.1 tier management (mori_sticky_rebalance)")
     ap.add_argument("--verbose", action="store_true", help="per-step lines on stderr")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gather-leg", action="store_true")
