@@ -44,11 +44,22 @@ __device__ __forceinline__ int evict_digit(const EvictArgs& a, int page, int pas
   return a.which_tier == 0 ? (t == 1 ? 1 : 2) : (t == 0 ? 1 : 2);    // GPU: idle, busy / CPU: busy, idle
 }
 
+// Passes 1..3 sort on a byte of last_access that is zero for every resident page when the
+// counters are small (ticks): such a pass cannot change the order of the resident pages -- it would
+// only move free pages behind them, which the final type-rank pass does anyway -- so its three
+// kernels return at once.  max_last is the largest resident last_access, found by pass 0.
+__device__ __forceinline__ bool evict_pass_is_noop(int pass, const unsigned int* max_last) {
+  return pass >= 1 && pass <= 3 && (*max_last >> (8 * pass)) == 0;
+}
+
 __global__ void __launch_bounds__(kEvictTile)
 evict_hist_kernel(EvictArgs a, int pass, const int32_t* __restrict__ perm_in, int32_t* __restrict__ table,
-                  int32_t* __restrict__ n_resident) {
+                  int32_t* __restrict__ n_resident, unsigned int* __restrict__ max_last) {
+  if (evict_pass_is_noop(pass, max_last)) return;
   __shared__ int hist[256];
   __shared__ int resident;
+  __shared__ unsigned int tile_max;
+  if (threadIdx.x == 0) tile_max = 0;
   if (threadIdx.x < 256) hist[threadIdx.x] = 0;
   if (threadIdx.x == 0) resident = 0;
   __syncthreads();
@@ -58,17 +69,18 @@ evict_hist_kernel(EvictArgs a, int pass, const int32_t* __restrict__ perm_in, in
     atomicAdd(&hist[evict_digit(a, page, pass)], 1);
     if (pass == 0) {
       const int o = a.page_owner[page];
-      if (o >= 0 && o < a.n_programs) atomicAdd(&resident, 1);
+      if (o >= 0 && o < a.n_programs) { atomicAdd(&resident, 1); atomicMax(&tile_max, a.last_access[page]); }
     }
   }
   __syncthreads();
   if (threadIdx.x < 256) table[threadIdx.x * a.tiles + blockIdx.x] = hist[threadIdx.x];
-  if (pass == 0 && threadIdx.x == 0 && resident) atomicAdd(n_resident, resident);
+  if (pass == 0 && threadIdx.x == 0 && resident) { atomicAdd(n_resident, resident); atomicMax(max_last, tile_max); }
 }
 
 // exclusive scan of table[256 * tiles] in place (digit-major), one CTA of 1024 threads
 __global__ void __launch_bounds__(kRankMaxThreads)
-evict_scan_kernel(int32_t* __restrict__ table, int entries) {
+evict_scan_kernel(int32_t* __restrict__ table, int entries, int pass, const unsigned int* __restrict__ max_last) {
+  if (evict_pass_is_noop(pass, max_last)) return;
   __shared__ uint64_t warp_tot[33];
   const int per = (entries + blockDim.x - 1) / blockDim.x;
   const int lo = threadIdx.x * per, hi = min(entries, lo + per);
@@ -81,7 +93,13 @@ evict_scan_kernel(int32_t* __restrict__ table, int entries) {
 
 __global__ void __launch_bounds__(kEvictTile)
 evict_scatter_kernel(EvictArgs a, int pass, const int32_t* __restrict__ perm_in,
-                     const int32_t* __restrict__ table, int32_t* __restrict__ perm_out) {
+                     const int32_t* __restrict__ table, int32_t* __restrict__ perm_out,
+                     const unsigned int* __restrict__ max_last) {
+  if (evict_pass_is_noop(pass, max_last)) {                          // identity pass: just hand the order on
+    const long long j = (long long)blockIdx.x * kEvictTile + threadIdx.x;
+    if (j < a.n_pages) perm_out[j] = perm_in[j];
+    return;
+  }
   __shared__ int wcnt[32][257];                                      // [warp][digit]; 257: no bank clash
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int e = threadIdx.x; e < 32 * 257; e += kEvictTile) (&wcnt[0][0])[e] = 0;

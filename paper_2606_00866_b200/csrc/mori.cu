@@ -80,6 +80,7 @@ struct mori_ctx {
   // the 16-node sequence of mori_eviction_order, captured once per argument set and replayed
   cudaGraphExec_t evict_exec = nullptr; cudaStream_t evict_cap_stream = nullptr;
   struct { int tier, n_programs; long long n_pages; const void *owner, *ptier, *last; void *victims, *nres; } evict_key{};
+  unsigned int* evict_max_last = nullptr;
   int32_t* evict_perm[2] = {nullptr, nullptr}; int32_t* evict_table = nullptr; long long evict_cap = 0;   // scratch, grown on demand
   int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
   Direction dir[2];                              // 0 demote, 1 promote
@@ -369,6 +370,7 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   CKC(cudaMalloc((void**)&c->idl_a, sizeof(double) * (size_t)cfg->max_programs * c->idl_k));
   CKC(cudaMalloc((void**)&c->idl_pushed, sizeof(int32_t) * (size_t)cfg->max_programs));
   CKC(cudaMemset(c->idl_pushed, 0, sizeof(int32_t) * (size_t)cfg->max_programs));
+  CKC(cudaMalloc((void**)&c->evict_max_last, sizeof(unsigned int)));
   CKC(cudaMalloc((void**)&c->sticky_order, sizeof(int32_t) * kRankTickets * (size_t)cfg->max_programs));
   if (cfg->host_arena) {
     // The arena may also be DEVICE memory -- a second pool in this GPU's HBM, or a peer GPU's HBM
@@ -434,6 +436,7 @@ int mori_destroy(mori_ctx* c) {
   if (c->evict_cap_stream) cudaStreamDestroy(c->evict_cap_stream);
   for (int b = 0; b < 2; ++b) if (c->evict_perm[b]) cudaFree(c->evict_perm[b]);
   if (c->evict_table) cudaFree(c->evict_table);
+  if (c->evict_max_last) cudaFree(c->evict_max_last);
   if (c->idl_r) cudaFree(c->idl_r);
   if (c->idl_a) cudaFree(c->idl_a);
   if (c->idl_pushed) cudaFree(c->idl_pushed);
@@ -603,12 +606,14 @@ int mori_eviction_order(mori_ctx* c, void* stream, int32_t which_tier, int64_t n
   auto enqueue = [&](cudaStream_t q) -> cudaError_t {
     cudaError_t e = cudaMemsetAsync(n_resident, 0, sizeof(int32_t), q);
     if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(c->evict_max_last, 0, sizeof(unsigned int), q);
+    if (e != cudaSuccess) return e;
     const int32_t* in = nullptr;                   // pass 0 reads the pages in id order
     for (int pass = 0; pass < mori::kEvictPasses; ++pass) {
       int32_t* out = pass == mori::kEvictPasses - 1 ? victims : c->evict_perm[pass & 1];
-      mori::evict_hist_kernel<<<tiles, mori::kEvictTile, 0, q>>>(a, pass, in, c->evict_table, n_resident);
-      mori::evict_scan_kernel<<<1, mori::kRankMaxThreads, 0, q>>>(c->evict_table, 256 * tiles);
-      mori::evict_scatter_kernel<<<tiles, mori::kEvictTile, 0, q>>>(a, pass, in, c->evict_table, out);
+      mori::evict_hist_kernel<<<tiles, mori::kEvictTile, 0, q>>>(a, pass, in, c->evict_table, n_resident, c->evict_max_last);
+      mori::evict_scan_kernel<<<1, mori::kRankMaxThreads, 0, q>>>(c->evict_table, 256 * tiles, pass, c->evict_max_last);
+      mori::evict_scatter_kernel<<<tiles, mori::kEvictTile, 0, q>>>(a, pass, in, c->evict_table, out, c->evict_max_last);
       in = out;
     }
     return cudaGetLastError();
