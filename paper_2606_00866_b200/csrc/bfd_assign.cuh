@@ -4,11 +4,13 @@
 //
 // Order: largest candidate first; equal sizes keep the promotion priority (returning before new,
 // least idle, index).  The order comes from ranking unique 128-bit keys by counting on every SM
-// (as in sticky_rebalance.cuh); the last CTA then walks the candidates in that order: one thread
-// keeps every replica's free pages in registers, picks the replica with the most (ties: lowest
-// index) and admits the candidate there if it fits.  The walk is the one inherently sequential
-// step of the rule (every admission changes the next arg-max); a warp-wide shuffle arg-max per
-// candidate measured 3x slower than this single thread (shuffle latency on the critical path).
+// (as in sticky_rebalance.cuh); the last CTA then walks the candidates in that order.  The walk is
+// the one inherently sequential step of the rule (every admission changes the next arg-max), so
+// what matters is the latency of one arg-max: with 32-bit capacities (the usual case) lane r of
+// one warp holds replica r, the maximum is one redux.sync and the winner the lowest set bit of a
+// ballot of "equals the maximum" (~100 cycles per admitted candidate); capacities beyond 2^31
+// take a single-thread walk with the replicas in registers.  A shuffle-butterfly arg-max on
+// 64-bit values measured 3x slower than either.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -97,7 +99,28 @@ bfd_assign_kernel(int m, const int32_t* __restrict__ size, const float* __restri
     ssize[k] = s > 0 ? s : 0;
   }
   __syncthreads();
-  if (tid == 0) {
+  bool small = true;                                                  // every capacity fits an int?
+  for (int r = 0; r < n_replicas; ++r) small = small && free_pages[r] <= 0x7FFFFFFFll;
+  if (small) {
+    // 32-bit capacities (the usual case): warp 0, lane r = replica r; the maximum comes from one
+    // redux.sync, the winner from a ballot of "equals the maximum" (lowest set bit).
+    if (warp == 0) {
+      int fr = lane < n_replicas ? (int)free_pages[lane] : -1;
+      int best = __reduce_max_sync(0xFFFFFFFFu, fr);
+      int who = __ffs(__ballot_sync(0xFFFFFFFFu, fr == best)) - 1;
+      for (int k = 0; k < m; ++k) {
+        const int s = ssize[k];                                       // broadcast read
+        const bool fits = s <= best;
+        if (lane == 0) sdest[k] = fits ? who : -1;
+        if (fits) {
+          if (lane == who) fr -= s;
+          best = __reduce_max_sync(0xFFFFFFFFu, fr);
+          who = __ffs(__ballot_sync(0xFFFFFFFFu, fr == best)) - 1;
+        }
+      }
+      if (lane < n_replicas) free_out[lane] = fr;
+    }
+  } else if (tid == 0) {
     if (n_replicas <= 8) bfd_walk<8>(m, ssize, sdest, n_replicas, free_pages, free_out);
     else if (n_replicas <= 16) bfd_walk<16>(m, ssize, sdest, n_replicas, free_pages, free_out);
     else bfd_walk<32>(m, ssize, sdest, n_replicas, free_pages, free_out);

@@ -59,3 +59,11 @@ def test_free_out_may_alias_free_pages_and_errors(ctx, mori):
         ctx.mori_bfd_assign(size, iota, flags, torch.zeros(33, dtype=torch.int64, device="cuda"), rep,
                             torch.zeros(33, dtype=torch.int64, device="cuda"))
     assert e.value.code == mori.ERR_UNSUPPORTED
+
+
+def test_capacities_beyond_int32_take_the_wide_walk(ctx):
+    rng = np.random.default_rng(3)
+    size, iota, flags, _ = rand_bfd_case(rng, 500, 4)
+    free = np.array([2 ** 40, 2 ** 33 + 5, 17, 2 ** 40], np.int64)
+    got, want = gpu_bfd(ctx, size, iota, flags, free), oracle.bfd_assign(size, iota, flags, free)
+    assert np.array_equal(got[0], want[0]) and np.array_equal(got[1], want[1])
