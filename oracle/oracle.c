@@ -24,6 +24,14 @@
  * Readings of the paper adopted where it is silent are listed in DESIGN.md section 3 (R1..R14);
  * the ones that matter here are repeated next to the code.
  *
+ * Further down, each with its own header comment and its own pins file under tests/:
+ *   oracle_sticky_rebalance      P:L206, L208 (section 4.3.1)       tests/test_oracle_sticky_pins.py
+ *   oracle_idleness_update/eval  Eq. (1), P:L190-196                tests/test_oracle_idleness_pins.py
+ *   oracle_eviction_order        P:L212-221 (section 4.3.2)         tests/test_oracle_eviction_pins.py
+ *   oracle_bfd_assign            P:L208-210                         tests/test_oracle_bfd_pins.py
+ *   oracle_rank_partition_tiers  P:L339-351 (section 7.1)           tests/test_oracle_tiers_pins.py
+ * Every function is pinned (none is "parity unpinned"); DESIGN.md sections 10 and 12-15 say by what.
+ *
  * Pins (tests/test_oracle_pins.py): brute force on n <= 9, numpy stable argsort / cumsum /
  * searchsorted restatement, closed forms (equal sizes, zero and infinite capacity), the
  * ordering / capacity / maximality invariants, list set identities, and for the movers the
