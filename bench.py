@@ -276,9 +276,14 @@ def run_ours(args):
 
     rank, world, local = replicas.env_rank()
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    if args.device_index >= 0:
+        local = args.device_index                    # testing only: several replicas on one GPU
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(args.backend)
 
     scale = args.scale or _pick_scale(args.config, world, W)
     cfg = W.get_config(args.config, scale)
@@ -760,6 +765,9 @@ def main():
     ap.add_argument("--policy", default="partition", choices=["partition", "sticky"],
                     help="partition: re-partition every epoch (the hot path, default); sticky: the paper's "
                          "section-4.3.1 tier management (mori_sticky_rebalance)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="process-group backend for N > 1 (gloo + --device-index: exercise the N > 1 path on one GPU)")
+    ap.add_argument("--device-index", type=int, default=-1, help="CUDA device to use instead of LOCAL_RANK")
     ap.add_argument("--verbose", action="store_true", help="per-step lines on stderr")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gather-leg", action="store_true")
