@@ -124,7 +124,7 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def measure_link_peak(arena, nbytes=GIB, reps=5):
+def measure_link_peak(arena, nbytes=GIB, reps=5, stream_chunks=1):
     """Pinned cudaMemcpyAsync of ONE contiguous buffer: D2H alone, H2D alone, both at once on
     two streams -- the host-link denominators (GB/s).  Uses the first bytes of the arena before
     the workload touches it, and a scratch device buffer."""
@@ -161,6 +161,26 @@ def measure_link_peak(arena, nbytes=GIB, reps=5):
            "d2h": nbytes / run(True, False) / 1e9,
            "h2d": nbytes / run(False, True) / 1e9,
            "bidir_sum": 2 * nbytes / run(True, True) / 1e9}
+    if stream_chunks > 1:
+        # the same copy streamed over `stream_chunks` successive regions of the arena, ONE timing:
+        # what the link sustains right now (on a box that has been busy for minutes this reads a
+        # few per cent under the best-of-5 figure above; on a fresh box the two agree)
+        k = int(min(stream_chunks, arena.numel() // nbytes))
+        for name, d2h in (("d2h_streamed", True), ("h2d_streamed", False)):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(s1)
+            with torch.cuda.stream(s1):
+                for i in range(k):
+                    h = arena[i * nbytes:(i + 1) * nbytes]
+                    if d2h:
+                        h.copy_(d1, non_blocking=True)
+                    else:
+                        d1.copy_(h, non_blocking=True)
+            e1.record(s1)
+            torch.cuda.synchronize()
+            out[name] = k * nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9
+        out["streamed_chunks"] = k
     del d1, d2
     return out
 
@@ -293,7 +313,7 @@ def run_ours(args):
     thp0 = _meminfo_kb("AnonHugePages")
     arena = binding.Mori.mori_host_alloc(cfg.cpu_pool_pages * sh.page_bytes)
     arena_thp_gib = (_meminfo_kb("AnonHugePages") - thp0) / (1 << 20)
-    link = measure_link_peak(arena)
+    link = measure_link_peak(arena, stream_chunks=16)
     paths = {"auto": 0, "zerocopy": 1, "staged": 2, "copyengine": 3}
     r = GpuRunner(cfg, seed, arena=arena, staging_bytes=args.staging_mib << 20,
                   path_demote=paths[args.path_demote], path_promote=paths[args.path_promote],
@@ -424,6 +444,9 @@ def run_ours(args):
         model = sum(memcpy_model_seconds(s["dem"], s["pro"], link) for s in st)
         out = {"frac_of_measured_link_peak": ideal / meas if meas > 0 else None,
                "frac_of_pinned_memcpy_model": model / meas if meas > 0 else None}
+        if "d2h_streamed" in link and meas > 0:      # the same bound from the streamed (sustained) rates
+            sl = dict(link, d2h=link["d2h_streamed"], h2d=link["h2d_streamed"])
+            out["frac_of_streamed_link_rate"] = sum(ideal_seconds(s["dem"], s["pro"], sl) for s in st) / meas
         for name, sel in (("demote_only", lambda s: s["dem"] > 0 and s["pro"] == 0),
                           ("promote_only", lambda s: s["pro"] > 0 and s["dem"] == 0),
                           ("bidirectional", lambda s: s["pro"] > 0 and s["dem"] > 0)):
