@@ -147,13 +147,24 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
     for (int i = 0; i < IPT; ++i) if (victim[i]) vdest[tid * IPT + i] = 1;
     if (tid == 0) bcast[0] = usage_cpu0 + freed;
   } else if (tid == 0) {
-    long long cpu = usage_cpu0;
-    for (int k = 0; k < v; ++k) {
-      const bool fits = cpu + vsize[k] <= cap_cpu;
-      vdest[k] = fits ? 1 : 2;
-      if (fits) cpu += vsize[k];
+    // the loop-carried part is one add and one compare; the sizes are read four ahead so that the
+    // shared-memory latency is off that chain
+    long long room = cap_cpu - usage_cpu0;
+    int k = 0;
+    for (; k + 4 <= v; k += 4) {
+      const int s0 = vsize[k], s1 = vsize[k + 1], s2 = vsize[k + 2], s3 = vsize[k + 3];
+      const bool f0 = s0 <= room; room -= f0 ? s0 : 0;
+      const bool f1 = s1 <= room; room -= f1 ? s1 : 0;
+      const bool f2 = s2 <= room; room -= f2 ? s2 : 0;
+      const bool f3 = s3 <= room; room -= f3 ? s3 : 0;
+      vdest[k] = f0 ? 1 : 2; vdest[k + 1] = f1 ? 1 : 2; vdest[k + 2] = f2 ? 1 : 2; vdest[k + 3] = f3 ? 1 : 2;
     }
-    bcast[0] = cpu;
+    for (; k < v; ++k) {
+      const int s0 = vsize[k];
+      const bool f0 = s0 <= room; room -= f0 ? s0 : 0;
+      vdest[k] = f0 ? 1 : 2;
+    }
+    bcast[0] = cap_cpu - room;
   }
   __syncthreads();
   const long long usage_cpu1 = bcast[0];
