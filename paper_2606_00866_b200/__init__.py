@@ -4,4 +4,4 @@
 ``include/mori.h``); ``paper_2606_00866_b200.workload`` makes the seeded synthetic inputs.
 There is no CPU fallback: using the binding without the built CUDA library raises.
 """
-__all__ = ["binding", "workload", "build"]
+__all__ = ["binding", "workload", "build", "harness", "replicas"]

@@ -6,8 +6,7 @@ and one libmori context.  No oracle here, no CPU fallback: placement comes from
 """
 from __future__ import annotations
 
-import ctypes as C
-from typing import List, Optional
+from typing import Optional
 
 import numpy as np
 import torch
