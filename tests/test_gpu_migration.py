@@ -261,3 +261,24 @@ def test_auto_keeps_issue_order_when_consecutive_calls_take_different_paths(mori
         oracle.demote(L, chunk, pool_m, arena_m, g_b, h_b)
         assert np.array_equal(arena.numpy(), arena_m), rep
     m.close()
+
+
+def test_profile_counts_the_gather_launches_of_a_staged_call(mori):
+    L, H, D, T, P, S = 2, 8, 128, 16, 64, 64
+    chunk = 2 * H * T * D * 2
+    m, pool, arena, pool_m, arena_m, _ = _mk_ctx(mori, L, H, D, T, P, S, 2, 2, staging=10 * L * chunk)
+    g = np.arange(25, dtype=np.int32); h = np.arange(25, dtype=np.int32)
+    m.mori_profile(True)
+    l0 = m.mori_launch_count()
+    m.mori_demote(g, h)
+    m.mori_sync(mori.BOTH)
+    ms, launches, nbytes = m.mori_profile_read(mori.DEMOTE)
+    assert launches == 3 and nbytes == 25 * L * chunk and ms > 0          # segments of 10, 10, 5 pages
+    assert m.mori_launch_count() - l0 == 4                                # + the index upload
+    assert m.mori_profile_read(mori.DEMOTE) == (0.0, 0, 0)                # read clears
+    assert m.mori_profile_read(mori.PROMOTE) == (0.0, 0, 0)
+    m.mori_profile(False)
+    m.mori_demote(g, h)
+    m.mori_sync(mori.BOTH)
+    assert m.mori_profile_read(mori.DEMOTE) == (0.0, 0, 0)
+    m.close()
