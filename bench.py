@@ -564,9 +564,9 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the gather kernel from the committed
 # ncu --set full capture (profiles/); filled in once that capture exists.
 NCU_TRAFFIC: dict = {
-    "bytes_per_launch": 1783.92e6,              # dram__bytes_read.sum 914.44 MB + write 869.48 MB
+    "bytes_per_launch": 1780.91e6,              # dram__bytes_read.sum 914.38 MB + write 866.52 MB
     "algorithmic_bytes_same_launch": 1828.72e6,  # that launch gathered 436 pages of 2 MiB, x2
-    "ratio": 0.975,
+    "ratio": 0.974,
     "source": "profiles/r1_gather_ncu_full.md, launch 4 (ncu --set full, one in-step gather launch)",
 }
 
