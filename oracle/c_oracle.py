@@ -39,7 +39,7 @@ def _load():
         L.oracle_bruteforce_partition.restype = C.c_int
         L.oracle_sticky_rebalance.argtypes = [i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
         L.oracle_sticky_rebalance.restype = C.c_int
-        L.oracle_rank_partition_tiers.argtypes = [i32, vp, vp, i32, vp, vp, vp, vp, vp]
+        L.oracle_rank_partition_tiers.argtypes = [i32, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
         L.oracle_rank_partition_tiers.restype = C.c_int
         L.oracle_bfd_assign.argtypes = [i32, vp, vp, vp, i32, vp, vp, vp]
         L.oracle_bfd_assign.restype = C.c_int
@@ -108,18 +108,27 @@ def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
                 lists=[lists[k, :counts[k]].copy() for k in range(5)])
 
 
-def rank_partition_tiers(iota, s, caps):
-    """oracle_rank_partition_tiers -> dict(order, tier (T = waiting), bounds[T], used[T])."""
+def rank_partition_tiers(iota, s, caps, prev_tier=None):
+    """oracle_rank_partition_tiers -> dict(order, tier (T = waiting), bounds[T], used[T]) and, with
+    ``prev_tier``, moves = [down (most idle first), up (least idle first)]."""
     iota = np.ascontiguousarray(iota, dtype=np.float32)
     s = np.ascontiguousarray(s, dtype=np.int32)
     caps = np.ascontiguousarray(caps, dtype=np.int64)
+    prev = None if prev_tier is None else np.ascontiguousarray(prev_tier, dtype=np.uint8)
     n, T = iota.size, caps.size
     order = np.empty(max(n, 1), np.int32); tier = np.empty(max(n, 1), np.uint8)
     bounds = np.zeros(max(T, 1), np.int32); used = np.zeros(max(T, 1), np.int64)
-    rc = _load().oracle_rank_partition_tiers(n, _p(iota), _p(s), T, _p(caps), _p(order), _p(tier), _p(bounds), _p(used))
+    moves = np.full((2, max(n, 1)), -1, np.int32); counts = np.zeros(2, np.int32)
+    rc = _load().oracle_rank_partition_tiers(n, _p(iota), _p(s), T, _p(caps), _p(prev), _p(order), _p(tier),
+                                             _p(bounds), _p(used), _p(moves), _p(counts))
     if rc != 0:
         raise ValueError(f"oracle_rank_partition_tiers: bad argument (rc={rc})")
-    return dict(order=order[:n], tier=tier[:n], bounds=bounds[:T], used=used[:T])
+    out = dict(order=order[:n], tier=tier[:n], bounds=bounds[:T], used=used[:T])
+    if prev is not None:
+        # rows are n apart in the C layout
+        flat = moves.reshape(-1)
+        out["moves"] = [flat[k * n:k * n + counts[k]].copy() for k in range(2)]
+    return out
 
 
 def bfd_assign(size, iota, flags, free_pages):

@@ -497,8 +497,9 @@ int oracle_bfd_assign(int32_t m, const int32_t *size, const float *iota, const u
  * what is left is Waiting (tier value T).
  */
 int oracle_rank_partition_tiers(int32_t n, const float *iota, const int32_t *s, int32_t n_tiers,
-                                const int64_t *cap, int32_t *order, uint8_t *tier, int32_t *bounds,
-                                int64_t *used) {
+                                const int64_t *cap, const uint8_t *prev_tier, int32_t *order,
+                                uint8_t *tier, int32_t *bounds, int64_t *used, int32_t *moves,
+                                int32_t *move_counts) {
   if (n < 0 || n_tiers < 1 || n_tiers > 8 || !cap) return ORACLE_ERR_ARG;
   for (int t = 0; t < n_tiers; ++t) if (cap[t] < 0) return ORACLE_ERR_ARG;
   for (int32_t p = 0; p < n; ++p) if (s[p] < 0) return ORACLE_ERR_ARG;
@@ -515,5 +516,19 @@ int oracle_rank_partition_tiers(int32_t n, const float *iota, const int32_t *s, 
     bounds[t] = b; used[t] = sum;
   }
   for (int32_t r = b; r < n; ++r) tier[order[r]] = (uint8_t)n_tiers;
+  /* move lists, the two-tier rule of P:L206 / L208 carried over: programs that go DOWN the
+   * hierarchy (to a slower tier or to Waiting) most idle first, programs that go UP least idle
+   * first; prev_tier values >= n_tiers mean Waiting. */
+  if (prev_tier && moves && move_counts) {
+    move_counts[0] = move_counts[1] = 0;
+    for (int32_t r = n - 1; r >= 0; --r) {
+      int32_t p = order[r]; int was = prev_tier[p] < n_tiers ? prev_tier[p] : n_tiers;
+      if (tier[p] > was) moves[0 * (size_t)n + move_counts[0]++] = p;
+    }
+    for (int32_t r = 0; r < n; ++r) {
+      int32_t p = order[r]; int was = prev_tier[p] < n_tiers ? prev_tier[p] : n_tiers;
+      if (tier[p] < was) moves[1 * (size_t)n + move_counts[1]++] = p;
+    }
+  }
   return ORACLE_OK;
 }

@@ -171,7 +171,7 @@ def bfd_assign(size, iota, flags, free_pages):
 # ------------------------------------------------------------------------------------------------
 # NEXT-4(ii): the partition with T capacities
 # ------------------------------------------------------------------------------------------------
-def rank_partition_tiers(iota, s, caps):
+def rank_partition_tiers(iota, s, caps, prev_tier=None):
     s = np.asarray(s, dtype=np.int64)
     n = s.shape[0]
     order = rank(iota)
@@ -186,4 +186,11 @@ def rank_partition_tiers(iota, s, caps):
         base = top if nb > b else base
         b = nb
         bounds.append(b)
-    return dict(order=order, tier=tier, bounds=np.array(bounds, np.int32), used=np.array(used, np.int64))
+    out = dict(order=order, tier=tier, bounds=np.array(bounds, np.int32), used=np.array(used, np.int64))
+    if prev_tier is not None:
+        was = np.minimum(np.asarray(prev_tier, dtype=np.int64), len(caps))
+        now = tier.astype(np.int64)
+        desc = order[::-1]
+        out["moves"] = [desc[now[desc] > was[desc]].astype(np.int32),       # down: most idle first
+                        order[now[order] < was[order]].astype(np.int32)]    # up: least idle first
+    return out

@@ -68,3 +68,30 @@ def test_bad_arguments():
         oracle.rank_partition_tiers([0.1], [1], [1] * 9)
     with pytest.raises(ValueError):
         oracle.rank_partition_tiers([0.1], [1], [-1])
+
+
+def test_move_lists_generalise_the_two_tier_lists():
+    """With T = 2 the down list is demote + drop merged in rank order (most idle first) and the up
+    list is promote + admit + reserve (least idle first) of the pinned two-tier oracle; for any T
+    the C loops and the numpy masks agree, and the lists are exactly the programs whose tier
+    changed."""
+    rng = np.random.default_rng(12)
+    for n in (0, 1, 8, 100, 2000):
+        for _ in range(8):
+            iota, s, prev, cg, cc = _rand_case(rng, n)
+            prev = rng.integers(0, 4, n).astype(np.uint8) if prev is None else prev
+            two = oracle.rank_partition_tiers(iota, s, [cg, cc], prev)
+            ref = oracle.rank_partition(iota, s, prev, cg, cc)
+            pos = np.empty(n, np.int64); pos[ref["order"]] = np.arange(n)
+            down = np.concatenate([ref["lists"][0], ref["lists"][2]]); down = down[np.argsort(-pos[down], kind="stable")]
+            up = np.concatenate([ref["lists"][1], ref["lists"][3], ref["lists"][4]]); up = up[np.argsort(pos[up], kind="stable")]
+            assert np.array_equal(two["moves"][0], down) and np.array_equal(two["moves"][1], up)
+            T = int(rng.integers(1, 9))
+            caps = rng.integers(0, max(2, int(np.sum(s)) // T + 2), T)
+            pv = rng.integers(0, T + 2, n).astype(np.uint8)
+            a, b = oracle.rank_partition_tiers(iota, s, caps, pv), oracle_np.rank_partition_tiers(iota, s, caps, pv)
+            for k in range(2):
+                assert np.array_equal(a["moves"][k], b["moves"][k])
+            changed = set(np.flatnonzero(a["tier"] != np.minimum(pv, T)).tolist())
+            assert changed == set(a["moves"][0].tolist()) | set(a["moves"][1].tolist())
+            assert len(changed) == a["moves"][0].size + a["moves"][1].size
