@@ -291,11 +291,16 @@ int mori_bfd_assign(mori_ctx* ctx, void* stream, int32_t m, const int32_t* size,
  * the move lists.  One launch on `stream`; array pointers are DEVICE pointers.
  *
  *   n_tiers      1 .. 8;  cap_pages  HOST int64[n_tiers], >= 0, read before the call returns
+ *   prev_tier    [n] uint8 or NULL (values >= n_tiers mean Waiting); NULL: no move lists
  *   order [n], tier [n], bounds [n_tiers] (end rank of every tier), used_pages [n_tiers]: out
+ *   moves        [2][n] out: row 0 the programs that go DOWN the hierarchy (to a slower tier or to
+ *                Waiting) most idle first, row 1 those that go UP least idle first -- the order of
+ *                P:L206 / L208; from and to are prev_tier[p] and tier[p].  move_counts [2] out
  */
 int mori_rank_partition_tiers(mori_ctx* ctx, void* stream, int32_t n, const float* idleness,
                               const int32_t* kv_pages, int32_t n_tiers, const int64_t* cap_pages,
-                              int32_t* order, uint8_t* tier, int32_t* bounds, int64_t* used_pages);
+                              const uint8_t* prev_tier, int32_t* order, uint8_t* tier, int32_t* bounds,
+                              int64_t* used_pages, int32_t* moves, int32_t* move_counts);
 
 /* Kernel timing for the roofline: while enabled, every gather/scatter kernel launched by
  * mori_demote / mori_promote is bracketed by CUDA events on its stream.  mori_profile_read

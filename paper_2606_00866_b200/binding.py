@@ -68,7 +68,7 @@ def load():
         L.mori_destroy.argtypes = [vp]
         L.mori_rank_partition.argtypes = [vp, vp, i32, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
         L.mori_sticky_rebalance.argtypes = [vp, vp, i32, vp, vp, vp, vp, i64, i64, vp, vp, vp, vp, vp]
-        L.mori_rank_partition_tiers.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp, vp, vp]
+        L.mori_rank_partition_tiers.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
         L.mori_bfd_assign.argtypes = [vp, vp, i32, vp, vp, vp, i32, vp, vp, vp]
         L.mori_eviction_order.argtypes = [vp, vp, i32, i64, vp, i32, vp, vp, vp, vp]
         L.mori_idleness_update.argtypes = [vp, vp, i64, vp, vp, vp, vp]
@@ -206,12 +206,13 @@ class Mori:
 
     # -- NEXT-4(ii): the partition with T capacities --------------------------------------------
     def mori_rank_partition_tiers(self, n, idleness, kv_pages, cap_pages, order, tier, bounds,
-                                  used_pages, stream=None):
+                                  used_pages, prev_tier=None, moves=None, move_counts=None, stream=None):
         """``cap_pages``: host sequence of 1..8 capacities; the rest are CUDA tensors."""
         caps = np.ascontiguousarray(cap_pages, dtype=np.int64)
         return self._ck(self._lib.mori_rank_partition_tiers(
             self._h, _stream_handle(stream), int(n), _ptr(idleness), _ptr(kv_pages), int(caps.size),
-            caps.ctypes.data, _ptr(order), _ptr(tier), _ptr(bounds), _ptr(used_pages)))
+            caps.ctypes.data, _ptr(prev_tier), _ptr(order), _ptr(tier), _ptr(bounds), _ptr(used_pages),
+            _ptr(moves), _ptr(move_counts)))
 
     # -- NEXT-4(i): Best-Fit-Decreasing across replicas ------------------------------------------
     def mori_bfd_assign(self, size, idleness, flags, free_pages, replica, free_out, stream=None):

@@ -263,15 +263,16 @@ cudaError_t launch_rank_multi(int grid, size_t smem, cudaStream_t s, int n, cons
 
 template <int IPT>
 cudaError_t launch_tiers(int grid, size_t smem, cudaStream_t s, int n, const float* idl, const int32_t* kv,
-                         const mori::TierCaps& caps, int32_t* order, uint8_t* tier, int32_t* bounds,
-                         long long* used, unsigned int* ticket) {
+                         const mori::TierCaps& caps, const uint8_t* prev, int32_t* order, uint8_t* tier,
+                         int32_t* bounds, long long* used, int32_t* moves, int32_t* move_counts,
+                         unsigned int* ticket) {
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(mori::rank_tiers_kernel<IPT>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
-  mori::rank_tiers_kernel<IPT><<<grid, mori::kRankMaxThreads, smem, s>>>(n, idl, kv, caps, order, tier, bounds,
-                                                                        used, ticket);
+  mori::rank_tiers_kernel<IPT><<<grid, mori::kRankMaxThreads, smem, s>>>(n, idl, kv, caps, prev, order, tier, bounds,
+                                                                        used, moves, move_counts, ticket);
   return cudaGetLastError();
 }
 
@@ -521,13 +522,14 @@ int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idl
 }
 
 int mori_rank_partition_tiers(mori_ctx* c, void* stream, int32_t n, const float* idleness, const int32_t* kv_pages,
-                              int32_t n_tiers, const int64_t* cap_pages, int32_t* order, uint8_t* tier,
-                              int32_t* bounds, int64_t* used) {
+                              int32_t n_tiers, const int64_t* cap_pages, const uint8_t* prev_tier, int32_t* order,
+                              uint8_t* tier, int32_t* bounds, int64_t* used, int32_t* moves, int32_t* move_counts) {
   if (!c) return MORI_ERR_INVALID_ARG;
   if (c->sticky) return c->sticky;
   if (n < 0 || n > c->cfg.max_programs) return fail(c, MORI_ERR_INVALID_ARG, "n out of range (0..max_programs)");
   if (n_tiers < 1 || n_tiers > mori::kMaxTiers || !cap_pages) return fail(c, MORI_ERR_INVALID_ARG, "n_tiers must be 1..8");
   if (!bounds || !used || (n > 0 && (!idleness || !kv_pages || !order || !tier))) return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
+  if (prev_tier && (!moves || !move_counts)) return fail(c, MORI_ERR_INVALID_ARG, "prev_tier given but moves/move_counts NULL");
   mori::TierCaps caps{};
   caps.n_tiers = n_tiers;
   for (int t = 0; t < n_tiers; ++t) {
@@ -542,7 +544,7 @@ int mori_rank_partition_tiers(mori_ctx* c, void* stream, int32_t n, const float*
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   long long* u = reinterpret_cast<long long*>(used);
   cudaError_t e;
-#define LT(I) launch_tiers<I>(grid, smem, s, n, idleness, kv_pages, caps, order, tier, bounds, u, tk)
+#define LT(I) launch_tiers<I>(grid, smem, s, n, idleness, kv_pages, caps, prev_tier, order, tier, bounds, u, moves, move_counts, tk)
   switch (n_pad / 1024) {
     case 1: e = LT(1); break;
     case 2: e = LT(2); break;

@@ -298,8 +298,9 @@ struct TierCaps { long long cap[kMaxTiers]; int n_tiers; };
 template <int IPT>
 __global__ void __launch_bounds__(kRankMaxThreads, 1)
 rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __restrict__ kv_pages,
-                  const TierCaps caps, int32_t* __restrict__ order, uint8_t* __restrict__ tier,
-                  int32_t* __restrict__ bounds, long long* __restrict__ used,
+                  const TierCaps caps, const uint8_t* __restrict__ prev_tier, int32_t* __restrict__ order,
+                  uint8_t* __restrict__ tier, int32_t* __restrict__ bounds, long long* __restrict__ used,
+                  int32_t* __restrict__ moves, int32_t* __restrict__ move_counts,
                   unsigned int* __restrict__ ticket) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
@@ -375,6 +376,31 @@ rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __re
   }
 #pragma unroll
   for (int i = 0; i < IPT; ++i) if (prog[i] >= 0) tier[prog[i]] = (uint8_t)my_tier[i];
+  if (prev_tier == nullptr) return;
+
+  // move lists (the two-tier rule of P:L206 / L208 carried over): DOWN the hierarchy most idle
+  // first, UP least idle first; one scan of two 32-bit counters packed in a 64-bit word
+  int dir[IPT];
+  uint64_t packed = 0;
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    dir[i] = -1;
+    if (prog[i] >= 0) {
+      const int pv = prev_tier[prog[i]];
+      const int was = pv < caps.n_tiers ? pv : caps.n_tiers;
+      if (my_tier[i] > was) { dir[i] = 0; packed += 1ull; }
+      else if (my_tier[i] < was) { dir[i] = 1; packed += 1ull << 32; }
+    }
+  }
+  uint64_t ptot;
+  uint64_t pex = block_excl_scan(packed, warp_tot, &ptot);
+  const int n_down = (int)(ptot & 0xFFFFFFFFu);
+#pragma unroll
+  for (int i = 0; i < IPT; ++i) {
+    if (dir[i] == 0) { moves[n_down - 1 - (int)(pex & 0xFFFFFFFFu)] = prog[i]; pex += 1ull; }
+    else if (dir[i] == 1) { moves[(size_t)n + (int)(pex >> 32)] = prog[i]; pex += 1ull << 32; }
+  }
+  if (threadIdx.x == 0) { move_counts[0] = n_down; move_counts[1] = (int)(ptot >> 32); }
 }
 
 }  // namespace mori
