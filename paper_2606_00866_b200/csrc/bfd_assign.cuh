@@ -60,8 +60,7 @@ bfd_assign_kernel(int m, const int32_t* __restrict__ size, const float* __restri
   extern __shared__ __align__(16) unsigned char smem_raw[];
   uint64_t* khi = reinterpret_cast<uint64_t*>(smem_raw);             // [m]
   uint64_t* klo = khi + m;                                           // [m]
-  __shared__ unsigned int s_ticket;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   for (int i = tid; i < m; i += blockDim.x) {
     const int s = size[i] > 0 ? size[i] : 0;
@@ -69,26 +68,9 @@ bfd_assign_kernel(int m, const int32_t* __restrict__ size, const float* __restri
     klo[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;       // least idle, then index
   }
   __syncthreads();
-  const int per = (m + gridDim.x - 1) / gridDim.x;
-  const int lo_i = blockIdx.x * per, hi_i = min(m, lo_i + per);
-  for (int i = lo_i + warp; i < hi_i; i += n_warps) {
-    const uint64_t h = khi[i], l = klo[i];
-    int c = 0;
-    for (int j = lane; j < m; j += 32) {
-      const uint64_t hj = khi[j];
-      c += (hj < h) || (hj == h && klo[j] < l);
-    }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
-    if (lane == 0) order[c] = i;
-  }
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);
-  __syncthreads();
-  if (s_ticket != gridDim.x - 1) return;
-  if (tid == 0) *ticket = 0;
-  __threadfence();
+  if (!rank_by_counting(m, [&](int j, int i) { return khi[j] < khi[i] || (khi[j] == khi[i] && klo[j] < klo[i]); },
+                        order, ticket))
+    return;
 
   // ---- last CTA: sizes in packing order into shared memory, then the one-warp walk ---------------
   int32_t* ssize = reinterpret_cast<int32_t*>(khi);                  // [m] (keys are dead)

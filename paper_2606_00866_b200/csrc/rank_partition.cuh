@@ -54,6 +54,38 @@ __device__ __forceinline__ uint64_t block_excl_scan(uint64_t v, uint64_t* warp_t
   return warp_tot[warp] + incl - v;
 }
 
+// Ranking by counting, shared by every kernel that orders more keys than one CTA sorts well
+// (rank_partition_multi, rank_tiers, sticky_rebalance, bfd_assign).  Keys are unique, so
+// position(i) = #{j : key_j < key_i}.  Every CTA holds all n keys in its shared memory (built by
+// the caller, __syncthreads() done); this CTA ranks the items of its slice -- one warp per item,
+// lanes striding j, shuffle reduction -- and writes order[position] = item.  Returns true in
+// exactly one CTA, the LAST to finish (atomic ticket, reset for the next launch), after every
+// CTA's order[] writes are visible to it (read them with __ldcg): that CTA carries on with the
+// part of the algorithm that needs the whole order.  `less(j, i)` says key_j < key_i.
+template <class Less>
+__device__ __forceinline__ bool rank_by_counting(int n, Less less, int32_t* __restrict__ order,
+                                                 unsigned int* __restrict__ ticket) {
+  __shared__ unsigned int s_ticket;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+  const int per = (n + gridDim.x - 1) / gridDim.x;
+  const int lo = blockIdx.x * per, hi = min(n, lo + per);
+  for (int i = lo + warp; i < hi; i += n_warps) {
+    int c = 0;
+    for (int j = lane; j < n; j += 32) c += less(j, i) ? 1 : 0;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
+    if (lane == 0) order[c] = i;
+  }
+  __threadfence();                                   // this CTA's order[] writes are visible ...
+  __syncthreads();
+  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);    // ... before its ticket is
+  __syncthreads();
+  if (s_ticket != gridDim.x - 1) return false;
+  if (tid == 0) *ticket = 0;                         // ready for the next launch that uses this counter
+  __threadfence();
+  return true;
+}
+
 // Steps a2-a4 for one CTA whose thread t owns ranks [t*IPT, (t+1)*IPT): prog[i] is the program at
 // rank t*IPT + i (or -1 past n).  warp_tot = 33 words, bcast = 2 words of shared memory.
 template <int IPT>
@@ -250,32 +282,11 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
   uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
   uint64_t* warp_tot = keys + n;                                     // [33]
   long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
-  __shared__ unsigned int s_ticket;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
-
+  const int tid = threadIdx.x;
   for (int i = tid; i < n; i += blockDim.x)
     keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;
   __syncthreads();
-
-  const int per = (n + gridDim.x - 1) / gridDim.x;
-  const int lo = blockIdx.x * per, hi = min(n, lo + per);
-  for (int i = lo + warp; i < hi; i += n_warps) {
-    const uint64_t ki = keys[i];
-    int c = 0;
-    for (int j = lane; j < n; j += 32) c += keys[j] < ki;
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
-    if (lane == 0) order[c] = i;
-  }
-
-  // ---- last CTA done? ---------------------------------------------------------------------------
-  __threadfence();                                   // this CTA's order[] writes are visible ...
-  __syncthreads();
-  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);    // ... before its ticket is
-  __syncthreads();
-  if (s_ticket != gridDim.x - 1) return;
-  if (tid == 0) *ticket = 0;                         // ready for the next launch that uses this counter
-  __threadfence();
+  if (!rank_by_counting(n, [&](int j, int i) { return keys[j] < keys[i]; }, order, ticket)) return;
 
   int prog[IPT];
 #pragma unroll
@@ -306,28 +317,11 @@ rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __re
   uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
   uint64_t* warp_tot = keys + n;                                     // [33]
   long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
-  __shared__ unsigned int s_ticket;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+  const int tid = threadIdx.x;
   for (int i = tid; i < n; i += blockDim.x)
     keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;
   __syncthreads();
-  const int per = (n + gridDim.x - 1) / gridDim.x;
-  const int lo = blockIdx.x * per, hi = min(n, lo + per);
-  for (int i = lo + warp; i < hi; i += n_warps) {
-    const uint64_t ki = keys[i];
-    int c = 0;
-    for (int j = lane; j < n; j += 32) c += keys[j] < ki;
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
-    if (lane == 0) order[c] = i;
-  }
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);
-  __syncthreads();
-  if (s_ticket != gridDim.x - 1) return;
-  if (tid == 0) *ticket = 0;
-  __threadfence();
+  if (!rank_by_counting(n, [&](int j, int i) { return keys[j] < keys[i]; }, order, ticket)) return;
 
   int prog[IPT];
   long long incl[IPT];

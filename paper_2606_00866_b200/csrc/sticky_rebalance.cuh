@@ -61,38 +61,17 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
   uint64_t* klo = khi + n;                                           // [n]
   uint64_t* warp_tot = klo + n;                                      // [33]
   long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [4]
-  __shared__ unsigned int s_ticket;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+  const int tid = threadIdx.x;
 
   for (int p = tid; p < n; p += blockDim.x) {
     const int pv = prev_tier[p];
     sticky_key(p, idleness[p], kv_pages[p], pv == 0 ? 0 : (pv == 1 ? 1 : 2), flags[p], khi[p], klo[p]);
   }
   __syncthreads();
-
-  // ---- position of every program of this CTA's slice = number of smaller keys -------------------
-  const int per = (n + gridDim.x - 1) / gridDim.x;
-  const int lo_p = blockIdx.x * per, hi_p = min(n, lo_p + per);
-  for (int p = lo_p + warp; p < hi_p; p += n_warps) {
-    const uint64_t h = khi[p], l = klo[p];
-    int c = 0;
-    for (int j = lane; j < n; j += 32) {
-      const uint64_t hj = khi[j];
-      c += (hj < h) || (hj == h && klo[j] < l);
-    }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
-    if (lane == 0) order[c] = p;
-  }
-
-  // ---- last CTA done? ---------------------------------------------------------------------------
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);
-  __syncthreads();
-  if (s_ticket != gridDim.x - 1) return;
-  if (tid == 0) *ticket = 0;
-  __threadfence();
+  // ---- position of every program = number of smaller 128-bit keys; the last CTA goes on ---------
+  if (!rank_by_counting(n, [&](int j, int i) { return khi[j] < khi[i] || (khi[j] == khi[i] && klo[j] < klo[i]); },
+                        order, ticket))
+    return;
 
   // ---- this thread's positions ------------------------------------------------------------------
   int32_t* vsize = reinterpret_cast<int32_t*>(khi);                  // [n] victims' sizes, by position
