@@ -12,5 +12,5 @@ Two independent statements of the same definitions live here:
 Citations ``P:Lnnn`` are lines of the paper text.
 """
 from .c_oracle import (build, rank_partition, bruteforce_partition, demote, promote,  # noqa: F401
-                       sticky_rebalance, IdlenessTracker, eviction_order, bfd_assign, rank_partition_tiers, lib_path)
+                       sticky_rebalance, IdlenessTracker, eviction_order, bfd_assign, rank_partition_tiers, move_slots, lib_path)
 from . import oracle_np  # noqa: F401

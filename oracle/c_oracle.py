@@ -49,6 +49,8 @@ def _load():
         L.oracle_idleness_update.restype = C.c_int
         L.oracle_idleness_eval.argtypes = [i32, vp, vp, vp, i32, vp, vp, vp]
         L.oracle_idleness_eval.restype = C.c_int
+        L.oracle_move_slots.argtypes = [i64, vp, i64, vp, i64, i64, vp, vp]
+        L.oracle_move_slots.restype = C.c_int
         for f in (L.oracle_demote, L.oracle_promote):
             f.argtypes = [i32, i64, vp, i64, vp, i64, i64, vp, vp]
             f.restype = C.c_int
@@ -229,3 +231,17 @@ def demote(n_layers, chunk, pool, arena, gpu_pages, host_slots):
 
 def promote(n_layers, chunk, pool, arena, host_slots, gpu_pages):
     _move(_load().oracle_promote, n_layers, chunk, pool, arena, host_slots, gpu_pages)
+
+
+def move_slots(page_bytes, src, dst, src_slots, dst_slots):
+    """src arena (flat uint8 [S1][page_bytes]) -> dst arena (flat uint8 [S2][page_bytes]), in place:
+    whole page slots, one memcpy each (the arena <-> arena mover of a three-tier hierarchy)."""
+    assert src.dtype == np.uint8 and dst.dtype == np.uint8 and src.flags.c_contiguous and dst.flags.c_contiguous
+    assert src.size % page_bytes == 0 and dst.size % page_bytes == 0
+    a = np.ascontiguousarray(src_slots, dtype=np.int32)
+    b = np.ascontiguousarray(dst_slots, dtype=np.int32)
+    assert a.shape == b.shape
+    rc = _load().oracle_move_slots(int(page_bytes), _p(src), src.size // page_bytes, _p(dst),
+                                   dst.size // page_bytes, a.size, _p(a), _p(b))
+    if rc != 0:
+        raise ValueError(f"oracle_move_slots: bad argument (rc={rc})")

@@ -30,6 +30,7 @@
  *   oracle_eviction_order        P:L212-221 (section 4.3.2)         tests/test_oracle_eviction_pins.py
  *   oracle_bfd_assign            P:L208-210                         tests/test_oracle_bfd_pins.py
  *   oracle_rank_partition_tiers  P:L339-351 (section 7.1)           tests/test_oracle_tiers_pins.py
+ *   oracle_move_slots            P:L339-351 (arena <-> arena)       tests/test_oracle_tiers_pins.py
  * Every function is pinned (none is "parity unpinned"); DESIGN.md sections 10 and 12-15 say by what.
  *
  * Pins (tests/test_oracle_pins.py): brute force on n <= 9, numpy stable argsort / cumsum /
@@ -220,6 +221,26 @@ int oracle_promote(int32_t n_layers, int64_t chunk, uint8_t *pool, int64_t pool_
     if (g < 0 || g >= pool_pages || h < 0 || h >= arena_slots) return ORACLE_ERR_ARG;
     for (int64_t l = 0; l < n_layers; ++l)
       memcpy(pool + (l * pool_pages + g) * chunk, arena + (h * n_layers + l) * chunk, (size_t)chunk);
+  }
+  return ORACLE_OK;
+}
+
+/*
+ * NEXT-4(ii): with "an intermediate tier" between GPU HBM and host DRAM a
+ * program can also move between two page-major arenas.  A slot is one whole logical page (all
+ * layers, K and V: page_bytes = n_layers * chunk, contiguous), so the move is one memcpy per page:
+ *   dst + dst_slots[j] * page_bytes  <-  src + src_slots[j] * page_bytes.
+ * Pinned by tests/test_oracle_tiers_pins.py (byte-by-byte loop, fancy-index restatement, and the
+ * reduction of a three-pool epoch with an empty middle tier to the two-pool epochs).
+ */
+int oracle_move_slots(int64_t page_bytes, const uint8_t *src, int64_t src_slots_n, uint8_t *dst,
+                      int64_t dst_slots_n, int64_t total_pages, const int32_t *src_slots,
+                      const int32_t *dst_slots) {
+  if (page_bytes <= 0 || total_pages < 0) return ORACLE_ERR_ARG;
+  for (int64_t j = 0; j < total_pages; ++j) {
+    int64_t a = src_slots[j], b = dst_slots[j];
+    if (a < 0 || a >= src_slots_n || b < 0 || b >= dst_slots_n) return ORACLE_ERR_ARG;
+    memcpy(dst + b * page_bytes, src + a * page_bytes, (size_t)page_bytes);
   }
   return ORACLE_OK;
 }

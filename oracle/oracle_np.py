@@ -78,6 +78,13 @@ def promote(n_layers, chunk, pool, arena, host_slots, gpu_pages):
 ACTING, READY, NEW = 1, 2, 4
 
 
+def move_slots(page_bytes, src, dst, src_slots, dst_slots):
+    """Arena -> arena as one fancy-index assignment of whole page slots."""
+    sv = src.reshape(-1, page_bytes)
+    dv = dst.reshape(-1, page_bytes)
+    dv[np.asarray(dst_slots, dtype=np.int64)] = sv[np.asarray(src_slots, dtype=np.int64)]
+
+
 def sticky_rebalance(iota, s, prev_tier, flags, cap_gpu, cap_cpu):
     """Second statement of oracle_sticky_rebalance: instead of picking one victim / one candidate
     at a time it sorts each group once by the paper's priority and cuts the sorted list with a

@@ -518,3 +518,121 @@ class Sim:
         self.epoch += 1
         self._pending = None
         return plan
+
+
+# --------------------------------------------------------------------------------------------
+# more tiers (SURVEY 8f NEXT-4 ii): the same epoch state machine over a hierarchy
+# --------------------------------------------------------------------------------------------
+class SimTiers:
+    """Epoch state machine for T storage tiers: tier 0 is the paged GPU pool, tiers 1 .. T-1 are
+    page-major arenas from fast to slow (e.g. peer-GPU HBM, then host DRAM: the "intermediate tier"
+    of P:L347), tier value T is Waiting.  Like ``Sim`` it holds none of the method's arithmetic:
+    the placement (tier per program + the DOWN / UP move lists of a T-capacity partition) comes
+    from the caller, and is turned into page / slot tables here.
+
+    ``pool_ids[t]`` = physical pages / slots of tier t; ``caps[t]`` = the capacity the ranker is
+    given (physical minus headroom, R23).  Ids freed by a move of this epoch are not
+    handed out again before the next join ("sync_all"), so moves of one phase never alias and the
+    movers need no cross-tier tickets."""
+
+    def __init__(self, cfg: Config, seed: int, pool_ids: List[int], caps: List[int]):
+        assert len(pool_ids) == len(caps) >= 1
+        self.cfg, self.seed, self.T = cfg, seed, len(caps)
+        self.pool_ids, self.caps = list(pool_ids), list(caps)
+        self.trace = Trace(cfg, seed)
+        n = cfg.n_programs
+        arng = np.random.Generator(np.random.PCG64(config_seed(seed, cfg) + 7919)) if cfg.random_pages else None
+        self.alloc = [IdAllocator(pool_ids[0], arng)] + [IdAllocator(k, None) for k in pool_ids[1:]]
+        self.tier = np.full(n, self.T, np.uint8)
+        self.where = np.full(n, -1, np.int64)               # tier that holds the program's bytes, -1: none
+        self.ids: List[np.ndarray] = [np.zeros(0, np.int32) for _ in range(n)]
+        self.epoch = 0
+        self._pending = None
+
+    def begin_epoch(self) -> EpochPlan:
+        # the trace gates on "not in the GPU tier": tier 0 here as well
+        iota, tokens, replaced = self.trace.advance(np.where(self.tier == 0, TIER_GPU, TIER_WAIT).astype(np.uint8))
+        for p in np.flatnonzero(replaced):
+            self._drop(int(p))
+            self.tier[p] = self.T
+        Tk = self.cfg.shape.page_tokens
+        kv_pages = ((tokens + Tk - 1) // Tk).astype(np.int32)
+        plan = EpochPlan(iota=iota, kv_pages=kv_pages, prev_tier=self.tier.copy())
+        self._pending = plan
+        return plan
+
+    def _drop(self, p: int):
+        if self.where[p] >= 0 and self.ids[p].size:
+            self.alloc[self.where[p]].release(self.ids[p])
+        self.ids[p] = np.zeros(0, np.int32)
+        self.where[p] = -1
+
+    def apply_placement(self, tier: np.ndarray, moves: List[np.ndarray]) -> EpochPlan:
+        """``moves`` = [down (most idle first), up (least idle first)] as the T-capacity partition
+        lists them.  plan.ops entries: ("move", program, from_tier, to_tier, src_ids, dst_ids) and
+        ("sync_all",)."""
+        plan = self._pending
+        tier = np.asarray(tier, dtype=np.uint8)
+        queue = []
+        for p in list(moves[0]) + list(moves[1]):
+            p = int(p)
+            to = int(tier[p])
+            if to >= self.T:                                 # P:L178 "discarded entirely"
+                self._drop(p)
+            elif self.where[p] >= 0 and self.where[p] != to and self.ids[p].size:
+                queue.append((p, int(self.where[p]), to))
+            # else: a label without bytes (R9); a GPU-tier one is filled in end_epoch
+        ops, progressed_since_sync = [], True
+        while queue:
+            rest, did = [], False
+            for p, frm, to in queue:
+                k = int(self.ids[p].size)
+                al = self.alloc[to]
+                if al.n_free(clean_only=True) >= k:
+                    dst, _ = al.alloc(k, clean_only=True) if to == 0 else al.alloc_run(k)
+                    src = self.ids[p]
+                    ops.append(("move", p, frm, to, src.copy(), dst))
+                    self.alloc[frm].release(src, tag=1)      # not reusable before the next join
+                    self.ids[p], self.where[p] = dst, to
+                    plan.demote_pages += k if to > frm else 0
+                    plan.promote_pages += k if to < frm else 0
+                    did = True
+                else:
+                    rest.append((p, frm, to))
+            queue = rest
+            if did:
+                progressed_since_sync = True
+            elif queue:
+                if not progressed_since_sync:
+                    raise MemoryError("placement does not fit the physical pools")
+                ops.append(("sync_all",))
+                for al in self.alloc:
+                    al.clear_tags()
+                progressed_since_sync = False
+        plan.ops = ops
+        self.tier = tier.copy()
+        return plan
+
+    def end_epoch(self) -> EpochPlan:
+        plan = self._pending
+        for al in self.alloc:
+            al.clear_tags()
+        for p in np.flatnonzero(self.tier == 0):             # admit + growth: recompute prefill (P:L178)
+            have = int(self.ids[p].size) if self.where[p] == 0 else 0
+            need = int(plan.kv_pages[p]) - have
+            if need > 0:
+                new, _ = self.alloc[0].alloc(need)
+                plan.fills.append((int(self.trace.uid[p]), have, new))
+                self.ids[p] = np.concatenate([self.ids[p], new]) if have else new
+                self.where[p] = 0
+        self.epoch += 1
+        self._pending = None
+        return plan
+
+    def resident(self):
+        """-> per tier, [(uid, 0, ids)] of every program whose bytes live there."""
+        out = [[] for _ in range(self.T)]
+        for p in range(self.cfg.n_programs):
+            if self.where[p] >= 0 and self.ids[p].size:
+                out[self.where[p]].append((int(self.trace.uid[p]), 0, self.ids[p]))
+        return out

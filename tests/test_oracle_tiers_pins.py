@@ -95,3 +95,173 @@ def test_move_lists_generalise_the_two_tier_lists():
             changed = set(np.flatnonzero(a["tier"] != np.minimum(pv, T)).tolist())
             assert changed == set(a["moves"][0].tolist()) | set(a["moves"][1].tolist())
             assert len(changed) == a["moves"][0].size + a["moves"][1].size
+
+
+# ------------------------------------------------------------------------------------------------
+# the arena <-> arena mover and whole three-pool epochs (an intermediate tier)
+# ------------------------------------------------------------------------------------------------
+def test_move_slots_is_a_per_page_copy():
+    rng = np.random.default_rng(3)
+    page = 48
+    src = rng.integers(0, 256, 9 * page, dtype=np.uint8)
+    dst0 = rng.integers(0, 256, 7 * page, dtype=np.uint8)
+    a, b = np.array([8, 0, 3, 3], np.int32), np.array([1, 6, 0, 4], np.int32)
+    dst = dst0.copy()
+    oracle.move_slots(page, src, dst, a, b)
+    want = dst0.copy()
+    for j in range(len(a)):                                  # byte by byte
+        for x in range(page):
+            want[b[j] * page + x] = src[a[j] * page + x]
+    assert np.array_equal(dst, want)
+    dst2 = dst0.copy()
+    oracle_np.move_slots(page, src, dst2, a, b)              # fancy-index restatement
+    assert np.array_equal(dst2, want)
+    untouched = np.setdiff1d(np.arange(7), b)
+    assert np.array_equal(dst.reshape(7, page)[untouched], dst0.reshape(7, page)[untouched])
+    back = np.zeros_like(src)                                # round trip into other slots
+    oracle.move_slots(page, dst, back, b[:3], np.array([2, 5, 7], np.int32))
+    assert np.array_equal(back.reshape(9, page)[[2, 5, 7]], src.reshape(9, page)[a[:3]])
+    with pytest.raises(ValueError):
+        oracle.move_slots(page, src, dst, np.array([9], np.int32), np.array([0], np.int32))
+    with pytest.raises(ValueError):
+        oracle.move_slots(page, src, dst, np.array([0], np.int32), np.array([7], np.int32))
+    oracle.move_slots(page, src, dst, np.zeros(0, np.int32), np.zeros(0, np.int32))
+
+
+def test_move_slots_equals_demote_of_a_one_layer_pool():
+    """An arena described as a pool of ONE layer whose chunk is a whole page is the same bytes, so
+    the arena <-> arena move must equal the (already pinned) pool -> arena mover on that view."""
+    rng = np.random.default_rng(4)
+    page, S1, S2 = 96, 20, 30
+    src = rng.integers(0, 256, S1 * page, dtype=np.uint8)
+    d1 = rng.integers(0, 256, S2 * page, dtype=np.uint8)
+    d2 = d1.copy()
+    a = rng.permutation(S1)[:12].astype(np.int32)
+    b = rng.permutation(S2)[:12].astype(np.int32)
+    oracle.move_slots(page, src, d1, a, b)
+    oracle.demote(1, page, src, d2, a, b)
+    assert np.array_equal(d1, d2)
+
+
+def three_pool_epochs(cfg, seed, pool_ids, caps, epochs, on_epoch=None):
+    """Whole epochs of a three-tier hierarchy on the ORACLE side: oracle_rank_partition_tiers decides,
+    workload.SimTiers turns the move lists into tables, the oracle's memcpy movers carry them out on
+    byte mirrors of the three pools.  Yields nothing; calls on_epoch(e, sim, plan, res, mirrors)."""
+    from paper_2606_00866_b200 import workload as W
+    sh = cfg.shape
+    sim = W.SimTiers(cfg, seed, pool_ids, caps)
+    pool = np.zeros(sh.n_layers * pool_ids[0] * sh.chunk_bytes, np.uint8)
+    mid = np.zeros(pool_ids[1] * sh.page_bytes, np.uint8)
+    host = np.zeros(pool_ids[2] * sh.page_bytes, np.uint8)
+    for e in range(epochs):
+        plan = sim.begin_epoch()
+        res = oracle.rank_partition_tiers(plan.iota, plan.kv_pages, caps, plan.prev_tier)
+        sim.apply_placement(res["tier"], res["moves"])
+        oracle_apply_moves(plan.ops, sh, pool, mid, host)
+        sim.end_epoch()
+        pv = pool.reshape(sh.n_layers, pool_ids[0], sh.chunk_bytes)
+        for uid, first, pages in plan.fills:
+            for j, g in enumerate(pages):
+                pv[:, g] = W.page_content(seed, uid, first + j, sh)
+        if on_epoch:
+            on_epoch(e, sim, plan, res, (pool, mid, host))
+    return sim, (pool, mid, host)
+
+
+def oracle_apply_moves(ops, sh, pool, mid, host):
+    arenas = {1: mid, 2: host}
+    for op in ops:
+        if op[0] != "move":
+            continue
+        _, p, frm, to, src, dst = op
+        if frm == 0:
+            oracle.demote(sh.n_layers, sh.chunk_bytes, pool, arenas[to], src, dst)
+        elif to == 0:
+            oracle.promote(sh.n_layers, sh.chunk_bytes, pool, arenas[frm], src, dst)
+        else:
+            oracle.move_slots(sh.page_bytes, arenas[frm], arenas[to], src, dst)
+
+
+def _check_resident_against_generator(sim, mirrors, seed):
+    """Every byte of every resident page, in whichever pool it lives, equals the counter-based
+    generator G(seed, uid, logical page): a check that needs no second mover."""
+    from paper_2606_00866_b200 import workload as W
+    sh = sim.cfg.shape
+    pool, mid, host = mirrors
+    views = [pool.reshape(sh.n_layers, -1, sh.chunk_bytes), mid.reshape(-1, sh.n_layers, sh.chunk_bytes),
+             host.reshape(-1, sh.n_layers, sh.chunk_bytes)]
+    n = 0
+    for t, tri in enumerate(sim.resident()):
+        for uid, first, ids in tri:
+            for j, i in enumerate(ids):
+                want = W.page_content(seed, uid, first + j, sh)
+                have = views[0][:, i] if t == 0 else views[t][i]
+                assert np.array_equal(have, want), (t, uid, j)
+                n += 1
+    return n
+
+
+def _small_cfg2():
+    """cfg 2's scaled twin (same programs, page counts and trace) with a small KV shape, so that the
+    byte-level checks of these CPU pins stay fast: 16 KiB pages instead of 2 MiB."""
+    from dataclasses import replace
+    from paper_2606_00866_b200 import workload as W
+    return replace(W.get_config(2, 128), shape=W.KVShape(4, 2, 32, 16))
+
+
+def test_three_pool_epochs_keep_every_resident_page_intact():
+    cfg = _small_cfg2()
+    mid_ids, mid_cap = 160, 160 - cfg.max_program_pages
+    pool_ids = [cfg.gpu_pool_pages, mid_ids, cfg.cpu_pool_pages]
+    caps = [cfg.cap_gpu_pages, mid_cap, cfg.cap_cpu_pages]
+    seen = {"pairs": set(), "pages": 0}
+
+    def on_epoch(e, sim, plan, res, mirrors):
+        for op in plan.ops:
+            if op[0] == "move":
+                seen["pairs"].add((op[2], op[3]))
+        # capacities of the partition hold for what is physically resident too
+        for t in range(3):
+            assert sum(int(x[2].size) for x in sim.resident()[t]) <= pool_ids[t]
+        if e % 5 == 4:
+            seen["pages"] += _check_resident_against_generator(sim, mirrors, 866)
+
+    three_pool_epochs(cfg, 866, pool_ids, caps, 40, on_epoch)
+    assert seen["pages"] > 500
+    # the hierarchy was really exercised: bytes went down and up between all neighbouring pairs
+    assert {(0, 1), (1, 0), (1, 2)} <= seen["pairs"], seen["pairs"]
+
+
+def test_three_pool_epochs_with_an_empty_middle_tier_are_the_two_pool_epochs():
+    """T = 3 with capacity 0 in the middle reduces to the pinned two-tier path: the same tiers and
+    the same programs moving the same way every epoch (down = demote + drop, up = promote + admit +
+    reserve), and the same logical bytes for every program afterwards."""
+    from paper_2606_00866_b200 import workload as W
+    cfg = _small_cfg2()
+    seed = 867
+    sim2 = W.Sim(cfg, seed)
+    two = []
+
+    for e in range(25):
+        plan = sim2.begin_epoch()
+        r2 = oracle.rank_partition(plan.iota, plan.kv_pages, plan.prev_tier, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+        sim2.apply_placement(r2["tier"], r2["lists"])
+        sim2.end_epoch()
+        two.append((r2, plan))
+
+    def on_epoch(e, sim, plan, res, mirrors):
+        r2, plan2 = two[e]
+        assert np.array_equal(plan.iota, plan2.iota) and np.array_equal(plan.kv_pages, plan2.kv_pages)
+        t3 = res["tier"].copy()
+        assert not np.any(t3 == 1)                           # nobody fits a tier of capacity 0 (sizes > 0)
+        assert np.array_equal(np.where(t3 == 2, 1, np.where(t3 == 3, 2, t3)), r2["tier"])
+        moved3 = {(op[1], op[2], op[3]) for op in plan.ops if op[0] == "move"}
+        moved2 = {(op[2], 0, 2) for op in plan2.ops if op[0] == "demote"} | \
+                 {(op[2], 2, 0) for op in plan2.ops if op[0] == "promote"}
+        assert moved3 == moved2, e
+        assert plan.demote_pages == plan2.demote_pages and plan.promote_pages == plan2.promote_pages
+
+    sim3, mirrors = three_pool_epochs(cfg, seed, [cfg.gpu_pool_pages, 8, cfg.cpu_pool_pages],
+                                      [cfg.cap_gpu_pages, 0, cfg.cap_cpu_pages], 25, on_epoch)
+    assert _check_resident_against_generator(sim3, mirrors, seed) > 100
+    assert not mirrors[1].any()                              # nothing ever touched the middle pool
