@@ -58,23 +58,6 @@ def _meminfo_kb(key: str) -> int:
     return 0
 
 
-def _pick_scale(cfg_index: int, world: int, W) -> int:
-    """SURVEY 8(d) scale rule: the smallest power of two that lets the pinned arena of every
-    rank fit host RAM (70 % of MemTotal, shared by the ranks of the node -- MemTotal, not
-    MemAvailable, so that every rank of a job picks the same scale) and the pool fit HBM."""
-    import torch
-    avail = int(_meminfo_kb("MemTotal") * 1024 * 0.70) // max(1, world)
-    free_hbm, _ = torch.cuda.mem_get_info()
-    scale = 1
-    while True:
-        cfg = W.get_config(cfg_index, scale)
-        sh = cfg.shape
-        if (cfg.cpu_pool_pages * sh.page_bytes <= avail
-                and cfg.gpu_pool_pages * sh.page_bytes + (3 << 30) <= free_hbm):
-            return scale
-        scale *= 2
-
-
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons every 200 ms while the timed region runs
     (B200_PROFILING.md 'clocks line')."""
@@ -208,24 +191,62 @@ def memcpy_model_seconds(dem_bytes, pro_bytes, link):
 # ------------------------------------------------------------------------------------------------
 # the CPU oracle legs (cpu_baseline, --impl reference): the only places bench.py touches oracle/
 # ------------------------------------------------------------------------------------------------
-class OracleEpochs:
-    """The oracle as it stands on a scaled twin of the bench workload (same L/H/D/T/n, pools and
-    contexts divided by ``scale`` so that byte mirrors of both pools fit host RAM)."""
+def _cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
-    def __init__(self, cfg_index: int, scale: int, seed: int):
+
+class OracleEpochs:
+    """The oracle as it stands on a scaled twin of a bench workload (same L/H/D/T/n, pools and
+    contexts divided by ``scale`` so that byte mirrors of both pools fit host RAM).  ``threads``
+    > 1 splits the pages of every move evenly over that many host threads, each calling the
+    oracle's single-threaded mover on its share (the threading lives here, not in oracle.c; ctypes
+    releases the GIL for the duration of a call)."""
+
+    def __init__(self, cfg_index: int, scale: int, seed: int, f_busy=None):
         import oracle
         from paper_2606_00866_b200 import workload as W
         self.oracle, self.W = oracle, W
         oracle.build()
-        self.cfg = W.get_config(cfg_index, scale)
+        self.cfg = W.get_config(cfg_index, scale, f_busy)
         sh = self.cfg.shape
         self.sim = W.Sim(self.cfg, seed)
-        rng = np.random.default_rng(seed)
-        self.pool = rng.integers(0, 256, sh.n_layers * self.cfg.gpu_pool_pages * sh.chunk_bytes, dtype=np.uint8)
-        self.arena = np.zeros(self.cfg.cpu_pool_pages * sh.page_bytes, np.uint8)
-        self.arena[::4096] = 1                       # touch every page before timing
+        # byte mirrors of both pools; contents are irrelevant to the timing, every page is touched
+        self.pool = np.empty(sh.n_layers * self.cfg.gpu_pool_pages * sh.chunk_bytes, np.uint8)
+        self.arena = np.empty(self.cfg.cpu_pool_pages * sh.page_bytes, np.uint8)
+        self._touch(self.pool, 0x5A)
+        self._touch(self.arena, 0x01)
+        self.pool_exec = None
 
-    def step(self):
+    @staticmethod
+    def _touch(a, v):
+        from concurrent.futures import ThreadPoolExecutor
+        n = max(1, min(os.cpu_count() or 1, 8))
+        step = -(-a.size // n)
+        with ThreadPoolExecutor(n) as ex:
+            list(ex.map(lambda k: a[k * step:(k + 1) * step:4096].fill(v), range(n)))
+
+    def _move(self, fn, a, b, threads):
+        sh = self.cfg.shape
+        if threads <= 1 or len(a) < 2 * threads:
+            fn(sh.n_layers, sh.chunk_bytes, self.pool, self.arena, a, b)
+            return
+        if self.pool_exec is None or self.pool_exec._max_workers != threads:
+            from concurrent.futures import ThreadPoolExecutor
+            self.pool_exec = ThreadPoolExecutor(threads)
+        cuts = np.linspace(0, len(a), threads + 1).astype(int)
+        futs = [self.pool_exec.submit(fn, sh.n_layers, sh.chunk_bytes, self.pool, self.arena,
+                                      a[cuts[t]:cuts[t + 1]], b[cuts[t]:cuts[t + 1]]) for t in range(threads)]
+        for f in futs:
+            f.result()
+
+    def step(self, threads=1):
         """One epoch.  -> (seconds in the oracle, bytes migrated)."""
         cfg, sh, o = self.cfg, self.cfg.shape, self.oracle
         plan = self.sim.begin_epoch()
@@ -236,51 +257,82 @@ class OracleEpochs:
         t0 = time.perf_counter()
         for op in plan.ops:
             if op[0] == "demote":
-                o.demote(sh.n_layers, sh.chunk_bytes, self.pool, self.arena, op[3], op[4])
+                self._move(o.demote, op[3], op[4], threads)
             elif op[0] == "promote":
-                o.promote(sh.n_layers, sh.chunk_bytes, self.pool, self.arena, op[3], op[4])
+                self._move(o.promote, op[3], op[4], threads)
         t += time.perf_counter() - t0
         self.sim.end_epoch()                         # page contents are irrelevant to the timing
         return t, (plan.demote_pages + plan.promote_pages) * sh.page_bytes
 
 
-def cpu_baseline(cfg_index: int, budget_s: float = 12.0, scale: int = 16):
-    oe = OracleEpochs(cfg_index, scale, SEED)
+def cpu_baseline(cfg_index: int, budget_s: float = 6.0, scale: int = 16, f_busy=None, max_bytes=12 * GIB):
+    """The oracle as it stands on the box's host cores: one thread, then all cores (pages of every
+    move split evenly), on alternating epochs of the scaled twin of config ``cfg_index``."""
+    from paper_2606_00866_b200 import workload as W
+    while True:                                      # mirrors of both pools must stay small enough to touch quickly
+        c = W.get_config(cfg_index, scale, f_busy)
+        if (c.gpu_pool_pages + c.cpu_pool_pages) * c.shape.page_bytes <= max_bytes or c.cpu_pool_pages < 64:
+            break
+        scale *= 2
+    oe = OracleEpochs(cfg_index, scale, SEED, f_busy)
+    cores = os.cpu_count() or 1
     for _ in range(3):
         oe.step()
-    t_sum, b_sum, n = 0.0, 0, 0
-    t_wall = time.perf_counter()
-    while (time.perf_counter() - t_wall < budget_s and n < oe.cfg.epochs - 3) or n < 3:
-        t, b = oe.step()
-        t_sum += t; b_sum += b; n += 1
-    return {"value": b_sum / t_sum / 1e9 if t_sum > 0 else 0.0, "unit": UNIT, "cores": 1,
-            "host_cores_available": os.cpu_count(), "kind": "oracle",
-            "sample": f"{n} epochs of {oe.cfg.name} (cfg {cfg_index} with pools and contexts / {scale}, "
-                      f"same L/H/D/T/n), {b_sum / GIB:.1f} GiB migrated host->host by oracle.c "
-                      f"(qsort + prefix loop + per-(page,layer) memcpy, single thread)"}
+    acc = {1: [0.0, 0, 0], cores: [0.0, 0, 0]}
+    t_wall, n = time.perf_counter(), 0
+    while (time.perf_counter() - t_wall < budget_s and n < oe.cfg.epochs - 3) or n < 4:
+        th = 1 if n % 2 == 0 else cores
+        t, b = oe.step(th)
+        acc[th][0] += t; acc[th][1] += b; acc[th][2] += 1
+        n += 1
+    def gbps(a):
+        return a[1] / a[0] / 1e9 if a[0] > 0 and a[1] > 0 else 0.0
+    sample = (f"{n} epochs of {oe.cfg.name} (cfg {cfg_index} with pools and contexts / {scale}, same L/H/D/T/n), "
+              f"alternating 1 thread / {cores} threads; {acc[1][1] / GIB:.1f} + {acc[cores][1] / GIB:.1f} GiB migrated "
+              f"host->host by oracle.c (qsort + prefix loop + per-(page,layer) memcpy; threads split a move's pages evenly)")
+    return {"value": gbps(acc[1]), "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+            "all_cores": {"value": gbps(acc[cores]), "unit": UNIT, "cores": cores},
+            "host_cores_available": cores, "cpu_model": _cpu_model(), "scale": scale, "workload": oe.cfg.name}
+
+
+def _reference_scale(cfg_index: int, W, f_busy=None) -> int:
+    """The smallest power-of-two scale whose byte mirrors of BOTH pools fit this host (80 % of
+    MemAvailable): /2 for cfg 2 on a 196 GiB box."""
+    avail = int(_meminfo_kb("MemAvailable") * 1024 * 0.80)
+    scale = 1
+    while True:
+        c = W.get_config(cfg_index, scale, f_busy)
+        if (c.gpu_pool_pages + c.cpu_pool_pages) * c.shape.page_bytes <= avail:
+            return scale
+        scale *= 2
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    scale = 16
-    oe = OracleEpochs(args.config, scale, SEED)
+    from paper_2606_00866_b200 import workload as W
+    scale = args.scale or _reference_scale(args.config, W, args.f_busy)
+    threads = args.ref_threads if args.ref_threads > 0 else 1
+    oe = OracleEpochs(args.config, scale, SEED, args.f_busy)
     for _ in range(args.warmup):
-        oe.step()
+        oe.step(threads)
     t_sum, b_sum = 0.0, 0
     for _ in range(args.steps):
-        t, b = oe.step()
+        t, b = oe.step(threads)
         t_sum += t; b_sum += b
     v = b_sum / t_sum / 1e9 if t_sum > 0 else 0.0
-    sample = (f"{args.steps} epochs of {oe.cfg.name} (pools and contexts / {scale}), "
-              f"{b_sum / GIB:.1f} GiB migrated host->host, single thread")
+    sh = oe.cfg.shape
+    sample = (f"{args.steps} epochs of {oe.cfg.name} (pools and contexts / {scale}: byte mirrors of "
+              f"{oe.cfg.gpu_pool_pages * sh.page_bytes / GIB:.0f} + {oe.cfg.cpu_pool_pages * sh.page_bytes / GIB:.0f} GiB), "
+              f"{b_sum / GIB:.1f} GiB migrated host->host, {threads} thread(s)")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_sum / max(1, args.steps),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
-        "data": "synthetic", "config": {"workload": oe.cfg.name, "scale": scale},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "data": "synthetic", "config": {"workload": oe.cfg.name, "bj_config": f"configs[{args.config - 1}]", "scale": scale},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                         "host_cores_available": os.cpu_count(), "cpu_model": _cpu_model()},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -288,46 +340,73 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------------
-def run_ours(args):
+def _load_ncu_traffic() -> dict:
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the gather kernel, from the tracked
+    summary of the committed ``ncu --set full`` capture (profiles/ncu_traffic.json names the command,
+    the launch and its size)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f)
+    except (OSError, ValueError):
+        return {}
+
+
+def _hbm_peak():
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        return float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def link_report(st, link):
+    """Achieved fractions of the measured pinned-memcpy peaks over the steps ``st``."""
+    ideal = sum(ideal_seconds(s["dem"], s["pro"], link) for s in st)
+    meas = sum(s["ms"] for s in st) * 1e-3
+    model = sum(memcpy_model_seconds(s["dem"], s["pro"], link) for s in st)
+    out = {"frac_of_measured_link_peak": ideal / meas if meas > 0 and ideal > 0 else None,
+           "frac_of_pinned_memcpy_model": model / meas if meas > 0 and model > 0 else None}
+    if "d2h_streamed" in link and meas > 0:      # the same bound from the streamed (sustained) rates
+        sl = dict(link, d2h=link["d2h_streamed"], h2d=link["h2d_streamed"])
+        out["frac_of_streamed_link_rate"] = sum(ideal_seconds(s["dem"], s["pro"], sl) for s in st) / meas
+    for name, sel in (("demote_only", lambda s: s["dem"] > 0 and s["pro"] == 0),
+                      ("promote_only", lambda s: s["pro"] > 0 and s["dem"] == 0),
+                      ("bidirectional", lambda s: s["pro"] > 0 and s["dem"] > 0)):
+        sub = [s for s in st if sel(s)]
+        if sub:
+            byt = sum(s["dem"] + s["pro"] for s in sub)
+            sec = sum(s["ms"] for s in sub) * 1e-3
+            peak = {"demote_only": link["d2h"], "promote_only": link["h2d"]}.get(name)
+            ent = {"steps": len(sub), "GBps": byt / sec / 1e9, "GiB": byt / GIB}
+            ent["frac"] = (ent["GBps"] / peak) if peak else \
+                sum(ideal_seconds(s["dem"], s["pro"], link) for s in sub) / sec
+            if not peak:
+                ent["frac_of_pinned_memcpy_model"] = \
+                    sum(memcpy_model_seconds(s["dem"], s["pro"], link) for s in sub) / sec
+            out[name] = ent
+    return out
+
+
+def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, do_e2e=True,
+                   gather_reps=20, clocks_on=True, size_matched_leg=True):
+    """K timed epochs of one config on the CUDA path (device-resident inputs), the same epochs again
+    through the public API from host buffers, the in-step roofline of the gather/scatter kernel and
+    the standalone device halves.  -> dict of raw totals and derived records."""
     import torch
-    import torch.distributed as dist
-    from paper_2606_00866_b200 import binding, replicas, workload as W
+    from paper_2606_00866_b200 import binding, workload as W
     from paper_2606_00866_b200.harness import GpuRunner
-
-    rank, world, local = replicas.env_rank()
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
-    if args.device_index >= 0:
-        local = args.device_index                    # testing only: several replicas on one GPU
-    torch.cuda.set_device(local)
-    if world > 1:
-        if args.backend == "nccl":
-            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-        else:
-            dist.init_process_group(args.backend)
-
-    scale = args.scale or _pick_scale(args.config, world, W)
-    cfg = W.get_config(args.config, scale)
     sh = cfg.shape
-    seed = replicas.replica_seed(SEED, rank)
-    t_setup = time.perf_counter()
-    thp0 = _meminfo_kb("AnonHugePages")
-    arena = binding.Mori.mori_host_alloc(cfg.cpu_pool_pages * sh.page_bytes)
-    arena_thp_gib = (_meminfo_kb("AnonHugePages") - thp0) / (1 << 20)
-    link = measure_link_peak(arena, stream_chunks=16)
+    page_b = sh.page_bytes
+    hbm_peak, peak_src = _hbm_peak()
     paths = {"auto": 0, "zerocopy": 1, "staged": 2, "copyengine": 3}
     r = GpuRunner(cfg, seed, arena=arena, staging_bytes=args.staging_mib << 20,
                   path_demote=paths[args.path_demote], path_promote=paths[args.path_promote],
                   copy_kernel={"auto": 0, "ldst": 1, "tma": 2}[args.kernel])
-    kernel_name = binding.KERNEL_NAMES[r.mori.copy_kernel]
     sim = W.Sim(cfg, seed)
-    t_setup = time.perf_counter() - t_setup
     cur = torch.cuda.current_stream()
-    page_b = sh.page_bytes
+    sticky = args.policy == "sticky"
 
     def ev():
         return torch.cuda.Event(enable_timing=True)
-
-    sticky = args.policy == "sticky"
 
     def epoch(mode):
         """One step.  mode 'dev': inputs resident, regions A+B timed; 'e2e': host buffers, one
@@ -375,132 +454,214 @@ def run_ours(args):
                     h2d=plan.promote_pages * page_b + 9 * n + n_tab,
                     d2h=plan.demote_pages * page_b + r.h_out.numel())
 
+    for _ in range(warmup):
+        epoch("dev")
+    # ---- timed: K steps, device-resident inputs ---------------------------------------------------
+    r.mori.mori_profile(True)
+    r.mori.mori_profile_read(binding.DEMOTE); r.mori.mori_profile_read(binding.PROMOTE)
+    clocks = ClockSampler(local) if clocks_on else None
+    barrier()
+    if clocks:
+        clocks.start()
+    l0 = r.mori.mori_launch_count()
+    st = [epoch("dev") for _ in range(steps)]
+    barrier()
+    launches = r.mori.mori_launch_count() - l0
+    clk = clocks.stop() if clocks else None
+    prof = {"demote": r.mori.mori_profile_read(binding.DEMOTE),
+            "promote": r.mori.mori_profile_read(binding.PROMOTE)}
+    r.mori.mori_profile(False)
+    if args.verbose:
+        for i, x in enumerate(st):
+            gb = (x["dem"] + x["pro"]) / 1e9
+            print(f"{cfg.name} step {i}: {x['ms']:.3f} ms  demote {x['dem'] / GIB:.2f} GiB  promote {x['pro'] / GIB:.2f} GiB  "
+                  f"{gb / (x['ms'] * 1e-3) if x['ms'] > 0 else 0:.1f} GB/s  ops {x['ops']}", file=sys.stderr)
+    # ---- timed: the SAME epochs again through the public API from host buffers (the trace and the
+    #      placement are deterministic in the seed, so `e2e` and `value` move identical bytes) -------
+    st_e2e = []
+    if do_e2e:
+        sim = W.Sim(cfg, seed)
+        for _ in range(warmup):
+            epoch("e2e")
+        barrier()
+        st_e2e = [epoch("e2e") for _ in range(steps)]
+        barrier()
+
+    def total(x, k):
+        return float(sum(s_[k] for s_ in x))
+
+    out = {"cfg": cfg, "runner_paths": r.mori_paths, "kernel_name": binding.KERNEL_NAMES[r.mori.copy_kernel],
+           "steps": st, "steps_e2e": st_e2e, "launches": launches, "clocks": clk,
+           "t_dev": total(st, "ms") * 1e-3, "b_dev": total(st, "dem") + total(st, "pro"),
+           "t_e2e": total(st_e2e, "ms") * 1e-3, "b_e2e": total(st_e2e, "dem") + total(st_e2e, "pro"),
+           "h2d_per_step": total(st_e2e, "h2d") / max(1, len(st_e2e)),
+           "d2h_per_step": total(st_e2e, "d2h") / max(1, len(st_e2e))}
+
+    # ---- size-matched peak (SURVEY 8d): a plain pinned memcpy of ONE epoch's mean bytes; for GiB-
+    #      sized epochs it equals the asymptotic peak, for cfg 1's KiB-sized ones it is what
+    #      "latency-bound" means on this link ---------------------------------------------------------
+    moving = [x for x in st if x["dem"] + x["pro"] > 0]
+    out["moving_steps"] = len(moving)
+    out["size_matched"] = None
+    if moving and size_matched_leg:
+        mean_b = int(sum(x["dem"] + x["pro"] for x in moving) / len(moving))
+        mean_b = max(4096, min(mean_b, arena.numel() // 2, 2 * GIB)) // 4096 * 4096
+        sm = measure_link_peak(arena, nbytes=mean_b, reps=10)
+        ach = sum(x["dem"] + x["pro"] for x in moving) / (sum(x["ms"] for x in moving) * 1e-3) / 1e9
+        out["size_matched"] = {"bytes": mean_b, "d2h_GBps": sm["d2h"], "h2d_GBps": sm["h2d"],
+                               "epochs_GBps": ach, "epochs_over_d2h": ach / sm["d2h"],
+                               "note": "one-direction denominator: epochs that move both ways can exceed it"}
+
+    # ---- roofline of the HBM-bound kernel, from the library's per-launch CUDA events ---------------
+    ncu = _load_ncu_traffic()
+    k_ms = prof["demote"][0] + prof["promote"][0]
+    k_n = prof["demote"][1] + prof["promote"][1]
+    k_b = prof["demote"][2] + prof["promote"][2]
+    staged_bytes = sum(x["dem"] + x["pro"] for x in st)
+    roofline = None
+    if binding.PATH_STAGED in r.mori_paths and k_ms > 0 and k_b >= 0.5 * staged_bytes and k_b / k_n > (64 << 20):
+        ach = 2.0 * k_b / (k_ms * 1e-3) / 1e9                     # read + write, per DESIGN.md 5
+        roofline = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                    "traffic": ncu.get("dram_bytes_per_launch"),
+                    "kernel": f"copy_pages_{binding.KERNEL_NAMES[r.mori.copy_kernel]}"
+                              " (gather/scatter of the STAGED path, inside the timed steps)",
+                    "peak_source": peak_src, "traffic_source": ncu.get("source"),
+                    "traffic_launch_algorithmic_bytes": ncu.get("algorithmic_bytes_same_launch"),
+                    "traffic_over_algorithmic_same_launch": ncu.get("ratio"),
+                    "launches": k_n, "avg_launch_us": 1e3 * k_ms / k_n,
+                    "algorithmic_bytes_per_launch": 2.0 * k_b / k_n}
+    out["roofline"] = roofline
+    # ---- the device halves alone: pool <-> contiguous device buffer, >= 4 GiB per launch ------------
+    out["gather_scatter"] = gather_scatter_leg(r, sim, hbm_peak, reps=gather_reps) if gather_reps > 0 else None
+    out["free_gpu_pages"] = max(0, cfg.cap_gpu_pages - int(sum(p_.size for p_ in sim.gpu_pages)))
+    out["runner"] = r
+    return out
+
+
+def _per_config_record(m, link, scale):
+    """The compact per-config sub-record of the bench line (north_star: "reported per config as an
+    absolute number and as a fraction of the measured pinned-memcpy host-link peak")."""
+    cfg = m["cfg"]
+    sh = cfg.shape
+    lr = link_report(m["steps"], link)
+    rec = {"workload": cfg.name, "bj_config": f"configs[{cfg.index - 1}]", "scale": scale, "f_busy": cfg.f_busy,
+           "GBps": m["b_dev"] / m["t_dev"] / 1e9 if m["t_dev"] > 0 else 0.0,
+           "frac_of_measured_link_peak": lr["frac_of_measured_link_peak"],
+           "frac_of_pinned_memcpy_model": lr["frac_of_pinned_memcpy_model"],
+           "e2e_GBps": m["b_e2e"] / m["t_e2e"] / 1e9 if m["t_e2e"] > 0 else None,
+           "steps": len(m["steps"]), "moving_steps": m["moving_steps"], "migrated_GiB": m["b_dev"] / GIB,
+           "ms_per_step": 1e3 * m["t_dev"] / max(1, len(m["steps"])),
+           "ranker_capacity_pages": {"gpu": cfg.cap_gpu_pages, "cpu": cfg.cap_cpu_pages,
+                                     "gpu_GiB": cfg.cap_gpu_pages * sh.page_bytes / GIB,
+                                     "note": "physical pool minus headroom (DESIGN.md R23)"},
+           "pools_GiB": {"gpu": cfg.gpu_pool_pages * sh.page_bytes / GIB, "cpu": cfg.cpu_pool_pages * sh.page_bytes / GIB},
+           "paths": [PATH_NAME.get(x, str(x)) for x in m["runner_paths"]], "gpu_launches": int(m["launches"])}
+    for k in ("demote_only", "promote_only", "bidirectional"):
+        if k in lr:
+            rec[k] = {"steps": lr[k]["steps"], "GBps": lr[k]["GBps"], "frac": lr[k]["frac"]}
+    if m["size_matched"]:
+        smx = m["size_matched"]
+        rec["size_matched"] = {"bytes": smx["bytes"], "pinned_memcpy_GBps": smx["d2h_GBps"],
+                               "epochs_GBps": smx["epochs_GBps"], "frac": smx["epochs_over_d2h"]}
+    if m["roofline"]:
+        rec["in_step_gather_scatter_frac_of_measured_hbm"] = m["roofline"]["frac"]
+        rec["in_step_launches"] = m["roofline"]["launches"]
+    gs = m["gather_scatter"]
+    if gs:
+        rec["standalone_gather_frac_of_measured_hbm"] = gs["gather_frac_of_measured_hbm"]
+        rec["standalone_scatter_frac_of_measured_hbm"] = gs["scatter_frac_of_measured_hbm"]
+        rec["standalone_GiB_per_launch"] = gs["GiB_per_launch"]
+    return rec
+
+
+PATH_NAME = {1: "zerocopy", 2: "staged", 3: "copyengine"}
+
+
+def _fit_scale(cfg_index: int, world: int, W, f_busy=None) -> int:
+    """SURVEY 8(d) scale rule: the smallest power of two that lets the pinned arena fit host RAM and
+    the pool fit HBM.  One replica: the arena plus 20 GiB must fit MemAvailable (cfg 3's 160 GiB does
+    on a 196 GiB box, cfg 4's 200 GiB does not).  Several replicas share the node: 70 % of MemTotal
+    divided by the ranks (MemTotal so that every rank picks the same scale)."""
+    import torch
+    if world > 1:
+        avail = int(_meminfo_kb("MemTotal") * 1024 * 0.70) // world
+    else:
+        avail = _meminfo_kb("MemAvailable") * 1024 - 20 * GIB
+    free_hbm, _ = torch.cuda.mem_get_info()
+    scale = 1
+    while True:
+        cfg = W.get_config(cfg_index, scale, f_busy)
+        sh = cfg.shape
+        if (cfg.cpu_pool_pages * sh.page_bytes <= avail
+                and cfg.gpu_pool_pages * sh.page_bytes + (5 << 30) <= free_hbm):
+            return scale
+        scale *= 2
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_00866_b200 import binding, replicas, workload as W
+
+    rank, world, local = replicas.env_rank()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    if args.device_index >= 0:
+        local = args.device_index                    # testing only: several replicas on one GPU
+    torch.cuda.set_device(local)
+    if world > 1:
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(args.backend)
+
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        epoch("dev")
-    # ---- timed: K steps, device-resident inputs ---------------------------------------------------
-    r.mori.mori_profile(True)
-    r.mori.mori_profile_read(binding.DEMOTE); r.mori.mori_profile_read(binding.PROMOTE)
-    clocks = ClockSampler(local)
-    barrier()
-    clocks.start()
-    l0 = r.mori.mori_launch_count()
-    steps = [epoch("dev") for _ in range(args.steps)]
-    barrier()
-    if args.verbose and rank == 0:
-        for i, st in enumerate(steps):
-            gb = (st["dem"] + st["pro"]) / 1e9
-            print(f"step {i}: {st['ms']:.2f} ms  demote {st['dem'] / GIB:.2f} GiB  promote {st['pro'] / GIB:.2f} GiB  "
-                  f"{gb / (st['ms'] * 1e-3) if st['ms'] > 0 else 0:.1f} GB/s  ops {st['ops']}", file=sys.stderr)
-    launches = r.mori.mori_launch_count() - l0
-    clk = clocks.stop()
-    prof = {"demote": r.mori.mori_profile_read(binding.DEMOTE),
-            "promote": r.mori.mori_profile_read(binding.PROMOTE)}
-    r.mori.mori_profile(False)
-    # ---- timed: K steps through the public API from host buffers -----------------------------------
-    # the SAME epochs again (the trace and the placement are deterministic in the seed), so that
-    # `e2e` and `value` move identical bytes: fresh Sim, W untimed epochs, then K timed ones
-    sim = W.Sim(cfg, seed)
-    for _ in range(args.warmup):
-        epoch("e2e")
-    barrier()
-    steps_e2e = [epoch("e2e") for _ in range(args.steps)]
-    barrier()
+    # ---- which configs run: the headline one (BASELINE.json configs[1] unless --config), then, on a
+    #      default single-GPU run, every other config of BASELINE.json as a `per_config` sub-record ----
+    scale = args.scale or _fit_scale(args.config, world, W, args.f_busy)
+    cfg = W.get_config(args.config, scale, args.f_busy)
+    others = []
+    if args.per_config and world == 1 and rank == 0:
+        for idx, fb in ((1, None), (3, 0.25), (3, 0.5), (3, 0.75), (4, None), (5, None), (2, None)):
+            if idx == args.config and (fb == args.f_busy or idx != 3):
+                continue
+            others.append((idx, fb, 1 if idx == 1 else _fit_scale(idx, world, W, fb)))
+    sh = cfg.shape
+    seed = replicas.replica_seed(SEED, rank)
+    t_setup = time.perf_counter()
+    thp0 = _meminfo_kb("AnonHugePages")
+    arena_bytes = max([cfg.cpu_pool_pages * sh.page_bytes] +
+                      [W.get_config(i, sc, fb).cpu_pool_pages * W.get_config(i, sc, fb).shape.page_bytes
+                       for i, fb, sc in others])
+    arena_full = binding.Mori.mori_host_alloc(arena_bytes)          # ONE pinned arena serves every config
+    arena_thp_gib = (_meminfo_kb("AnonHugePages") - thp0) / (1 << 20)
+    link = measure_link_peak(arena_full, stream_chunks=16)
+    t_setup = time.perf_counter() - t_setup
+    hbm_peak, peak_src = _hbm_peak()
+    page_b = sh.page_bytes
 
-    def total(st, k):
-        return float(sum(s[k] for s in st))
-
-    t_dev, t_e2e = total(steps, "ms") * 1e-3, total(steps_e2e, "ms") * 1e-3
-    b_dev = total(steps, "dem") + total(steps, "pro")
-    b_e2e = total(steps_e2e, "dem") + total(steps_e2e, "pro")
+    m = measure_config(args, cfg, seed, arena_full[:cfg.cpu_pool_pages * page_b], link, args.steps, args.warmup,
+                       local, barrier, do_e2e=True, gather_reps=0 if (args.no_gather_leg or rank != 0) else 20)
+    r = m["runner"]
     (t_dev, t_e2e), (b_dev, b_e2e, launches) = replicas.aggregate(
-        [t_dev, t_e2e], [b_dev, b_e2e, float(launches)], device="cuda")
+        [m["t_dev"], m["t_e2e"]], [m["b_dev"], m["b_e2e"], float(m["launches"])], device="cuda")
     value = b_dev / t_dev / 1e9 if t_dev > 0 else 0.0
     value_e2e = b_e2e / t_e2e / 1e9 if t_e2e > 0 else 0.0
-
-    # ---- size-matched peak (SURVEY 8d): a plain pinned memcpy of ONE epoch's mean bytes; for GiB-
-    #      sized epochs it equals the asymptotic peak, for cfg 1's KiB-sized ones it is what
-    #      "latency-bound" means on this link ---------------------------------------------------------
-    moving = [s for s in steps if s["dem"] + s["pro"] > 0]
-    size_matched = None
-    if moving and rank == 0:
-        mean_b = int(sum(s["dem"] + s["pro"] for s in moving) / len(moving))
-        mean_b = max(4096, min(mean_b, arena.numel() // 2, 2 * GIB)) // 4096 * 4096
-        sm = measure_link_peak(arena, nbytes=mean_b, reps=10)
-        ach = sum(s["dem"] + s["pro"] for s in moving) / (sum(s["ms"] for s in moving) * 1e-3) / 1e9
-        size_matched = {"bytes": mean_b, "d2h_GBps": sm["d2h"], "h2d_GBps": sm["h2d"],
-                        "epochs_GBps": ach, "epochs_over_d2h": ach / sm["d2h"],
-                        "note": "one-direction denominator: epochs that move both ways can exceed it"}
-
-    # ---- link fractions (rank 0's own steps against rank 0's own measured peaks) -------------------
-    def link_report(st):
-        ideal = sum(ideal_seconds(s["dem"], s["pro"], link) for s in st)
-        meas = sum(s["ms"] for s in st) * 1e-3
-        model = sum(memcpy_model_seconds(s["dem"], s["pro"], link) for s in st)
-        out = {"frac_of_measured_link_peak": ideal / meas if meas > 0 else None,
-               "frac_of_pinned_memcpy_model": model / meas if meas > 0 else None}
-        if "d2h_streamed" in link and meas > 0:      # the same bound from the streamed (sustained) rates
-            sl = dict(link, d2h=link["d2h_streamed"], h2d=link["h2d_streamed"])
-            out["frac_of_streamed_link_rate"] = sum(ideal_seconds(s["dem"], s["pro"], sl) for s in st) / meas
-        for name, sel in (("demote_only", lambda s: s["dem"] > 0 and s["pro"] == 0),
-                          ("promote_only", lambda s: s["pro"] > 0 and s["dem"] == 0),
-                          ("bidirectional", lambda s: s["pro"] > 0 and s["dem"] > 0)):
-            sub = [s for s in st if sel(s)]
-            if sub:
-                byt = sum(s["dem"] + s["pro"] for s in sub)
-                sec = sum(s["ms"] for s in sub) * 1e-3
-                peak = {"demote_only": link["d2h"], "promote_only": link["h2d"]}.get(name)
-                ent = {"steps": len(sub), "GBps": byt / sec / 1e9, "GiB": byt / GIB}
-                ent["frac"] = (ent["GBps"] / peak) if peak else \
-                    sum(ideal_seconds(s["dem"], s["pro"], link) for s in sub) / sec
-                if not peak:
-                    ent["frac_of_pinned_memcpy_model"] = \
-                        sum(memcpy_model_seconds(s["dem"], s["pro"], link) for s in sub) / sec
-                out[name] = ent
-        return out
-
-    # ---- roofline of the HBM-bound kernel, from the library's per-launch CUDA events ---------------
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        hbm_peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
-    else:
-        hbm_peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-    k_ms = prof["demote"][0] + prof["promote"][0]
-    k_n = prof["demote"][1] + prof["promote"][1]
-    k_b = prof["demote"][2] + prof["promote"][2]
-    staged = binding.PATH_STAGED in r.mori_paths
-    roofline = None
-    if staged and k_ms > 0:
-        ach = 2.0 * k_b / (k_ms * 1e-3) / 1e9                     # read + write, per DESIGN.md 5
-        roofline = {"bound": "hbm", "kernel": f"copy_pages_{binding.KERNEL_NAMES[r.mori.copy_kernel]}"
-                                              " (gather/scatter of the STAGED path, inside the timed steps)",
-                    "achieved": ach, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s",
-                    "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC.get("bytes_per_launch"),
-                    "traffic_source": NCU_TRAFFIC.get("source"),
-                    "traffic_over_algorithmic_same_launch": NCU_TRAFFIC.get("ratio"),
-                    "launches": k_n, "avg_launch_us": 1e3 * k_ms / k_n,
-                    "algorithmic_bytes_per_launch": 2.0 * k_b / k_n}
-
-    # ---- the device halves alone: pool <-> contiguous device buffer, >= 4 GiB per launch ------------
-    gs = None
-    if rank == 0 and not args.no_gather_leg:
-        gs = gather_scatter_leg(r, sim, hbm_peak)
-        if roofline is None and gs:
-            roofline = {"bound": "hbm", "kernel": gs["kernel"] + " (standalone gather launches)",
-                        "achieved": gs["gather_GBps"], "peak": hbm_peak, "peak_source": peak_src,
-                        "unit": "GB/s", "frac": gs["gather_GBps"] / hbm_peak,
-                        "traffic": NCU_TRAFFIC.get("bytes_per_launch"),
-                        "traffic_source": NCU_TRAFFIC.get("source")}
+    roofline, gs = m["roofline"], m["gather_scatter"]
+    if roofline is None and gs:
+        ncu = _load_ncu_traffic()
+        roofline = {"bound": "hbm", "achieved": gs["gather_GBps"], "peak": hbm_peak, "unit": "GB/s",
+                    "frac": gs["gather_GBps"] / hbm_peak, "traffic": ncu.get("dram_bytes_per_launch"),
+                    "kernel": gs["kernel"] + " (standalone gather launches)", "peak_source": peak_src,
+                    "traffic_source": ncu.get("source")}
 
     # ---- the shared Waiting queue across replicas: all-gather every replica's
     #      free GPU pages (NCCL; stays on the device) and pack the same queue on every rank ---------
-    free_all = replicas.gather_free_capacity(max(0, cfg.cap_gpu_pages - int(sum(p.size for p in sim.gpu_pages))),
-                                             device="cuda")
+    free_all = replicas.gather_free_capacity(m["free_gpu_pages"], device="cuda")
     wq_rng = np.random.default_rng(SEED)                             # one queue, identical on every rank
     wq_n = cfg.n_programs                                            # (the context is sized for n programs)
     wq = [torch.from_numpy(x).cuda() for x in (
@@ -514,38 +675,82 @@ def run_ours(args):
                      "admitted_here": int((wq_rep == rank).sum().item()),
                      "admitted_total": int((wq_rep >= 0).sum().item()), "free_pages_left": wq_left.tolist()}
     r.close()
-    rp = rank_partition_leg(with_oracle=(world == 1 and not args.no_cpu_baseline)) if rank == 0 else None
-    evl = eviction_leg(with_oracle=(world == 1 and not args.no_cpu_baseline)) if rank == 0 else None
+    m["runner"] = None
+    del r
+    torch.cuda.empty_cache()
+
+    # ---- every other BASELINE.json config, driver-timed in the same run (single GPU only) ----------
+    per_config = [_per_config_record(m, link, scale)]
+    for idx, fb, sc in others:
+        t0 = time.perf_counter()
+        try:
+            c2 = W.get_config(idx, sc, fb)
+            m2 = measure_config(args, c2, seed, arena_full[:c2.cpu_pool_pages * c2.shape.page_bytes], link,
+                                args.per_config_steps if idx != 1 else c2.epochs - 4, 4, local, barrier,
+                                do_e2e=(idx == 1), gather_reps=0 if (args.no_gather_leg or idx == 1) else 5,
+                                clocks_on=False)
+            m2["runner"].close()
+            m2["runner"] = None
+            rec = _per_config_record(m2, link, sc)
+            rec["leg_seconds"] = time.perf_counter() - t0
+            per_config.append(rec)
+            del m2
+        except Exception as e:                                       # a failed side leg must not lose the headline
+            per_config.append({"workload": f"cfg{idx}" + (f"-f{fb:g}" if fb else ""), "scale": sc,
+                               "error": f"{type(e).__name__}: {e}"})
+        torch.cuda.empty_cache()
+    per_config.sort(key=lambda x: x.get("workload", ""))
+    binding.Mori.mori_host_free(arena_full)
+
+    with_oracle = world == 1 and not args.no_cpu_baseline
+    rp = rank_partition_leg(with_oracle=with_oracle) if rank == 0 else None
+    evl = eviction_leg(with_oracle=with_oracle) if rank == 0 else None
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = cpu_baseline(args.config)
+    if rank == 0 and with_oracle:
+        cpu = cpu_baseline(args.config, f_busy=args.f_busy)
+        if args.per_config:
+            cpu["per_config"] = []
+            for idx, fb, sc in others:
+                try:
+                    cb = cpu_baseline(idx, budget_s=2.0, f_busy=fb, max_bytes=6 * GIB)
+                    cpu["per_config"].append({"workload": cb["workload"], "scale": cb["scale"], "GBps_1_core": cb["value"],
+                                              "GBps_all_cores": cb["all_cores"]["value"], "cores": cb["all_cores"]["cores"]})
+                except Exception as e:
+                    cpu["per_config"].append({"workload": f"cfg{idx}", "error": f"{type(e).__name__}: {e}"})
     if rank == 0:
         K = args.steps
+        lr = link_report(m["steps"], link)
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+            "metric": METRIC, "value": value, "unit": UNIT,
+            "frac_of_measured_link_peak": lr["frac_of_measured_link_peak"],
+            "roofline_frac": roofline["frac"] if roofline else None,
+            "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": 1e3 * t_dev / K, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": cfg.name, "bj_config": f"configs[{args.config - 1}]", "scale": scale,
                        "n_programs": cfg.n_programs, "gpu_pool_GiB": cfg.gpu_pool_pages * page_b / GIB,
                        "host_arena_GiB": cfg.cpu_pool_pages * page_b / GIB,
+                       "ranker_gpu_capacity_GiB": cfg.cap_gpu_pages * page_b / GIB,
+                       "ranker_cpu_capacity_GiB": cfg.cap_cpu_pages * page_b / GIB,
                        "page_bytes": page_b, "chunk_bytes": sh.chunk_bytes,
                        "parallelism": f"replicas x{world} (no data-path collective)",
-                       "path_demote": binding.PATH_NAMES[r.mori_paths[0]],
-                       "path_promote": binding.PATH_NAMES[r.mori_paths[1]],
-                       "copy_kernel": kernel_name,
+                       "path_demote": binding.PATH_NAMES[m["runner_paths"][0]],
+                       "path_promote": binding.PATH_NAMES[m["runner_paths"][1]],
+                       "copy_kernel": m["kernel_name"],
                        "staging_MiB": args.staging_mib, "policy": args.policy,
                        "l2": "inputs larger than L2 (GiB per step vs 126 MB); no flush needed",
                        "migrated_GiB": b_dev / GIB, "setup_s": t_setup,
                        "host_arena_on_huge_pages_GiB": arena_thp_gib},
-            "clocks": clk,
+            "clocks": m["clocks"],
             "e2e": {"value": value_e2e, "unit": UNIT,
-                    "h2d_bytes_per_step": total(steps_e2e, "h2d") / K,
-                    "d2h_bytes_per_step": total(steps_e2e, "d2h") / K,
+                    "h2d_bytes_per_step": m["h2d_per_step"],
+                    "d2h_bytes_per_step": m["d2h_per_step"],
                     "ms_per_step": 1e3 * t_e2e / K, "migrated_GiB": b_e2e / GIB,
-                    "link": link_report(steps_e2e)},
+                    "link": link_report(m["steps_e2e"], link)},
             "gpu_launches": int(launches),
             "roofline": roofline,
-            "link": dict(link_report(steps), peaks_GBps=link, size_matched=size_matched,
+            "per_config": per_config,
+            "link": dict(lr, peaks_GBps=link, size_matched=m["size_matched"],
                          peak_how="pinned cudaMemcpyAsync of one contiguous 1 GiB buffer, best of 5, "
                                   "measured in this process before the run"),
             "gather_scatter": gs,
@@ -555,20 +760,9 @@ def run_ours(args):
             "cpu_baseline": cpu,
         }
         print(json.dumps(line))
-    binding.Mori.mori_host_free(arena)
     if world > 1:
         dist.barrier()                      # rank 0 is still running its single-rank legs
         dist.destroy_process_group()
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the gather kernel from the committed
-# ncu --set full capture (profiles/); filled in once that capture exists.
-NCU_TRAFFIC: dict = {
-    "bytes_per_launch": 1780.91e6,              # dram__bytes_read.sum 914.38 MB + write 866.52 MB
-    "algorithmic_bytes_same_launch": 1828.72e6,  # that launch gathered 436 pages of 2 MiB, x2
-    "ratio": 0.974,
-    "source": "profiles/r1_gather_ncu_full.md, launch 4 (ncu --set full, one in-step gather launch)",
-}
 
 
 def gather_scatter_leg(r, sim, hbm_peak, min_bytes=4 * GIB, reps=20, warm=3):
@@ -781,6 +975,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based")
     ap.add_argument("--scale", type=int, default=0, help="0 = auto (1 when the pools fit)")
+    ap.add_argument("--f-busy", type=float, default=None,
+                    help="stationary busy fraction of the trace (cfg 3 sweeps 0.25 / 0.5 / 0.75; default: the config's)")
+    ap.add_argument("--no-per-config", dest="per_config", action="store_false",
+                    help="skip the per_config legs (every other BASELINE.json config after the headline one)")
+    ap.add_argument("--per-config-steps", type=int, default=8, help="timed epochs of each per_config leg")
+    ap.add_argument("--ref-threads", type=int, default=1, help="--impl reference: host threads of the oracle's movers")
     ap.add_argument("--path-demote", default="auto", choices=["auto", "zerocopy", "staged", "copyengine"])
     ap.add_argument("--path-promote", default="auto", choices=["auto", "zerocopy", "staged", "copyengine"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "ldst", "tma"])

@@ -16,6 +16,13 @@
  *   - The caller owns the pool, the arena, the page allocator and every array it passes in;
  *     the library owns the context, its streams, events, staging and index buffers.
  *   - One context per GPU; calls on one context must come from one host thread at a time.
+ *   - The placement entry points (mori_rank_partition, mori_rank_partition_tiers,
+ *     mori_sticky_rebalance, mori_bfd_assign, mori_eviction_order, mori_idleness_*) take a caller
+ *     stream and share per-context scratch (last-CTA tickets, order buffers, the eviction sort's
+ *     tables): enqueue them on ONE stream at a time; if two streams are used, the caller orders
+ *     them (event or join) so that two such launches are never in flight together.
+ *   - MORI_DEBUG=1 in the environment of mori_create turns on validation that release builds
+ *     leave to the caller: duplicate destination ids (see mori_demote / mori_scatter_pages).
  *   - There is no CPU fallback: without a usable sm_100a device mori_create fails.
  *
  * Layouts (BASELINE.json north_star; the paper only says the cache is paged)
@@ -139,13 +146,18 @@ int mori_rank_partition(mori_ctx* ctx, void* stream, int32_t n, const float* idl
  * (host_slots[j], l) of the arena.  Asynchronous, on the context's demote stream(s).
  *
  *   gpu_pages, host_slots  HOST int32[total_pages]; ids out of range -> MORI_ERR_INVALID_ARG.
- *                          Duplicate destination slots are undefined behaviour.
- *   wait_promote_ticket    0, or a ticket returned by mori_promote: no byte of this call is
- *                          written before that promote call has completed (device-side wait).
+ *                          A destination slot listed twice in one call is undefined behaviour
+ *                          (two copies race for the same bytes); with MORI_DEBUG=1 in the
+ *                          environment of mori_create it is found on the host before anything is
+ *                          enqueued -> MORI_ERR_INVALID_ARG.
+ *   wait_promote_ticket    0, or a ticket returned by mori_promote: no byte of this call is read
+ *                          or written before that promote call has completed (device-side wait).
  *   ticket_out             NULL, or receives this call's ticket (> 0, increasing).
  * total_pages == 0 is a valid no-op that still yields a ticket.
  * Calls of one direction take effect in issue order (a later call that writes the same slots or
- * pages wins), whichever path each of them takes; the two directions are ordered only by tickets.
+ * pages wins), whichever path each of them takes; the two directions are ordered only by tickets,
+ * and a ticket means the same on every path (ZEROCOPY, STAGED, COPYENGINE, the one-launch path of
+ * a small call): what it names has completed before what it gates starts.
  */
 int mori_demote(mori_ctx* ctx, int64_t total_pages, const int32_t* gpu_pages,
                 const int32_t* host_slots, int64_t wait_promote_ticket, int64_t* ticket_out);
@@ -153,11 +165,18 @@ int mori_demote(mori_ctx* ctx, int64_t total_pages, const int32_t* gpu_pages,
 /*
  * Step a6, promotion ("CPU-to-GPU transfer over PCIe"): the mirror image,
  * arena (host_slots[j], l) -> pool (l, gpu_pages[j]), on the promote stream(s), concurrently
- * with demotions.  wait_demote_ticket orders the pool writes after the demotion that vacated
- * the destination pages (the host->device DMA of a STAGED promote may start earlier).
+ * with demotions.  A promotion touches two resources that a demotion may still be using, so it
+ * takes two tickets of mori_demote (0 = none):
+ *   pages_after_demote   no byte of the POOL is written before that demotion has completed (the
+ *                        demotion that vacates the destination pages);
+ *   slots_after_demote   no byte of the ARENA is read before that demotion has completed (a
+ *                        demotion that wrote the source slots and has not been joined since).
+ * Keeping them apart is what lets a STAGED promotion stream its bytes over the link while the
+ * pages it will land in are still being vacated.  Duplicate destination PAGES: as for mori_demote.
  */
 int mori_promote(mori_ctx* ctx, int64_t total_pages, const int32_t* host_slots,
-                 const int32_t* gpu_pages, int64_t wait_demote_ticket, int64_t* ticket_out);
+                 const int32_t* gpu_pages, int64_t pages_after_demote, int64_t slots_after_demote,
+                 int64_t* ticket_out);
 
 /* Step a7: block the host until every demote (1), promote (2) or both (3) call has finished;
  * returns the first asynchronous error if there was one. */
@@ -175,6 +194,9 @@ int mori_stream_wait(mori_ctx* ctx, void* stream, int32_t which);
  * The on-device halves of the STAGED paths, exposed because they are what the HBM roofline is
  * measured on: pool pages <-> a contiguous DEVICE buffer laid out [n_pages][n_layers][chunk].
  * gpu_pages is a DEVICE int32[n_pages].  One launch on `stream`; asynchronous.
+ * Ids are device data and are not checked in release.  With MORI_DEBUG=1 a validation kernel
+ * runs first on `stream` and the call waits for it (range; for scatter also duplicate pages):
+ * a bad table -> MORI_ERR_INVALID_ARG with nothing else enqueued.
  */
 int mori_gather_pages(mori_ctx* ctx, void* stream, int64_t n_pages, const int32_t* gpu_pages,
                       void* dst);

@@ -74,7 +74,7 @@ def load():
         L.mori_idleness_update.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         L.mori_idleness_eval.argtypes = [vp, vp, i32, vp, vp, vp]
         L.mori_demote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
-        L.mori_promote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
+        L.mori_promote.argtypes = [vp, i64, vp, vp, i64, i64, C.POINTER(i64)]
         L.mori_sync.argtypes = [vp, i32]
         L.mori_after_stream.argtypes = [vp, i32, vp]
         L.mori_stream_wait.argtypes = [vp, vp, i32]
@@ -252,12 +252,12 @@ class Mori:
                                        int(wait_promote_ticket), C.byref(t)))
         return t.value
 
-    def mori_promote(self, host_slots, gpu_pages, wait_demote_ticket=0) -> int:
+    def mori_promote(self, host_slots, gpu_pages, pages_after_demote=0, slots_after_demote=0) -> int:
         g, h = _host_i32(gpu_pages), _host_i32(host_slots)
         assert g.shape == h.shape and g.ndim == 1
         t = C.c_int64(0)
         self._ck(self._lib.mori_promote(self._h, g.size, h.ctypes.data, g.ctypes.data,
-                                        int(wait_demote_ticket), C.byref(t)))
+                                        int(pages_after_demote), int(slots_after_demote), C.byref(t)))
         return t.value
 
     def mori_sync(self, which=BOTH):

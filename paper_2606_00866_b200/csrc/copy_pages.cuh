@@ -13,16 +13,21 @@
 // of <= piece_bytes inside one chunk, contiguous on BOTH sides (the bulk-copy kernel uses whole
 // 64 KiB chunks as pieces; the LD/ST kernel 16 KiB).
 //
-// Two implementations:
+// Three implementations:
 //   copy_pages_tma   two threads per CTA drive the SM's bulk-copy engine: a loader issues
-//                    cp.async.bulk global->shared (mbarrier complete_tx) into a ring of stages,
-//                    a storer issues cp.async.bulk shared->global (bulk_group) and hands stages
-//                    back.  No registers, no LSU instructions per byte; up to 192 KiB of the
-//                    ring in flight per SM.
-//                    CTA b takes chunks b, b + grid, ...: one page-table load per chunk.
+//                    cp.async.bulk global->shared (mbarrier complete_tx) into a ring of stages
+//                    and publishes each stage's destination; a storer issues cp.async.bulk
+//                    shared->global (bulk_group) and hands stages back.  No registers, no LSU
+//                    instructions per byte; the rings of the CTAs resident on an SM take up to
+//                    192 KiB.  Chunks are handed out dynamically (one atomic per chunk, fetched
+//                    one chunk ahead) so that no SM idles while a slower one finishes a static
+//                    share; one page-table load per chunk.
 //   copy_pages_ldst  256 threads, 4 x 16-byte ld.global.nc.L1::no_allocate per thread issued
 //                    before the 4 st.global: 16 KiB in flight per CTA, 8 CTAs per SM; piece w
 //                    maps to (k, l, c) = (w / (L*ppc), (w / ppc) % L, w % ppc).
+//   copy_pages_small the LD/ST body with the page / slot ids passed BY VALUE in the kernel
+//                    parameters: a move of a few pages (cfg 1: KiBs per epoch) is one launch --
+//                    no index upload, no staging, no DMA -- straight to / from the mapped arena.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -42,6 +47,8 @@ struct CopyArgs {
   int pieces_per_chunk;       // ceil(chunk / piece)
   int stages;                 // bulk-copy kernel: ring depth (2 .. 24)
   int store_lag;              // bulk-copy kernel: 1 or 2 (< stages)
+  unsigned int* sched;        // bulk-copy kernel: [2] zeroed words (next chunk, CTAs done) for dynamic
+                              // chunk hand-out, or nullptr: CTA b takes chunks b, b + grid, ...
 };
 
 template <bool kGather>
@@ -177,66 +184,114 @@ __device__ __forceinline__ void chunk_addresses(const CopyArgs& a, long long w, 
 }
 
 // Shared memory: a.stages stage buffers of a.piece_bytes each, then a.stages "full" and a.stages
-// "empty" mbarriers.  Two single-thread roles so that neither waits for the other's latency:
-//   loader  (warp 0): for every piece, wait until its stage is empty, expect_tx + bulk load;
-//   storer  (warp 1): wait until the stage is full, bulk store, commit; once the store issued
-//                     `lag` groups ago has finished READING shared memory, hand its stage back
-//                     to the loader (lag = 2 on a deep ring, 1 on a ring of a few large stages).
-// CTA b takes chunks b, b + grid, ...; every CTA walks the same piece sequence in both roles.
+// "empty" mbarriers, then per stage the destination address and byte count the loader publishes.
+// Two single-thread roles so that neither waits for the other's latency:
+//   loader  (warp 0): takes the next chunk (statically b, b + grid, ..., or dynamically from
+//                     a.sched, fetched one chunk ahead so the atomic's latency is hidden); for
+//                     every piece: wait until its stage is empty, publish (dst, bytes),
+//                     expect_tx + bulk load.  After the last piece it publishes bytes = 0.
+//   storer  (warp 1): wait until the stage is full, bulk store to the published address, commit;
+//                     once the store issued `lag` groups ago has finished READING shared memory,
+//                     hand its stage back to the loader (lag = 2 on a deep ring, 1 on a ring of a
+//                     few large stages).  Stops at the bytes = 0 stage.
 // Stage index and mbarrier phase are carried incrementally (no division per piece).
 template <bool kGather>
-__global__ void __launch_bounds__(kTmaThreads, 1) copy_pages_tma(const CopyArgs a) {
+__global__ void __launch_bounds__(kTmaThreads) copy_pages_tma(const CopyArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int stages = a.stages;
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)stages * a.piece_bytes);
   uint64_t* empty = full + stages;
+  unsigned char** st_dst = reinterpret_cast<unsigned char**>(empty + stages);
+  uint32_t* st_bytes = reinterpret_cast<uint32_t*>(st_dst + stages);
   if (threadIdx.x == 0) {
     for (int s = 0; s < stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
   if ((threadIdx.x & 31) != 0) return;
-  const long long n_chunks = a.n_pages * a.n_layers;
-  const int ppc = a.pieces_per_chunk;
 
   if (threadIdx.x == 0) {
     // ---------------- loader ----------------
+    const long long n_chunks = a.n_pages * a.n_layers;
+    const int ppc = a.pieces_per_chunk;
+    unsigned int* sched = a.sched;
     int st = 0; uint32_t phase = 0; bool wrapped = false;          // phase of the NEXT wait on empty[st]
-    for (long long w = blockIdx.x; w < n_chunks; w += gridDim.x) {
+    long long w = blockIdx.x;
+    long long w_next = sched ? (long long)gridDim.x + atomicAdd(&sched[0], 1u) : w + gridDim.x;
+    while (w < n_chunks) {
       const unsigned char* src; unsigned char* dst;
       chunk_addresses<kGather>(a, w, src, dst);
       for (int c = 0; c < ppc; ++c) {
         const int off = c * a.piece_bytes;
         const uint32_t bytes = (uint32_t)min(a.piece_bytes, a.chunk_bytes - off);
         if (wrapped) mbar_wait(&empty[st], phase);
-        mbar_expect_tx(&full[st], bytes);
+        st_dst[st] = dst + off;
+        st_bytes[st] = bytes;
+        mbar_expect_tx(&full[st], bytes);                           // release: the storer sees (dst, bytes)
         bulk_g2s(smem + (size_t)st * a.piece_bytes, src + off, bytes, &full[st]);
         if (++st == stages) { st = 0; if (wrapped) phase ^= 1; wrapped = true; }
       }
+      w = w_next;
+      w_next = sched ? (long long)gridDim.x + atomicAdd(&sched[0], 1u) : w + gridDim.x;
     }
+    if (wrapped) mbar_wait(&empty[st], phase);
+    st_bytes[st] = 0;                                               // end marker for the storer
+    mbar_arrive(&full[st]);
+    // the last CTA to stop taking chunks re-arms the two words for the next launch that uses them
+    if (sched && atomicAdd(&sched[1], 1u) == gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
   } else {
     // ---------------- storer ----------------
     const int lag = a.store_lag;
     int st = 0; uint32_t phase = 0;                                 // stage / phase of the piece being stored
     int rel = 0; long long issued = 0;                              // next stage to hand back
-    for (long long w = blockIdx.x; w < n_chunks; w += gridDim.x) {
-      const unsigned char* src; unsigned char* dst;
-      chunk_addresses<kGather>(a, w, src, dst);
-      for (int c = 0; c < ppc; ++c) {
-        const int off = c * a.piece_bytes;
-        const uint32_t bytes = (uint32_t)min(a.piece_bytes, a.chunk_bytes - off);
-        mbar_wait(&full[st], phase);
-        bulk_s2g(dst + off, smem + (size_t)st * a.piece_bytes, bytes);
-        bulk_commit();
-        if (++st == stages) { st = 0; phase ^= 1; }
-        if (++issued > lag) {                                       // the group issued `lag` ago has left smem
-          if (lag == 1) bulk_wait_read<1>(); else bulk_wait_read<2>();
-          mbar_arrive(&empty[rel]);
-          if (++rel == stages) rel = 0;
-        }
+    for (;;) {
+      mbar_wait(&full[st], phase);
+      const uint32_t bytes = st_bytes[st];
+      if (bytes == 0) break;
+      bulk_s2g(st_dst[st], smem + (size_t)st * a.piece_bytes, bytes);
+      bulk_commit();
+      if (++st == stages) { st = 0; phase ^= 1; }
+      if (++issued > lag) {                                         // the group issued `lag` ago has left smem
+        if (lag == 1) bulk_wait_read<1>(); else bulk_wait_read<2>();
+        mbar_arrive(&empty[rel]);
+        if (++rel == stages) rel = 0;
       }
     }
     bulk_wait_all();   // writes complete before the CTA exits
+  }
+}
+
+// Shared-memory bytes of one copy_pages_tma CTA.
+__host__ __device__ inline size_t tma_smem_bytes(int stages, int piece_bytes) {
+  return (size_t)stages * piece_bytes + (size_t)stages * (2 * sizeof(uint64_t) + sizeof(void*) + sizeof(uint32_t));
+}
+
+// ------------------------------------------------------------------------------------------
+// Small moves: ids by value in the kernel parameters (no index upload), 4 KiB pieces so that even
+// a few pages spread over many SMs (the move is latency-bound: what matters is requests in
+// flight on the link, not per-SM efficiency).
+// ------------------------------------------------------------------------------------------
+constexpr int kSmallMaxPages = 448;
+constexpr int kSmallPiece = kLdstThreads * 16;
+struct SmallIds { int32_t gpu[kSmallMaxPages]; int32_t lin[kSmallMaxPages]; };
+
+template <bool kGather>
+__global__ void __launch_bounds__(kLdstThreads) copy_pages_small(const CopyArgs a, const SmallIds ids) {
+  const int ppc = a.pieces_per_chunk;                               // pieces of kSmallPiece bytes
+  const int per_page = a.n_layers * ppc;
+  const int n_pieces = (int)a.n_pages * per_page;
+  for (int w = blockIdx.x; w < n_pieces; w += gridDim.x) {
+    const int k = w / per_page, rem = w - k * per_page;
+    const int l = rem / ppc, c = rem - l * ppc;
+    const int off = c * kSmallPiece;
+    const unsigned char* pp = a.pool + ((long long)l * a.pool_pages + ids.gpu[k]) * a.chunk_bytes + off;
+    const unsigned char* lp = a.lin + ((long long)ids.lin[k] * a.n_layers + l) * a.chunk_bytes + off;
+    const int v = threadIdx.x;
+    if (v * 16 < a.chunk_bytes - off) {
+      const int4* s = reinterpret_cast<const int4*>(kGather ? pp : lp) + v;
+      int4* d = reinterpret_cast<int4*>(const_cast<unsigned char*>(kGather ? lp : pp)) + v;
+      st_stream(d, ld_stream(s));
+    }
   }
 }
 

@@ -9,6 +9,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <map>
 #include <mutex>
 #include <thread>
@@ -31,17 +32,26 @@ std::mutex g_host_mu;
 std::map<void*, std::pair<void*, size_t>> g_host_allocs;   // mori_host_alloc: aligned ptr -> (mmap base, length)
 
 constexpr int kTicketRing = 4096;
-constexpr int kRankTickets = 64;      // rank/partition launches that may be in flight at once
-#ifndef MORI_PIECE_BYTES
-#define MORI_PIECE_BYTES (64 * 1024)
-#endif
-#ifndef MORI_RING_BYTES
-#define MORI_RING_BYTES (192 * 1024)
-#endif
-constexpr int kPieceBytes = MORI_PIECE_BYTES;   // bytes per bulk copy = stage size (whole 64 KiB chunks)
-constexpr int kRingBytes = MORI_RING_BYTES;     // shared memory the ring of stages may take per CTA
+// Last-CTA tickets of the rankers and chunk counters of the copy kernel: one entry per launch,
+// taken round-robin and re-armed by the launch's own last CTA.  An entry is in use only while its
+// kernel is RESIDENT, and a device runs at most 128 grids at once, so 256 entries cannot collide.
+constexpr int kRankTickets = 256;
+constexpr int kSchedRing = 256;
+constexpr int kPieceBytesDefault = 64 * 1024;   // bytes per bulk copy = stage size (whole 64 KiB chunks)
+constexpr int kRingBytesDefault = 192 * 1024;   // shared memory the rings of one SM's CTAs may take
 constexpr int kMaxTmaStages = 24;
 constexpr long long kAutoMinRunBytes = 6LL << 20;   // AUTO: below this mean slot-run length, ZEROCOPY
+constexpr long long kSmallMaxBytes = 4LL << 20;     // calls up to this size (and kSmallMaxPages) take the one-launch path
+
+// Tuning overrides for experiments (read once per mori_create): MORI_PIECE_KIB, MORI_RING_KIB,
+// MORI_CTAS_PER_SM, MORI_SCHED (0 static, 1 dynamic), MORI_STAGING_MIB.  Unset = the defaults.
+long long env_ll(const char* name, long long dflt) {
+  const char* v = std::getenv(name);
+  if (!v || !*v) return dflt;
+  char* end = nullptr;
+  const long long x = std::strtoll(v, &end, 10);
+  return end && *end == 0 ? x : dflt;
+}
 
 struct ProfSpan { cudaEvent_t a, b; long long bytes; };
 
@@ -52,6 +62,7 @@ struct Direction {
   unsigned char* staging[2] = {nullptr, nullptr};
   cudaEvent_t kern_done[2] = {nullptr, nullptr}, copy_done[2] = {nullptr, nullptr};
   int buf = 0;
+  bool copy_busy = false;                        // DMAs enqueued on `copy` since the last join
   // index ring: pinned host (written by the CPU, read by the upload kernel) + device copy
   int32_t* idx_host = nullptr; int32_t* idx_host_dev = nullptr; int32_t* idx_dev = nullptr;
   long long idx_cap = 0, idx_used = 0;
@@ -68,18 +79,24 @@ struct mori_ctx {
   int device = 0, sm_count = 148;
   long long chunk = 0, page_bytes = 0, staging_bytes = 0, max_pages = 0;
   int copy_kernel = MORI_KERNEL_TMA;
-  int piece = kPieceBytes, ppc = 1, tma_stages = 3, tma_lag = 1;
+  int piece = kPieceBytesDefault, ppc = 1, tma_stages = 3, tma_lag = 1, ctas_per_sm = 1;
   int link_ctas = 32;
   size_t tma_smem = 0;
+  unsigned int* sched = nullptr;                 // [kSchedRing][2] chunk counters of the copy kernel (nullptr: static)
+  mutable unsigned long long sched_seq = 0;
+  bool debug = false;                            // MORI_DEBUG=1: duplicate-id validation
+  std::vector<uint8_t> dbg_seen;                 // scratch bitmap of the host-side duplicate check
+  int* dbg_flag = nullptr; unsigned int* dbg_bitmap = nullptr;   // device-side check of gather/scatter ids
+  int* dbg_flag_host = nullptr;
   unsigned char* arena_dev = nullptr;            // device-side alias of the pinned arena
   bool arena_is_device = false;                  // arena lives in (this or a peer GPU's) HBM
   unsigned int* rank_tickets = nullptr;          // [kRankTickets] last-CTA counters of the multi-CTA ranker
   unsigned long long rank_seq = 0;
   int idl_k = 5;                                 // window of Eq. (1)
   double* idl_r = nullptr; double* idl_a = nullptr; int32_t* idl_pushed = nullptr;   // [max_programs][k], [max_programs]
-  // the 16-node sequence of mori_eviction_order, captured once per argument set and replayed
-  cudaGraphExec_t evict_exec = nullptr; cudaStream_t evict_cap_stream = nullptr;
-  struct { int tier, n_programs; long long n_pages; const void *owner, *ptier, *last; void *victims, *nres; } evict_key{};
+  // the sequence of mori_eviction_order, captured once per (tier, argument set) and replayed
+  cudaGraphExec_t evict_exec[2] = {nullptr, nullptr}; cudaStream_t evict_cap_stream = nullptr;
+  struct EvictKey { int n_programs; long long n_pages; const void *owner, *ptier, *last; void *victims, *nres; } evict_key[2]{};
   unsigned int* evict_max_last = nullptr;
   int32_t* evict_perm[2] = {nullptr, nullptr}; int32_t* evict_table = nullptr; long long evict_cap = 0;   // scratch, grown on demand
   int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
@@ -114,6 +131,20 @@ __global__ void upload_idx_kernel(const int32_t* __restrict__ src, int32_t* __re
     dst[i] = src[i];
 }
 
+// MORI_DEBUG: range (and, for destinations, duplicate) check of a DEVICE id table.  flag: bit 0 =
+// out of range, bit 1 = duplicate.  The bitmap is left clean (second pass clears what was set).
+__global__ void validate_ids_kernel(const int32_t* __restrict__ ids, long long n, long long id_space,
+                                    unsigned int* __restrict__ bitmap, int check_dup, int clear, int* flag) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const int id = ids[i];
+    if (id < 0 || id >= id_space) { if (!clear) atomicOr(flag, 1); continue; }
+    if (!check_dup) continue;
+    const unsigned int bit = 1u << (id & 31);
+    if (clear) atomicAnd(&bitmap[id >> 5], ~bit);
+    else if (atomicOr(&bitmap[id >> 5], bit) & bit) atomicOr(flag, 2);
+  }
+}
+
 mori::CopyArgs make_args(const mori_ctx* c, unsigned char* lin, const int32_t* gpu_pages,
                          const int32_t* lin_idx, long long n_pages) {
   mori::CopyArgs a;
@@ -129,6 +160,7 @@ mori::CopyArgs make_args(const mori_ctx* c, unsigned char* lin, const int32_t* g
   a.pieces_per_chunk = c->ppc;
   a.stages = c->tma_stages;
   a.store_lag = c->tma_lag;
+  a.sched = nullptr;
   return a;
 }
 
@@ -140,9 +172,11 @@ cudaError_t launch_copy(const mori_ctx* c, const mori::CopyArgs& a, cudaStream_t
   if (n_pieces == 0) return cudaSuccess;
   c->launches += 1;
   if (c->copy_kernel == MORI_KERNEL_TMA) {
-    const long long max_grid = link ? c->link_ctas : c->sm_count;  // 1 CTA per SM (smem-bound)
-    const int grid = (int)std::min<long long>(a.n_pages * a.n_layers, max_grid);   // CTAs stride chunks
-    mori::copy_pages_tma<kGather><<<grid, mori::kTmaThreads, c->tma_smem, s>>>(a);
+    const long long max_grid = link ? c->link_ctas : (long long)c->sm_count * c->ctas_per_sm;  // smem-bound residency
+    const int grid = (int)std::min<long long>(a.n_pages * a.n_layers, max_grid);   // CTAs take whole chunks
+    mori::CopyArgs b = a;
+    if (c->sched && grid > 1) b.sched = c->sched + 2 * (c->sched_seq++ % kSchedRing);
+    mori::copy_pages_tma<kGather><<<grid, mori::kTmaThreads, c->tma_smem, s>>>(b);
   } else {
     mori::CopyArgs b = a;                                        // LD/ST works in 16 KiB pieces
     b.piece_bytes = (int)std::min<long long>(16 * 1024, a.chunk_bytes);
@@ -155,10 +189,33 @@ cudaError_t launch_copy(const mori_ctx* c, const mori::CopyArgs& a, cudaStream_t
   return cudaGetLastError();
 }
 
+// The one-launch path of a small move: ids by value in the kernel parameters, LD/ST straight
+// between the pool and the (mapped or device) arena.
+template <bool kGather>
+cudaError_t launch_small(const mori_ctx* c, long long n, const int32_t* gpu_pages, const int32_t* host_slots,
+                         cudaStream_t s) {
+  mori::SmallIds ids;
+  std::memcpy(ids.gpu, gpu_pages, sizeof(int32_t) * n);
+  std::memcpy(ids.lin, host_slots, sizeof(int32_t) * n);
+  mori::CopyArgs a = make_args(c, c->arena_dev, nullptr, nullptr, n);
+  a.pieces_per_chunk = (int)((c->chunk + mori::kSmallPiece - 1) / mori::kSmallPiece);
+  const long long n_pieces = n * a.n_layers * a.pieces_per_chunk;
+  const int grid = (int)std::min<long long>(n_pieces, (long long)c->sm_count * 4);
+  c->launches += 1;
+  mori::copy_pages_small<kGather><<<grid, mori::kLdstThreads, 0, s>>>(a, ids);
+  return cudaGetLastError();
+}
+
+// nullptr (and a latched MORI_ERR_CUDA) when the driver cannot create an event.
 cudaEvent_t get_event(mori_ctx* c, bool timing) {
   cudaEvent_t e = nullptr;
   if (!timing && !c->free_events.empty()) { e = c->free_events.back(); c->free_events.pop_back(); return e; }
-  cudaEventCreateWithFlags(&e, timing ? cudaEventDefault : cudaEventDisableTiming);
+  const cudaError_t rc = cudaEventCreateWithFlags(&e, timing ? cudaEventDefault : cudaEventDisableTiming);
+  if (rc != cudaSuccess) {
+    c->sticky = MORI_ERR_CUDA;
+    c->err = std::string("cudaEventCreateWithFlags: ") + cudaGetErrorString(rc);
+    return nullptr;
+  }
   return e;
 }
 
@@ -169,6 +226,23 @@ int check_ids(const mori_ctx* c, long long n, const int32_t* gpu_pages, const in
     if (host_slots[j] < 0 || host_slots[j] >= c->cfg.host_arena_slots)
       return fail(c, MORI_ERR_INVALID_ARG, "host slot id out of range at index " + std::to_string(j));
   }
+  return MORI_OK;
+}
+
+// MORI_DEBUG=1: a DESTINATION id listed twice in one call is undefined behaviour in release (two
+// copies race for the same bytes); here it is found on the host before anything is enqueued.
+int check_duplicates(mori_ctx* c, long long n, const int32_t* dst_ids, long long id_space, const char* what) {
+  if ((long long)c->dbg_seen.size() < id_space) c->dbg_seen.assign((size_t)id_space, 0);
+  int rc = MORI_OK;
+  long long j = 0;
+  for (; j < n; ++j) {
+    if (c->dbg_seen[dst_ids[j]]) { rc = MORI_ERR_INVALID_ARG; break; }
+    c->dbg_seen[dst_ids[j]] = 1;
+  }
+  const long long bad = j;
+  for (long long i = 0; i < (rc ? bad : n); ++i) c->dbg_seen[dst_ids[i]] = 0;
+  if (rc) return fail(c, rc, std::string("MORI_DEBUG: duplicate destination ") + what + " " +
+                             std::to_string(dst_ids[bad]) + " at index " + std::to_string(bad));
   return MORI_OK;
 }
 
@@ -214,16 +288,18 @@ int issue_ticket(mori_ctx* c, Direction& d, cudaStream_t s, int64_t* out) {
 void prof_begin(mori_ctx* c, Direction& d, cudaStream_t s, long long bytes) {
   if (!c->profiling) return;
   ProfSpan sp{get_event(c, true), get_event(c, true), bytes};
-  cudaEventRecord(sp.a, s);
+  if (!sp.a || !sp.b) { if (sp.a) cudaEventDestroy(sp.a); if (sp.b) cudaEventDestroy(sp.b); sp.a = sp.b = nullptr; }
+  if (sp.a) cudaEventRecord(sp.a, s);
   d.spans.push_back(sp);
 }
 void prof_end(mori_ctx* c, Direction& d, cudaStream_t s) {
-  if (!c->profiling) return;
+  if (!c->profiling || d.spans.empty() || !d.spans.back().b) return;
   cudaEventRecord(d.spans.back().b, s);
 }
 void prof_collect(Direction& d) {
   for (auto& sp : d.spans) {
     float ms = 0;
+    if (!sp.a) continue;
     if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) {
       d.prof_ms += ms; d.prof_launches += 1; d.prof_bytes += sp.bytes;
     }
@@ -334,15 +410,26 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   c->chunk = chunk;
   if (cfg->zerocopy_ctas > 0) c->link_ctas = cfg->zerocopy_ctas;
   c->page_bytes = chunk * cfg->n_layers;
-  c->piece = (int)std::min<long long>(kPieceBytes, chunk);
+  // Ring geometry of the bulk-copy kernel: `ctas_per_sm` CTAs share an SM's ring budget, each with
+  // as many stages of `piece` bytes as fit (DESIGN.md section 5.2 has the measurements behind the
+  // defaults).
+  c->ctas_per_sm = (int)std::max<long long>(1, std::min<long long>(8, env_ll("MORI_CTAS_PER_SM", 1)));
+  const long long ring_bytes = std::max<long long>(16, std::min<long long>(200, env_ll("MORI_RING_KIB", kRingBytesDefault >> 10))) << 10;
+  const long long piece_max = std::max<long long>(1, std::min<long long>(128, env_ll("MORI_PIECE_KIB", kPieceBytesDefault >> 10))) << 10;
+  c->piece = (int)std::min<long long>(piece_max, chunk);
   c->ppc = (int)((chunk + c->piece - 1) / c->piece);
   c->copy_kernel = cfg->copy_kernel == MORI_KERNEL_AUTO ? MORI_KERNEL_TMA : cfg->copy_kernel;
-  c->tma_stages = std::max(2, std::min(kMaxTmaStages, kRingBytes / c->piece));
+  c->tma_stages = (int)std::max<long long>(2, std::min<long long>(kMaxTmaStages, ring_bytes / c->ctas_per_sm / c->piece));
   c->tma_lag = c->tma_stages >= 6 ? 2 : 1;
-  c->tma_smem = (size_t)c->tma_stages * c->piece + 2 * c->tma_stages * sizeof(uint64_t);
+  c->tma_smem = mori::tma_smem_bytes(c->tma_stages, c->piece);
+  if (c->tma_smem > (size_t)prop.sharedMemPerBlockOptin) {
+    delete c;
+    return fail(nullptr, MORI_ERR_INVALID_ARG, "copy-kernel ring does not fit shared memory (chunk too large for 2 stages)");
+  }
+  c->debug = env_ll("MORI_DEBUG", 0) != 0;
   c->max_pages = cfg->max_pages_per_call ? cfg->max_pages_per_call
                                           : std::max<long long>(cfg->gpu_pool_pages, cfg->host_arena_slots);
-  c->staging_bytes = cfg->staging_bytes ? cfg->staging_bytes : (1024LL << 20);
+  c->staging_bytes = cfg->staging_bytes ? cfg->staging_bytes : (env_ll("MORI_STAGING_MIB", 1024) << 20);
   c->staging_bytes = std::min(c->staging_bytes, c->max_pages * c->page_bytes);   // never more than one call can fill
   c->staging_bytes = std::max(c->staging_bytes, c->page_bytes);
   c->staging_bytes -= c->staging_bytes % c->page_bytes;
@@ -362,10 +449,24 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
     }                                                                                         \
   } while (0)
 
-  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
-  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tma_smem));
+  // The attribute is per function and PROCESS-wide: every context sets it to the device's opt-in
+  // maximum, so contexts with different ring sizes never lower it under one another.
+  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
+  CKC(cudaFuncSetAttribute(mori::copy_pages_tma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
   CKC(cudaMalloc((void**)&c->rank_tickets, sizeof(unsigned int) * kRankTickets));
   CKC(cudaMemset(c->rank_tickets, 0, sizeof(unsigned int) * kRankTickets));
+  if (env_ll("MORI_SCHED", 1) != 0) {
+    CKC(cudaMalloc((void**)&c->sched, sizeof(unsigned int) * 2 * kSchedRing));
+    CKC(cudaMemset(c->sched, 0, sizeof(unsigned int) * 2 * kSchedRing));
+  }
+  if (c->debug) {
+    const long long ids = std::max<long long>(cfg->gpu_pool_pages, cfg->host_arena_slots);
+    CKC(cudaMalloc((void**)&c->dbg_bitmap, sizeof(unsigned int) * (size_t)((ids + 31) / 32)));
+    CKC(cudaMemset(c->dbg_bitmap, 0, sizeof(unsigned int) * (size_t)((ids + 31) / 32)));
+    CKC(cudaHostAlloc((void**)&c->dbg_flag_host, sizeof(int), cudaHostAllocMapped));
+    *c->dbg_flag_host = 0;
+    CKC(cudaHostGetDevicePointer((void**)&c->dbg_flag, c->dbg_flag_host, 0));
+  }
   c->idl_k = cfg->idleness_window ? cfg->idleness_window : 5;
   CKC(cudaMalloc((void**)&c->idl_r, sizeof(double) * (size_t)cfg->max_programs * c->idl_k));
   CKC(cudaMalloc((void**)&c->idl_a, sizeof(double) * (size_t)cfg->max_programs * c->idl_k));
@@ -432,8 +533,11 @@ int mori_destroy(mori_ctx* c) {
   }
   for (auto ev : c->free_events) cudaEventDestroy(ev);
   if (c->rank_tickets) cudaFree(c->rank_tickets);
+  if (c->sched) cudaFree(c->sched);
+  if (c->dbg_bitmap) cudaFree(c->dbg_bitmap);
+  if (c->dbg_flag_host) cudaFreeHost(c->dbg_flag_host);
   if (c->sticky_order) cudaFree(c->sticky_order);
-  if (c->evict_exec) cudaGraphExecDestroy(c->evict_exec);
+  for (int t = 0; t < 2; ++t) if (c->evict_exec[t]) cudaGraphExecDestroy(c->evict_exec[t]);
   if (c->evict_cap_stream) cudaStreamDestroy(c->evict_cap_stream);
   for (int b = 0; b < 2; ++b) if (c->evict_perm[b]) cudaFree(c->evict_perm[b]);
   if (c->evict_table) cudaFree(c->evict_table);
@@ -596,7 +700,7 @@ int mori_eviction_order(mori_ctx* c, void* stream, int32_t which_tier, int64_t n
   const int tiles = (int)((n_pages + mori::kEvictTile - 1) / mori::kEvictTile);
   if (n_pages > c->evict_cap) {                    // first use / larger pool: (re)allocate scratch
     CK(c, cudaStreamSynchronize(s));
-    if (c->evict_exec) { cudaGraphExecDestroy(c->evict_exec); c->evict_exec = nullptr; }
+    for (int t = 0; t < 2; ++t) if (c->evict_exec[t]) { cudaGraphExecDestroy(c->evict_exec[t]); c->evict_exec[t] = nullptr; }
     for (int b = 0; b < 2; ++b) { if (c->evict_perm[b]) cudaFree(c->evict_perm[b]); c->evict_perm[b] = nullptr; }
     if (c->evict_table) cudaFree(c->evict_table);
     c->evict_table = nullptr; c->evict_cap = 0;
@@ -620,30 +724,33 @@ int mori_eviction_order(mori_ctx* c, void* stream, int32_t which_tier, int64_t n
     }
     return cudaGetLastError();
   };
-  // Launch-bound (15 small kernels + a memset): captured once into a CUDA graph per argument set
-  // -- an engine passes the same tables every time -- and replayed with one cudaGraphLaunch.
-  const bool same = c->evict_exec && c->evict_key.tier == which_tier && c->evict_key.n_programs == n_programs &&
-                    c->evict_key.n_pages == n_pages && c->evict_key.owner == page_owner &&
-                    c->evict_key.ptier == program_tier && c->evict_key.last == last_access &&
-                    c->evict_key.victims == victims && c->evict_key.nres == n_resident;
+  // Launch-bound (15 small kernels + a memset): captured once into a CUDA graph per (tier,
+  // argument set) -- an engine passes the same tables every time, and alternating between the two
+  // tiers keeps both graphs -- and replayed with one cudaGraphLaunch.  The scratch is shared, so
+  // calls must be enqueued on one stream at a time (include/mori.h).
+  const int gi = which_tier == MORI_TIER_GPU ? 0 : 1;
+  cudaGraphExec_t& exec = c->evict_exec[gi];
+  mori_ctx::EvictKey& key = c->evict_key[gi];
+  const bool same = exec && key.n_programs == n_programs && key.n_pages == n_pages && key.owner == page_owner &&
+                    key.ptier == program_tier && key.last == last_access && key.victims == victims &&
+                    key.nres == n_resident;
   if (!same) {
-    if (c->evict_exec) { cudaGraphExecDestroy(c->evict_exec); c->evict_exec = nullptr; }
+    if (exec) { cudaGraphExecDestroy(exec); exec = nullptr; }
     if (!c->evict_cap_stream) cudaStreamCreateWithFlags(&c->evict_cap_stream, cudaStreamNonBlocking);
     cudaGraph_t g = nullptr;
     if (c->evict_cap_stream &&
         cudaStreamBeginCapture(c->evict_cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
       const cudaError_t e1 = enqueue(c->evict_cap_stream);
       const cudaError_t e2 = cudaStreamEndCapture(c->evict_cap_stream, &g);
-      if (e1 == cudaSuccess && e2 == cudaSuccess && g &&
-          cudaGraphInstantiate(&c->evict_exec, g, 0) != cudaSuccess)
-        c->evict_exec = nullptr;
-      if (e1 != cudaSuccess || e2 != cudaSuccess) c->evict_exec = nullptr;
+      if (e1 == cudaSuccess && e2 == cudaSuccess && g && cudaGraphInstantiate(&exec, g, 0) != cudaSuccess)
+        exec = nullptr;
+      if (e1 != cudaSuccess || e2 != cudaSuccess) exec = nullptr;
       if (g) cudaGraphDestroy(g);
     }
     cudaGetLastError();                            // a failed capture falls back to plain launches
-    c->evict_key = {which_tier, n_programs, n_pages, page_owner, program_tier, last_access, victims, n_resident};
+    key = {n_programs, n_pages, page_owner, program_tier, last_access, victims, n_resident};
   }
-  if (c->evict_exec) CK(c, cudaGraphLaunch(c->evict_exec, s));
+  if (exec) CK(c, cudaGraphLaunch(exec, s));
   else CK(c, enqueue(s));
   c->launches += 3 * mori::kEvictPasses;
   return MORI_OK;
@@ -678,10 +785,27 @@ int mori_idleness_eval(mori_ctx* c, void* stream, int32_t n, const double* open_
   return MORI_OK;
 }
 
+// MORI_DEBUG only: validates a DEVICE page table on `stream` and waits for the verdict.
+static int debug_validate(mori_ctx* c, cudaStream_t s, long long n, const int32_t* ids, bool check_dup) {
+  if (!c->debug || n == 0) return MORI_OK;
+  *c->dbg_flag_host = 0;
+  const int grid = (int)std::min<long long>((n + 255) / 256, 1024);
+  validate_ids_kernel<<<grid, 256, 0, s>>>(ids, n, c->cfg.gpu_pool_pages, c->dbg_bitmap, check_dup ? 1 : 0, 0, c->dbg_flag);
+  if (check_dup)
+    validate_ids_kernel<<<grid, 256, 0, s>>>(ids, n, c->cfg.gpu_pool_pages, c->dbg_bitmap, 1, 1, c->dbg_flag);
+  CK(c, cudaGetLastError());
+  CK(c, cudaStreamSynchronize(s));
+  const int f = *c->dbg_flag_host;
+  if (f & 1) return fail(c, MORI_ERR_INVALID_ARG, "MORI_DEBUG: gpu page id out of range in a device page table");
+  if (f & 2) return fail(c, MORI_ERR_INVALID_ARG, "MORI_DEBUG: duplicate destination gpu page in a device page table");
+  return MORI_OK;
+}
+
 int mori_gather_pages(mori_ctx* c, void* stream, int64_t n_pages, const int32_t* gpu_pages, void* dst) {
   if (!c) return MORI_ERR_INVALID_ARG;
   if (c->sticky) return c->sticky;
   if (n_pages < 0 || (n_pages > 0 && (!gpu_pages || !dst))) return fail(c, MORI_ERR_INVALID_ARG, "bad gather arguments");
+  if (int rc = debug_validate(c, static_cast<cudaStream_t>(stream), n_pages, gpu_pages, false)) return rc;
   mori::CopyArgs a = make_args(c, static_cast<unsigned char*>(dst), gpu_pages, nullptr, n_pages);
   CK(c, launch_copy<true>(c, a, static_cast<cudaStream_t>(stream), false));
   return MORI_OK;
@@ -691,14 +815,18 @@ int mori_scatter_pages(mori_ctx* c, void* stream, int64_t n_pages, const int32_t
   if (!c) return MORI_ERR_INVALID_ARG;
   if (c->sticky) return c->sticky;
   if (n_pages < 0 || (n_pages > 0 && (!gpu_pages || !src))) return fail(c, MORI_ERR_INVALID_ARG, "bad scatter arguments");
+  if (int rc = debug_validate(c, static_cast<cudaStream_t>(stream), n_pages, gpu_pages, true)) return rc;
   mori::CopyArgs a = make_args(c, static_cast<unsigned char*>(const_cast<void*>(src)), gpu_pages, nullptr, n_pages);
   CK(c, launch_copy<false>(c, a, static_cast<cudaStream_t>(stream), false));
   return MORI_OK;
 }
 
 // Shared body of mori_demote (dir 0) and mori_promote (dir 1).
+//   wait_pool   ticket of the OTHER direction after which this call may touch the POOL
+//   wait_arena  ticket of the OTHER direction after which this call may touch the ARENA
+// (mori_demote passes the same ticket twice.)  On every path both hold for every byte of the call.
 static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_pages, const int32_t* host_slots,
-                   long long wait_other, int64_t* ticket_out) {
+                   long long wait_pool, long long wait_arena, int64_t* ticket_out) {
   if (!c) return MORI_ERR_INVALID_ARG;
   if (c->sticky) return c->sticky;
   if (!c->cfg.host_arena) return fail(c, MORI_ERR_STATE, "context was created without a host arena");
@@ -708,41 +836,63 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
   Direction& d = c->dir[di];
   Direction& other = c->dir[1 - di];
   const bool demote = di == 0;
+  if (c->debug) {
+    const int rc = demote ? check_duplicates(c, total, host_slots, c->cfg.host_arena_slots, "host slot")
+                          : check_duplicates(c, total, gpu_pages, c->cfg.gpu_pool_pages, "gpu page");
+    if (rc) return rc;
+  }
+  for (long long t : {wait_pool, wait_arena})
+    if (t > 0 && t >= other.next_ticket) return fail(c, MORI_ERR_INVALID_ARG, "ticket was never issued");
   unsigned char* pool = static_cast<unsigned char*>(c->cfg.gpu_pool);
   unsigned char* arena = static_cast<unsigned char*>(c->cfg.host_arena);
   const long long pb = c->page_bytes;
 
-  // AUTO: a DMA per run of consecutive slots costs ~4.3 us of copy-engine
-  // set-up, so short runs (2 MiB: 89 % of the link peak, 4 MiB: 94 %) lose to SM-driven
-  // zero-copy (92 % whatever the run length); long runs (>= 8 MiB: 97-100 %) win.
+  // AUTO: a few pages -> the one-launch path.  Otherwise a DMA per run of
+  // consecutive slots costs ~4.3 us of copy-engine set-up, so short runs (2 MiB: 89 % of the link
+  // peak, 4 MiB: 94 %) lose to SM-driven zero-copy (92 % whatever the run length); long runs
+  // (>= 8 MiB: 97-100 %) win.
   int path = d.path;
+  bool small = false;
   if (d.auto_path && total > 0) {
+    small = total <= mori::kSmallMaxPages && total * pb <= kSmallMaxBytes;
     long long runs = 1;
     for (long long j = 1; j < total; ++j) runs += host_slots[j] != host_slots[j - 1] + 1;
-    path = (total * pb / runs < kAutoMinRunBytes) ? MORI_PATH_ZEROCOPY : MORI_PATH_STAGED;
+    path = (small || total * pb / runs < kAutoMinRunBytes) ? MORI_PATH_ZEROCOPY : MORI_PATH_STAGED;
   }
 
+  // one stream carries the whole call on every path but STAGED: it waits for both tickets
+  auto wait_both = [&](cudaStream_t s) -> int {
+    if (int rc = wait_ticket(c, other, wait_pool, s)) return rc;
+    if (wait_arena != wait_pool) if (int rc = wait_ticket(c, other, wait_arena, s)) return rc;
+    return MORI_OK;
+  };
+
   if (path == MORI_PATH_ZEROCOPY) {
-    if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc;
+    if (int rc = wait_both(d.kern)) return rc;
     // Calls of one direction take effect in issue order.  An earlier STAGED demote of this
     // direction may still have DMAs in flight on the copy stream: this kernel must not overtake
     // them (same-stream order covers every other combination of paths).
-    if (demote)
+    if (demote && d.copy_busy)
       for (int b = 0; b < 2; ++b)
         if (d.copy_done[b]) CK(c, cudaStreamWaitEvent(d.kern, d.copy_done[b], 0));
     if (total > 0) {
-      const int32_t *dg, *dh;
-      if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;
-      mori::CopyArgs a = make_args(c, c->arena_dev, dg, dh, total);
       prof_begin(c, d, d.kern, total * pb);
-      CK(c, demote ? launch_copy<true>(c, a, d.kern, !c->arena_is_device) : launch_copy<false>(c, a, d.kern, !c->arena_is_device));
+      if (small) {
+        CK(c, demote ? launch_small<true>(c, total, gpu_pages, host_slots, d.kern)
+                     : launch_small<false>(c, total, gpu_pages, host_slots, d.kern));
+      } else {
+        const int32_t *dg, *dh;
+        if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;
+        mori::CopyArgs a = make_args(c, c->arena_dev, dg, dh, total);
+        CK(c, demote ? launch_copy<true>(c, a, d.kern, !c->arena_is_device) : launch_copy<false>(c, a, d.kern, !c->arena_is_device));
+      }
       prof_end(c, d, d.kern);
     }
     return issue_ticket(c, d, d.kern, ticket_out);
   }
 
   if (path == MORI_PATH_COPYENGINE) {
-    if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc;
+    if (int rc = wait_both(d.kern)) return rc;
     const size_t dpitch = (size_t)c->cfg.gpu_pool_pages * c->chunk;   // layer stride in the pool
     for (long long j = 0; j < total; ++j) {
       unsigned char* dev = pool + (long long)gpu_pages[j] * c->chunk;
@@ -756,12 +906,21 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
   // STAGED.  demote:  kern stream: gather -> staging[b]      copy stream: staging[b] -> arena
   //          promote: copy stream: arena -> staging[b]       kern stream: staging[b] -> scatter
   // Double-buffered with events so the DMA of segment i overlaps the kernel of segment i+1.
+  // demote : the gather (pool reads) is first in the pipeline and every DMA follows a gather, so
+  //          both tickets gate the kernel stream.
+  // promote: the DMAs read the ARENA -> the copy stream waits for wait_arena; the scatters write
+  //          the POOL -> the kernel stream waits for wait_pool.  A promotion into pages that a
+  //          demotion is still vacating therefore streams its bytes over the link meanwhile.
   const long long seg_pages = c->staging_bytes / pb;
   const int32_t* dg = nullptr; const int32_t* dh = nullptr;
-  if (demote) { if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc; }
+  if (demote) { if (int rc = wait_both(d.kern)) return rc; }
+  else {
+    if (int rc = wait_ticket(c, other, wait_arena, d.copy)) return rc;
+    if (int rc = wait_ticket(c, other, wait_pool, d.kern)) return rc;
+  }
   if (total > 0)
     if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;
-  bool waited = demote;
+  if (total > 0) d.copy_busy = true;
   for (long long a0 = 0; a0 < total; a0 += seg_pages) {
     const long long cnt = std::min(seg_pages, total - a0);
     const int b = d.buf; d.buf ^= 1;
@@ -791,7 +950,6 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
       CK(c, cudaStreamWaitEvent(d.copy, d.kern_done[b], 0));       // staging[b] scattered
       if (int rc = dma(d.copy)) return rc;
       CK(c, cudaEventRecord(d.copy_done[b], d.copy));
-      if (!waited) { if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc; waited = true; }
       CK(c, cudaStreamWaitEvent(d.kern, d.copy_done[b], 0));
       prof_begin(c, d, d.kern, cnt * pb);
       CK(c, launch_copy<false>(c, a, d.kern, false));
@@ -799,28 +957,31 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
       CK(c, cudaEventRecord(d.kern_done[b], d.kern));
     }
   }
-  if (!waited) { if (int rc = wait_ticket(c, other, wait_other, d.kern)) return rc; }
   // the ticket marks the end of the LAST stage of the pipeline
   if (demote) {
-    // copy stream finishes last; make the kernel stream's order include it so that one event
-    // on one stream covers the call
+    // copy stream finishes last; it already follows the kernel stream, so one event on it covers
+    // the call
     cudaEvent_t ev = d.tickets[d.next_ticket % kTicketRing];
     const long long t = d.next_ticket++;
     CK(c, cudaEventRecord(ev, d.copy));
     if (ticket_out) *ticket_out = t;
     return MORI_OK;
   }
+  // promote: the kernel stream finishes last; an EMPTY call has put nothing on it that follows the
+  // copy stream's wait for wait_arena, so fold that in for the ticket to cover both waits
+  if (total == 0 && wait_arena > 0 && wait_arena != wait_pool)
+    if (int rc = wait_ticket(c, other, wait_arena, d.kern)) return rc;
   return issue_ticket(c, d, d.kern, ticket_out);
 }
 
 int mori_demote(mori_ctx* c, int64_t total, const int32_t* gpu_pages, const int32_t* host_slots,
                 int64_t wait_promote_ticket, int64_t* ticket_out) {
-  return migrate(c, 0, total, gpu_pages, host_slots, wait_promote_ticket, ticket_out);
+  return migrate(c, 0, total, gpu_pages, host_slots, wait_promote_ticket, wait_promote_ticket, ticket_out);
 }
 
 int mori_promote(mori_ctx* c, int64_t total, const int32_t* host_slots, const int32_t* gpu_pages,
-                 int64_t wait_demote_ticket, int64_t* ticket_out) {
-  return migrate(c, 1, total, gpu_pages, host_slots, wait_demote_ticket, ticket_out);
+                 int64_t pages_after_demote, int64_t slots_after_demote, int64_t* ticket_out) {
+  return migrate(c, 1, total, gpu_pages, host_slots, pages_after_demote, slots_after_demote, ticket_out);
 }
 
 int mori_sync(mori_ctx* c, int32_t which) {
@@ -836,6 +997,7 @@ int mori_sync(mori_ctx* c, int32_t which) {
       return fail(c, MORI_ERR_CUDA, std::string("asynchronous failure: ") + cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
     }
     d.idx_used = 0;
+    d.copy_busy = false;
     prof_collect(d);
   }
   return c->sticky;
@@ -843,7 +1005,9 @@ int mori_sync(mori_ctx* c, int32_t which) {
 
 int mori_after_stream(mori_ctx* c, int32_t which, void* stream) {
   if (!c || which < 1 || which > 3) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
   cudaEvent_t ev = get_event(c, false);
+  if (!ev) return c->sticky;
   CK(c, cudaEventRecord(ev, static_cast<cudaStream_t>(stream)));
   for (int i = 0; i < 2; ++i)
     if (which & (1 << i)) {
@@ -856,10 +1020,13 @@ int mori_after_stream(mori_ctx* c, int32_t which, void* stream) {
 
 int mori_stream_wait(mori_ctx* c, void* stream, int32_t which) {
   if (!c || which < 1 || which > 3) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
   for (int i = 0; i < 2; ++i)
     if (which & (1 << i))
       for (cudaStream_t s : {c->dir[i].kern, c->dir[i].copy}) {
+        if (s == c->dir[i].copy && !c->dir[i].copy_busy) continue;   // nothing enqueued there since the last join
         cudaEvent_t ev = get_event(c, false);
+        if (!ev) return c->sticky;
         CK(c, cudaEventRecord(ev, s));
         CK(c, cudaStreamWaitEvent(static_cast<cudaStream_t>(stream), ev, 0));
         c->free_events.push_back(ev);

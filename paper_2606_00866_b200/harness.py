@@ -136,17 +136,55 @@ class GpuRunner:
                     lists=[lists2d[k, :counts[k]].copy() for k in range(5)])
 
     # -- a5-a7 ---------------------------------------------------------------------------------
-    def execute(self, plan: W.EpochPlan, sync=True):
-        tickets = {}
+    def execute(self, plan: W.EpochPlan, sync=True, merge=True):
+        """Issues the epoch's moves.  A move is a flat list of pages (include/mori.h), so the
+        demotions of an epoch go out as ONE ``mori_demote`` per stretch of the plan that no promotion
+        depends on, and the promotions likewise as one ``mori_promote`` per stretch with the same
+        dependency: fewer calls, fewer ragged last staging segments, and the page order inside a
+        call is the plan's (the paper's move order, P:L206 / L208).  ``merge=False`` issues one call
+        per program."""
+        tickets = {}                      # demote number k -> ticket of the call that carried it
+        dem, pro, pro_dep = [], [], 0
+
+        def flush_dem():
+            if dem:
+                t = self.mori.mori_demote(np.concatenate([o[3] for o in dem]), np.concatenate([o[4] for o in dem]))
+                for o in dem:
+                    tickets[o[1]] = t
+                dem.clear()
+
+        def flush_pro():
+            nonlocal pro_dep
+            if pro:
+                if pro_dep > 0 and pro_dep not in tickets:
+                    flush_dem()
+                self.mori.mori_promote(np.concatenate([o[3] for o in pro]), np.concatenate([o[4] for o in pro]),
+                                       pages_after_demote=tickets.get(pro_dep, 0) if pro_dep > 0 else 0)
+                pro.clear()
+            pro_dep = 0
+
         for op in plan.ops:
             if op[0] == "demote":
-                tickets[op[1]] = self.mori.mori_demote(op[3], op[4])
+                dem.append(op)
+                if not merge:
+                    flush_dem()
             elif op[0] == "promote":
-                dep = tickets.get(op[5], 0) if op[5] > 0 else 0
-                self.mori.mori_promote(op[3], op[4], wait_demote_ticket=dep)
+                dep = op[5] if op[5] > 0 else 0
+                if pro and dep != pro_dep:        # a different dependency: its own call
+                    flush_pro()
+                if dep > 0 and dep not in tickets:
+                    flush_dem()                   # the demotion it follows ends its call here, so the
+                                                  # promotion waits for that much and no more
+                pro.append(op)
+                pro_dep = dep
+                if not merge:
+                    flush_pro()
             elif op[0] == "sync_all":
+                flush_dem(); flush_pro()
                 self.mori.mori_sync(binding.BOTH)
                 tickets.clear()
+        # both directions start together: the demote call first (it is what vacates pages)
+        flush_dem(); flush_pro()
         if sync:
             self.mori.mori_sync(binding.BOTH)
 
@@ -202,3 +240,108 @@ class GpuRunner:
 
     def close(self):
         self.mori.close()
+
+
+class TierRunner:
+    """A three-tier hierarchy on the CUDA path (SURVEY 8f NEXT-4 ii): the paged GPU
+    pool, a middle arena in device memory (a peer GPU's HBM over NVLink in production; a second
+    buffer of this GPU here) and the pinned host arena.  Placement comes from
+    ``mori_rank_partition_tiers``; bytes move through ``mori_demote`` / ``mori_promote`` of three
+    contexts, one per pair of pools:
+
+        pool <-> mid    the pool with a DEVICE arena (one full-grid kernel per call)
+        pool <-> host   the hot path's context (staged / zero-copy over the host link)
+        mid  <-> host   the middle arena described as a pool of ONE layer whose chunk is a whole
+                        page (n_kv_heads = L * H): a slot is then one contiguous chunk, and the
+                        arena <-> arena move is the same gather -> staging -> DMA pipeline
+
+    ``workload.SimTiers`` never reuses an id freed in the current phase before a join, so the three
+    contexts need no tickets between them."""
+
+    def __init__(self, cfg: W.Config, seed: int, mid_slots: int, host_arena: Optional[torch.Tensor] = None,
+                 staging_bytes=0, device="cuda:0"):
+        self.cfg, self.seed = cfg, seed
+        sh = cfg.shape
+        self.dev = torch.device(device)
+        torch.cuda.set_device(self.dev)
+        self.pool = torch.zeros(sh.n_layers * cfg.gpu_pool_pages * sh.chunk_bytes, dtype=torch.uint8, device=self.dev)
+        self.mid = torch.zeros(mid_slots * sh.page_bytes, dtype=torch.uint8, device=self.dev)
+        host_bytes = cfg.cpu_pool_pages * sh.page_bytes
+        if host_arena is None:
+            host_arena = torch.empty(host_bytes, dtype=torch.uint8, pin_memory=True)
+        self.host = host_arena[:host_bytes]
+        n = max(1, min(binding.MAX_PROGRAMS, cfg.n_programs))
+        kw = dict(elem_bytes=sh.elem_bytes, max_programs=n, staging_bytes=staging_bytes)
+        self.pool_mid = binding.Mori(sh.n_layers, sh.n_kv_heads, sh.head_dim, sh.page_tokens, self.pool, self.mid, **kw)
+        self.pool_host = binding.Mori(sh.n_layers, sh.n_kv_heads, sh.head_dim, sh.page_tokens, self.pool, self.host, **kw)
+        self.mid_host = binding.Mori(1, sh.n_layers * sh.n_kv_heads, sh.head_dim, sh.page_tokens, self.mid, self.host, **kw)
+        assert self.mid_host.chunk_bytes == sh.page_bytes
+        self.ctxs = (self.pool_mid, self.pool_host, self.mid_host)
+        d = self.dev
+        self.n = cfg.n_programs
+        self.d_iota = torch.empty(self.n, dtype=torch.float32, device=d)
+        self.d_kv = torch.empty(self.n, dtype=torch.int32, device=d)
+        self.d_prev = torch.empty(self.n, dtype=torch.uint8, device=d)
+        self.d_order = torch.empty(self.n, dtype=torch.int32, device=d)
+        self.d_tier = torch.empty(self.n, dtype=torch.uint8, device=d)
+        self.d_bounds = torch.empty(3, dtype=torch.int32, device=d)
+        self.d_used = torch.empty(3, dtype=torch.int64, device=d)
+        self.d_moves = torch.empty(2 * self.n, dtype=torch.int32, device=d)
+        self.d_counts = torch.empty(2, dtype=torch.int32, device=d)
+
+    def place(self, iota, kv_pages, prev_tier, caps):
+        n = self.n
+        self.d_iota.copy_(torch.from_numpy(np.ascontiguousarray(iota, dtype=np.float32)))
+        self.d_kv.copy_(torch.from_numpy(np.ascontiguousarray(kv_pages, dtype=np.int32)))
+        self.d_prev.copy_(torch.from_numpy(np.ascontiguousarray(prev_tier, dtype=np.uint8)))
+        self.pool_host.mori_rank_partition_tiers(n, self.d_iota, self.d_kv, caps, self.d_order, self.d_tier,
+                                                 self.d_bounds, self.d_used, prev_tier=self.d_prev,
+                                                 moves=self.d_moves, move_counts=self.d_counts)
+        torch.cuda.synchronize()
+        c, mv = self.d_counts.cpu().numpy(), self.d_moves.cpu().numpy()
+        return dict(order=self.d_order.cpu().numpy(), tier=self.d_tier.cpu().numpy(), bounds=self.d_bounds.cpu().numpy(),
+                    used=self.d_used.cpu().numpy(), moves=[mv[k * n:k * n + c[k]].copy() for k in range(2)])
+
+    def execute(self, plan: W.EpochPlan):
+        """One flat call per (from, to) pair and phase; a join where the planner asks for one."""
+        batch = {}
+
+        def flush():
+            for (frm, to), ops in batch.items():
+                src = np.concatenate([o[4] for o in ops])
+                dst = np.concatenate([o[5] for o in ops])
+                lo, hi = min(frm, to), max(frm, to)
+                ctx = {(0, 1): self.pool_mid, (0, 2): self.pool_host, (1, 2): self.mid_host}[(lo, hi)]
+                if to > frm:
+                    ctx.mori_demote(src, dst)                 # faster tier's ids first
+                else:
+                    ctx.mori_promote(src, dst)                # (slower tier's slots, faster tier's ids)
+            batch.clear()
+
+        def join():
+            for c in self.ctxs:
+                c.mori_sync(binding.BOTH)
+
+        for op in plan.ops:
+            if op[0] == "move":
+                batch.setdefault((op[2], op[3]), []).append(op)
+            elif op[0] == "sync_all":
+                flush(); join()
+        flush(); join()
+
+    def fill(self, fills):
+        if not fills:
+            return
+        wl = binding.load_workload_lib()
+        keys, pages, n = self._keys_pages(fills)
+        sh = self.cfg.shape
+        rc = wl.wl_fill_pages(self.pool.data_ptr(), self.cfg.gpu_pool_pages, sh.n_layers, sh.chunk_bytes,
+                              keys.data_ptr(), pages.data_ptr(), n, 0, torch.cuda.current_stream().cuda_stream)
+        assert rc == 0
+        torch.cuda.current_stream().synchronize()
+
+    _keys_pages = GpuRunner._keys_pages
+
+    def close(self):
+        for c in self.ctxs:
+            c.close()

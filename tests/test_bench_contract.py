@@ -13,7 +13,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def test_reference_arm_prints_one_contract_line():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference",
-                        "--steps", "3", "--warmup", "1"], capture_output=True, text=True, timeout=600)
+                        "--steps", "3", "--warmup", "1", "--scale", "64"], capture_output=True, text=True, timeout=600)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [l for l in r.stdout.splitlines() if l.strip()]
     assert len(lines) == 1
@@ -23,7 +23,26 @@ def test_reference_arm_prints_one_contract_line():
     assert d["value"] > 0 and d["ms_per_step"] > 0 and d["vs_baseline"] is None
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"] == {"value": d["value"], "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
-    assert "workload" in d["config"] and "model" not in d["config"]
+    assert "workload" in d["config"] and "model" not in d["config"] and d["config"]["scale"] == 64
+    assert d["cpu_baseline"]["cores"] == 1 and d["cpu_baseline"]["cpu_model"]
+
+
+def test_reference_arm_f_busy_and_threads():
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "3",
+                        "--f-busy", "0.75", "--steps", "6", "--warmup", "3", "--scale", "128", "--ref-threads", "2"],
+                       capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = json.loads(r.stdout.strip())
+    assert "f0.75" in d["config"]["workload"] and d["cpu_baseline"]["cores"] == 2 and d["value"] > 0
+
+
+def test_cpu_baseline_reports_one_core_and_all_cores():
+    sys.path.insert(0, ROOT)
+    import bench
+    cb = bench.cpu_baseline(2, budget_s=1.0, scale=64)
+    assert cb["cores"] == 1 and cb["value"] > 0 and cb["kind"] == "oracle"
+    assert cb["all_cores"]["cores"] == os.cpu_count() and cb["all_cores"]["value"] > 0
+    assert cb["cpu_model"] and cb["scale"] == 64
 
 
 def test_non_zero_ranks_of_the_reference_arm_exit_quietly():

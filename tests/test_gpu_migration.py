@@ -48,7 +48,7 @@ def test_demote_then_promote_byte_exact(mori, path, kernel, shape):
     assert np.array_equal(arena.numpy(), arena_m), "arena differs after demote"
     assert np.array_equal(pool.cpu().numpy(), pool_m), "pool changed by demote"
     g2 = rng.permutation(P)[:k].astype(np.int32)
-    m.mori_promote(h, g2, wait_demote_ticket=t)
+    m.mori_promote(h, g2, pages_after_demote=t, slots_after_demote=t)
     m.mori_sync(mori.BOTH)
     oracle.promote(L, chunk, pool_m, arena_m, h, g2)
     assert np.array_equal(pool.cpu().numpy(), pool_m), "pool differs after promote"
@@ -95,7 +95,7 @@ def test_migration_argument_errors(mori):
         with pytest.raises(mori.MoriError):
             m.mori_promote(h, g)
     with pytest.raises(mori.MoriError):
-        m.mori_promote(one, one, wait_demote_ticket=12345)          # never issued
+        m.mori_promote(one, one, pages_after_demote=12345)          # never issued
     with pytest.raises(mori.MoriError):
         m.mori_sync(0)
     m.mori_sync(mori.BOTH)
@@ -182,6 +182,36 @@ def test_scaled_twins_epochs_full_mirror(mori, idx, scale, epochs, path, kernel)
     assert moved > 0
 
 
+@pytest.mark.parametrize("f_busy", [0.25, 0.5, 0.75])
+def test_cfg3_busy_idle_sweep_epochs_full_mirror(mori, f_busy):
+    """BASELINE.json configs[2]: the busy:idle ratio swept 1:3, 1:1, 3:1.  Scaled twin with byte
+    mirrors of both pools, AUTO paths (the library picks per call), 16 epochs each."""
+    moved = _epochs_with_mirror(mori, W.get_config(3, 128, f_busy), 866, 16, 0, 0)
+    assert moved > 0
+
+
+def test_merged_and_per_program_calls_move_the_same_bytes(mori):
+    """The harness issues an epoch's demotions as one flat call (a move is a list of pages); one call
+    per program must leave both pools in the same state."""
+    cfg = W.get_config(2, 128)
+    sh = cfg.shape
+    states = []
+    for merge in (True, False):
+        sim = W.Sim(cfg, 867)
+        r = GpuRunner(cfg, 867, staging_bytes=sh.page_bytes * 5)
+        r.arena.zero_()
+        for e in range(12):
+            plan = sim.begin_epoch()
+            got = r.place(plan.iota, plan.kv_pages, plan.prev_tier)
+            sim.apply_placement(got["tier"], got["lists"])
+            r.execute(plan, merge=merge)
+            sim.end_epoch()
+            r.fill(plan.fills)
+        states.append((r.pool.cpu().numpy().copy(), r.arena.numpy().copy()))
+        r.close()
+    assert np.array_equal(states[0][0], states[1][0]) and np.array_equal(states[0][1], states[1][1])
+
+
 @pytest.mark.parametrize("idx,scale,epochs", [(2, 128, 30)])
 def test_sticky_policy_epochs_full_mirror(mori, idx, scale, epochs):
     """NEXT-1 end to end: placement from mori_sticky_rebalance (== the section-4.3.1 oracle every
@@ -236,7 +266,7 @@ def test_device_resident_arena_is_a_third_tier(mori, kernel):
     oracle.demote(L, chunk, pool_m, arena_m, g, h)
     assert np.array_equal(arena.cpu().numpy(), arena_m) and np.array_equal(pool.cpu().numpy(), pool_m)
     g2 = rng.permutation(P)[:200].astype(np.int32)
-    m.mori_promote(h, g2, wait_demote_ticket=t)
+    m.mori_promote(h, g2, pages_after_demote=t, slots_after_demote=t)
     m.mori_sync(mori.BOTH)
     oracle.promote(L, chunk, pool_m, arena_m, h, g2)
     assert np.array_equal(pool.cpu().numpy(), pool_m) and np.array_equal(arena.cpu().numpy(), arena_m)

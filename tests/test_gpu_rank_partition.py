@@ -107,12 +107,19 @@ def test_argument_errors(ctx, mori):
         ctx.mori_rank_partition(8, f, z, u, 1, 1, z, u, b, us, None, None)   # prev_tier without lists
 
 
-@pytest.mark.parametrize("idx,scale,epochs", [(1, 1, 20), (2, 1, 200), (3, 1, 60), (4, 1, 40), (5, 1, 60)])
-def test_config_traces_full_size_placement(ctx, idx, scale, epochs):
+# BASELINE.json's configs as written: full size, full epoch counts (20 / 200 / 200 x 3 / 100 / 500);
+# cfg 3 is three runs, the busy:idle ratio swept 1:3, 1:1, 3:1 (f_busy 0.25 / 0.5 / 0.75) "so the
+# partition boundary moves".
+@pytest.mark.parametrize("idx,f_busy,epochs", [(1, None, 20), (2, None, 200), (3, 0.25, 200), (3, 0.5, 200),
+                                               (3, 0.75, 200), (4, None, 100), (5, None, 500)])
+def test_config_traces_full_size_placement(ctx, idx, f_busy, epochs):
     """Placement on the configs' own traces at FULL size (placement needs no pools): every epoch
-    bit-exact; the sim advances on the oracle's placement."""
-    cfg = W.get_config(idx, scale)
-    for seed in (866, 867):
+    bit-exact; the sim advances on the oracle's placement.  Seed 866 runs every epoch BASELINE.json
+    asks for, seeds 867 / 868 the first 20."""
+    cfg = W.get_config(idx, 1, f_busy)
+    assert cfg.epochs == epochs
+    b_gpu_seen = set()
+    for seed in (866, 867, 868):
         sim = W.Sim(cfg, seed)
         for e in range(epochs if seed == 866 else min(epochs, 20)):
             plan = sim.begin_epoch()
@@ -122,5 +129,8 @@ def test_config_traces_full_size_placement(ctx, idx, scale, epochs):
             if idx == 1:
                 b = oracle.bruteforce_partition(plan.iota, plan.kv_pages, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
                 assert np.array_equal(b["tier"], got["tier"])
+            b_gpu_seen.add(int(got["bounds"][0]))
             sim.apply_placement(want["tier"], want["lists"])
             sim.end_epoch()
+    if idx in (2, 3, 4, 5):
+        assert len(b_gpu_seen) > 3, "the partition boundary never moved"

@@ -77,3 +77,54 @@ def test_argument_errors(ctx, mori):
     for caps in ([], [1] * 9, [3, -1]):
         with pytest.raises(mori.MoriError):
             ctx.mori_rank_partition_tiers(4, z, z, caps, z, z, z, z)
+
+
+@pytest.mark.parametrize("idx,scale,mid_frac,epochs", [(2, 64, 0.5, 30), (3, 128, 0.4, 20)])
+def test_three_tier_epochs_all_three_pools_byte_exact(mori, idx, scale, mid_frac, epochs):
+    """A whole epoch across three pools ("a second idleness threshold ... an intermediate
+    tier"): mori_rank_partition_tiers decides (tiers and both move lists bit-exact vs the oracle),
+    mori_demote / mori_promote of the three pair-contexts move the bytes (pool <-> device-resident
+    middle arena, pool <-> pinned host arena, middle <-> host), and after every epoch the GPU pool,
+    the middle arena and the host arena equal the oracle's three mirrors byte for byte."""
+    from paper_2606_00866_b200 import workload as W
+    from paper_2606_00866_b200.harness import TierRunner
+    from test_oracle_tiers_pins import oracle_apply_moves
+    cfg = W.get_config(idx, scale)
+    sh = cfg.shape
+    seed = 866
+    mid_ids = int(cfg.gpu_pool_pages * mid_frac)
+    pool_ids = [cfg.gpu_pool_pages, mid_ids, cfg.cpu_pool_pages]
+    caps = [cfg.cap_gpu_pages, max(0, mid_ids - cfg.max_program_pages // 2), cfg.cap_cpu_pages]
+    sim = W.SimTiers(cfg, seed, pool_ids, caps)
+    r = TierRunner(cfg, seed, mid_ids, staging_bytes=max(sh.page_bytes * 3, 1 << 20))
+    r.host.zero_()
+    pool_m = np.zeros(sh.n_layers * pool_ids[0] * sh.chunk_bytes, np.uint8)
+    mid_m = np.zeros(mid_ids * sh.page_bytes, np.uint8)
+    host_m = np.zeros(pool_ids[2] * sh.page_bytes, np.uint8)
+    pairs, moved = set(), 0
+    for e in range(epochs):
+        plan = sim.begin_epoch()
+        want = oracle.rank_partition_tiers(plan.iota, plan.kv_pages, caps, plan.prev_tier)
+        got = r.place(plan.iota, plan.kv_pages, plan.prev_tier, caps)
+        for k in ("order", "tier", "bounds", "used"):
+            assert np.array_equal(got[k], want[k]), (e, k)
+        for k in range(2):
+            assert np.array_equal(got["moves"][k], want["moves"][k]), (e, "moves", k)
+        sim.apply_placement(got["tier"], got["moves"])
+        r.execute(plan)
+        oracle_apply_moves(plan.ops, sh, pool_m, mid_m, host_m)
+        sim.end_epoch()
+        r.fill(plan.fills)
+        pv = pool_m.reshape(sh.n_layers, pool_ids[0], sh.chunk_bytes)
+        for uid, first, pages in plan.fills:
+            for j, g in enumerate(pages):
+                pv[:, g] = W.page_content(seed, uid, first + j, sh)
+        assert np.array_equal(r.pool.cpu().numpy(), pool_m), (e, "GPU pool")
+        assert np.array_equal(r.mid.cpu().numpy(), mid_m), (e, "middle arena")
+        assert np.array_equal(r.host.numpy(), host_m), (e, "host arena")
+        for op in plan.ops:
+            if op[0] == "move":
+                pairs.add((op[2], op[3]))
+                moved += len(op[4])
+    r.close()
+    assert moved > 0 and {(0, 1), (1, 0), (1, 2)} <= pairs, pairs
