@@ -126,14 +126,17 @@ def measure_link_peak(arena, nbytes=GIB, reps=5, stream_chunks=1):
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
             cur = torch.cuda.current_stream()
             e0 = torch.cuda.Event(enable_timing=True); e0.record(cur)
-            s1.wait_event(e0); s2.wait_event(e0)
-            if do_d2h:
+            if do_d2h and do_h2d:
+                s1.wait_event(e0); s2.wait_event(e0)
                 with torch.cuda.stream(s1):
                     h1.copy_(d1, non_blocking=True)
-            if do_h2d:
                 with torch.cuda.stream(s2):
                     d2.copy_(h2, non_blocking=True)
-            cur.wait_stream(s1); cur.wait_stream(s2)
+                cur.wait_stream(s1); cur.wait_stream(s2)
+            elif do_d2h:                                 # one direction: the copy alone between the two events
+                h1.copy_(d1, non_blocking=True)
+            else:
+                d2.copy_(h2, non_blocking=True)
             e1 = torch.cuda.Event(enable_timing=True); e1.record(cur)
             torch.cuda.synchronize()
             best = min(best, e0.elapsed_time(e1))
@@ -387,7 +390,7 @@ def link_report(st, link):
 
 
 def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, do_e2e=True,
-                   gather_reps=20, clocks_on=True, size_matched_leg=True):
+                   gather_reps=20, clocks_on=True, size_matched_leg=True, do_timeline=False):
     """K timed epochs of one config on the CUDA path (device-resident inputs), the same epochs again
     through the public API from host buffers, the in-step roofline of the gather/scatter kernel and
     the standalone device halves.  -> dict of raw totals and derived records."""
@@ -421,9 +424,12 @@ def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, 
             if sticky:                                             # NEXT-1 policy: status flags ride along
                 got = r.place_sticky(plan.iota, plan.kv_pages, plan.prev_tier, plan.flags, stream=cur)
             else:
-                got = r.place_resident(cur)                        # kernel + D2H of lists + sync
-            a1.record(cur)
+                got = r.place_resident(cur, done_event=a1)         # kernel (+ D2H of the lists), then sync
+            if sticky:
+                a1.record(cur)
             sim.apply_placement(got["tier"], got["lists"])         # harness allocator (untimed)
+            if timeline is not None:
+                r.mori.mori_profile(2)                             # time zero of this step's timeline
             b0.record(cur)
             r.mori.mori_after_stream(binding.BOTH, cur)
             r.execute(plan, sync=False)
@@ -431,7 +437,14 @@ def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, 
             b1.record(cur)
             r.mori.mori_sync(binding.BOTH)
             torch.cuda.synchronize()
-            ms = a0.elapsed_time(a1) + b0.elapsed_time(b1)
+            ms_a, ms_b = a0.elapsed_time(a1), b0.elapsed_time(b1)
+            ms = ms_a + ms_b
+            if timeline is not None:
+                timeline.append({"demote_bytes": plan.demote_pages * page_b, "promote_bytes": plan.promote_pages * page_b,
+                                 "region_b_ms": b0.elapsed_time(b1),
+                                 "rows": "kind 0 = gather/scatter kernel, 1 = one staging segment's DMAs; [kind, start_ms, end_ms, bytes]",
+                                 "demote": r.mori.mori_profile_timeline(binding.DEMOTE),
+                                 "promote": r.mori.mori_profile_timeline(binding.PROMOTE)})
         else:
             torch.cuda.synchronize()
             e0, e1 = ev(), ev()
@@ -449,13 +462,15 @@ def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, 
         sim.end_epoch()
         r.fill(plan.fills)                                          # stands in for prefill (untimed)
         n_tab = 8 * (plan.demote_pages + plan.promote_pages)        # page + slot ids, int32 each
-        return dict(ms=ms, ops=[(op[0][0], len(op[3])) for op in plan.ops if op[0] != "sync_all"],
+        return dict(ms=ms, ms_b=ms_b if mode == "dev" else None, ops=[(op[0][0], len(op[3])) for op in plan.ops if op[0] != "sync_all"],
                     dem=plan.demote_pages * page_b, pro=plan.promote_pages * page_b,
                     h2d=plan.promote_pages * page_b + 9 * n + n_tab,
                     d2h=plan.demote_pages * page_b + r.h_out.numel())
 
+    timeline = None
     for _ in range(warmup):
         epoch("dev")
+    timeline = [] if (do_timeline and getattr(args, "timeline", None)) else None
     # ---- timed: K steps, device-resident inputs ---------------------------------------------------
     r.mori.mori_profile(True)
     r.mori.mori_profile_read(binding.DEMOTE); r.mori.mori_profile_read(binding.PROMOTE)
@@ -471,6 +486,12 @@ def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, 
     prof = {"demote": r.mori.mori_profile_read(binding.DEMOTE),
             "promote": r.mori.mori_profile_read(binding.PROMOTE)}
     r.mori.mori_profile(False)
+    if timeline is not None:
+        with open(args.timeline, "w") as f:
+            json.dump({"workload": cfg.name, "how": "bench.py --timeline: CUDA events the library records around every "
+                       "kernel and every staging segment's DMAs, milliseconds since the start of the step's region B",
+                       "link_peaks_GBps": link, "steps": timeline}, f)
+        timeline = None
     if args.verbose:
         for i, x in enumerate(st):
             gb = (x["dem"] + x["pro"]) / 1e9
@@ -508,9 +529,13 @@ def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, 
         mean_b = max(4096, min(mean_b, arena.numel() // 2, 2 * GIB)) // 4096 * 4096
         sm = measure_link_peak(arena, nbytes=mean_b, reps=10)
         ach = sum(x["dem"] + x["pro"] for x in moving) / (sum(x["ms"] for x in moving) * 1e-3) / 1e9
+        ach_b = sum(x["dem"] + x["pro"] for x in moving) / (sum(x["ms_b"] for x in moving) * 1e-3) / 1e9
         out["size_matched"] = {"bytes": mean_b, "d2h_GBps": sm["d2h"], "h2d_GBps": sm["h2d"],
                                "epochs_GBps": ach, "epochs_over_d2h": ach / sm["d2h"],
-                               "note": "one-direction denominator: epochs that move both ways can exceed it"}
+                               "transfer_region_GBps": ach_b, "transfer_region_over_d2h": ach_b / sm["d2h"],
+                               "note": "one-direction denominator: epochs that move both ways can exceed it; "
+                                       "`epochs` = rank/partition + transfers, `transfer_region` = the demote/promote "
+                                       "calls up to the join only (what a plain memcpy of the same bytes competes with)"}
 
     # ---- roofline of the HBM-bound kernel, from the library's per-launch CUDA events ---------------
     ncu = _load_ncu_traffic()
@@ -562,7 +587,9 @@ def _per_config_record(m, link, scale):
     if m["size_matched"]:
         smx = m["size_matched"]
         rec["size_matched"] = {"bytes": smx["bytes"], "pinned_memcpy_GBps": smx["d2h_GBps"],
-                               "epochs_GBps": smx["epochs_GBps"], "frac": smx["epochs_over_d2h"]}
+                               "epochs_GBps": smx["epochs_GBps"], "frac": smx["epochs_over_d2h"],
+                               "transfer_region_GBps": smx["transfer_region_GBps"],
+                               "transfer_region_frac": smx["transfer_region_over_d2h"]}
     if m["roofline"]:
         rec["in_step_gather_scatter_frac_of_measured_hbm"] = m["roofline"]["frac"]
         rec["in_step_launches"] = m["roofline"]["launches"]
@@ -645,7 +672,8 @@ def run_ours(args):
     page_b = sh.page_bytes
 
     m = measure_config(args, cfg, seed, arena_full[:cfg.cpu_pool_pages * page_b], link, args.steps, args.warmup,
-                       local, barrier, do_e2e=True, gather_reps=0 if (args.no_gather_leg or rank != 0) else 20)
+                       local, barrier, do_e2e=True, gather_reps=0 if (args.no_gather_leg or rank != 0) else 20,
+                       do_timeline=(rank == 0))
     r = m["runner"]
     (t_dev, t_e2e), (b_dev, b_e2e, launches) = replicas.aggregate(
         [m["t_dev"], m["t_e2e"]], [m["b_dev"], m["b_e2e"], float(m["launches"])], device="cuda")
@@ -809,6 +837,104 @@ def gather_scatter_leg(r, sim, hbm_peak, min_bytes=4 * GIB, reps=20, warm=3):
     return out
 
 
+def copy_kernel_sweep(args):
+    """`--leg copy_sweep`: the gather/scatter kernel ALONE (1 / 2 / 4 GiB per launch) and IN-STEP (inside
+    a STAGED demotion, a STAGED promotion and both at once, i.e. next to the copy engines' DMA), for
+    the ring geometries, chunk hand-out and staging sizes that DESIGN.md section 7 discusses.  cfg-2
+    geometry on a 28 GiB pool and a 16 GiB pinned arena.  One JSON line: rows of fractions of the
+    measured HBM copy rate."""
+    import itertools
+    import torch
+    from paper_2606_00866_b200 import binding
+    L, H, D, T = 32, 8, 128, 16
+    page = L * 2 * H * T * D * 2
+    P, S = 14336, 8192
+    pool = torch.empty(P * page, dtype=torch.uint8, device="cuda")
+    pool.random_(0, 255)
+    arena = binding.Mori.mori_host_alloc(S * page)
+    peak, peak_src = _hbm_peak()
+    rng = np.random.default_rng(0)
+    cur = torch.cuda.current_stream()
+    variants = [(sched, piece, ctas, stg, "tma")
+                for sched, piece, ctas, stg in itertools.product((1, 0), (64, 32, 16), (1, 2), (1024, 2048))
+                if not (ctas == 2 and piece == 64) and not (sched == 0 and (ctas == 2 or piece != 64))]
+    variants += [(1, 64, 1, 1024, "ldst"), (1, 64, 1, 2048, "ldst")]
+    rows = []
+    for sched, piece, ctas, stg, kern in variants:
+        os.environ.update(MORI_SCHED=str(sched), MORI_PIECE_KIB=str(piece), MORI_CTAS_PER_SM=str(ctas))
+        m = binding.Mori(L, H, D, T, pool, arena, path_demote=2, path_promote=2,
+                         copy_kernel={"tma": 2, "ldst": 1}[kern], staging_bytes=stg << 20)
+        row = dict(kernel=kern, chunk_handout="dynamic" if sched else "static", piece_KiB=piece, ctas_per_sm=ctas,
+                   staging_MiB=stg)
+        for gib in (1, 2, 4):
+            n = gib * GIB // page
+            g = torch.from_numpy(rng.permutation(P)[:n].astype(np.int32)).cuda()
+            buf = torch.empty(n * page, dtype=torch.uint8, device="cuda")
+            ts = []
+            for _ in range(8):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(cur); m.mori_gather_pages(g, buf, stream=cur); e1.record(cur); torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            row[f"alone_{gib}GiB_us"] = 1e3 * float(np.median(ts[2:]))
+            row[f"alone_{gib}GiB_frac"] = 2 * n * page / (np.median(ts[2:]) * 1e-3) / 1e9 / peak
+            del buf
+        n = 6144                                                     # 12 GiB
+        for mode in ("demote", "promote", "both"):
+            g = rng.permutation(P)[:n].astype(np.int32)
+            g2 = np.setdiff1d(np.arange(P, dtype=np.int32), g)[:n]
+            h = np.arange(n, dtype=np.int32)
+            m.mori_profile(True); m.mori_profile_read(1); m.mori_profile_read(2)
+            if mode == "demote":
+                m.mori_demote(g, h)
+            elif mode == "promote":
+                m.mori_promote(h, g2)
+            else:
+                m.mori_demote(g[:n // 2], h[:n // 2]); m.mori_promote(h[n // 2:], g2[:n - n // 2])
+            m.mori_sync(3)
+            pd, pp = m.mori_profile_read(1), m.mori_profile_read(2)
+            ms, nl, nb = pd[0] + pp[0], pd[1] + pp[1], pd[2] + pp[2]
+            row[f"instep_{mode}_frac"] = 2 * nb / (ms * 1e-3) / 1e9 / peak
+            row[f"instep_{mode}_us_per_launch"] = 1e3 * ms / nl
+        m.close()
+        rows.append(row)
+    for k in ("MORI_SCHED", "MORI_PIECE_KIB", "MORI_CTAS_PER_SM"):
+        os.environ.pop(k, None)
+    binding.Mori.mori_host_free(arena)
+    print(json.dumps({"leg": "copy_sweep", "hbm_peak_GBps": peak, "peak_source": peak_src,
+                      "geometry": "cfg 2 (32 layers, 64 KiB chunks, 2 MiB pages), 28 GiB pool, 16 GiB pinned arena, "
+                                  "random page ids, consecutive slots", "rows": rows}))
+
+
+def launch_floor(m, cur, reps=200):
+    """The floor the latency-bound entry points are judged against: an EMPTY kernel (mori_noop)
+    launched through the same binding on the same stream -- device microseconds per call over `reps`
+    back-to-back launches, and host wall-clock of one launch + stream synchronize."""
+    import torch
+    for _ in range(10):
+        m.mori_noop(stream=cur)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(cur)
+    for _ in range(reps):
+        m.mori_noop(stream=cur)
+    e1.record(cur)
+    torch.cuda.synchronize()
+    wall = []
+    for _ in range(50):
+        t0 = time.perf_counter(); m.mori_noop(stream=cur); torch.cuda.synchronize(); wall.append(time.perf_counter() - t0)
+    return {"device_us_per_call": 1e3 * e0.elapsed_time(e1) / reps,
+            "host_launch_plus_sync_us": 1e6 * float(np.median(wall)),
+            "what": "mori_noop: an empty kernel through the same ctypes binding, same stream"}
+
+
+def _wall_us(call, reps=50):
+    import torch
+    ts = []
+    for _ in range(reps):
+        t0 = time.perf_counter(); call(); torch.cuda.synchronize(); ts.append(time.perf_counter() - t0)
+    return 1e6 * float(np.median(ts))
+
+
 def rank_partition_leg(with_oracle: bool, reps=200):
     """a1-a4 alone: device microseconds per call (CUDA events over `reps` back-to-back launches)
     and host wall-clock of one launch + sync, at cfg 2's n = 64 and cfg 5's n = 4096 (scores
@@ -820,7 +946,7 @@ def rank_partition_leg(with_oracle: bool, reps=200):
     m = binding.Mori(2, 2, 64, 16, pool, max_programs=4096)
     rng = np.random.default_rng(SEED)
     cur = torch.cuda.current_stream()
-    out = {}
+    out = {"floor": launch_floor(m, cur, reps)}
     for n in (64, 4096):
         iota = rng.lognormal(0.0, 1.0, n).astype(np.float32)
         kv = rng.integers(16, 513, n).astype(np.int32)
@@ -868,6 +994,7 @@ def rank_partition_leg(with_oracle: bool, reps=200):
         s1.record(cur)
         torch.cuda.synchronize()
         ent["sticky_device_us_per_call"] = 1e3 * s0.elapsed_time(s1) / reps
+        ent["sticky_host_launch_plus_sync_us"] = _wall_us(call_sticky)
         # NEXT-2: Eq. (1) on the device: one tick's events (one completed cycle for a quarter of
         # the programs) + evaluation of all n scores
         me = max(1, n // 4)
@@ -906,6 +1033,12 @@ def rank_partition_leg(with_oracle: bool, reps=200):
         b1.record(cur)
         torch.cuda.synchronize()
         ent["bfd_device_us_per_call"] = 1e3 * b0.elapsed_time(b1) / 50
+        ent["bfd_host_launch_plus_sync_us"] = _wall_us(call_bfd, 20)
+        fl_wall = out["floor"]["host_launch_plus_sync_us"]
+        ent["floor_us"] = fl_wall
+        ent["x_floor"] = {"rank_partition": ent["host_launch_plus_sync_us"] / fl_wall,
+                          "sticky": ent["sticky_host_launch_plus_sync_us"] / fl_wall,
+                          "bfd": ent["bfd_host_launch_plus_sync_us"] / fl_wall}
         if with_oracle:
             import oracle
             ts = []
@@ -957,6 +1090,22 @@ def eviction_leg(with_oracle: bool, n_pages=65536, n_programs=64, reps=50):
     e1.record(cur)
     torch.cuda.synchronize()
     out = {"n_pages": n_pages, "device_us_per_call": 1e3 * e0.elapsed_time(e1) / reps}
+    fl = launch_floor(m, cur)
+    out["host_launch_plus_sync_us"] = _wall_us(lambda: m.mori_eviction_order(binding.TIER_GPU, t_o, t_t, t_l, vic, nres, stream=cur))
+    out["floor_us"] = fl["host_launch_plus_sync_us"]
+    out["floor_device_us_per_call"] = fl["device_us_per_call"]
+    out["x_floor"] = out["host_launch_plus_sync_us"] / fl["host_launch_plus_sync_us"]
+    # full-range 32-bit counters (five radix passes instead of two)
+    t_l2 = torch.from_numpy(rng.integers(0, 2 ** 32, n_pages, dtype=np.uint64).astype(np.uint32).view(np.int32)).to(d)
+    for _ in range(3):
+        m.mori_eviction_order(binding.TIER_GPU, t_o, t_t, t_l2, vic, nres, stream=cur)
+    torch.cuda.synchronize()
+    e0.record(cur)
+    for _ in range(reps):
+        m.mori_eviction_order(binding.TIER_GPU, t_o, t_t, t_l2, vic, nres, stream=cur)
+    e1.record(cur)
+    torch.cuda.synchronize()
+    out["device_us_per_call_full_range_counters"] = 1e3 * e0.elapsed_time(e1) / reps
     if with_oracle:
         import oracle
         ts = []
@@ -992,11 +1141,18 @@ def main():
                     help="process-group backend for N > 1 (gloo + --device-index: exercise the N > 1 path on one GPU)")
     ap.add_argument("--device-index", type=int, default=-1, help="CUDA device to use instead of LOCAL_RANK")
     ap.add_argument("--verbose", action="store_true", help="per-step lines on stderr")
+    ap.add_argument("--timeline", default=None, metavar="FILE",
+                    help="write the per-stream event timeline of every timed step of the headline config to FILE (JSON)")
+    ap.add_argument("--leg", default=None, choices=["copy_sweep"],
+                    help="run one auxiliary measurement leg instead of the bench line (copy_sweep: the gather/scatter "
+                         "kernel alone and in-step for several ring geometries; profiles/ cites it)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gather-leg", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    if args.impl == "reference":
+    if args.leg == "copy_sweep":
+        copy_kernel_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -89,7 +89,8 @@ typedef struct {
   int32_t path_demote;       /* MORI_PATH_* */
   int32_t path_promote;      /* MORI_PATH_* */
   int32_t copy_kernel;       /* MORI_KERNEL_* */
-  int64_t staging_bytes;     /* per staging buffer (2 per direction); 0 -> 1 GiB */
+  int64_t staging_bytes;     /* per staging buffer (2 per direction); 0 -> 2 GiB when the device has
+                                >= 32 GiB free at mori_create, 1 GiB when >= 12 GiB, else 256 MiB */
   int64_t max_pages_per_call;/* 0 -> max(gpu_pool_pages, host_arena_slots) */
   int32_t zerocopy_ctas;     /* grid of a ZEROCOPY kernel (it is link-bound, a few CTAs saturate
                                 PCIe and the rest of the SMs stay free); 0 -> library default */
@@ -134,6 +135,10 @@ int mori_destroy(mori_ctx* ctx);
  *   used_pages   [2] out: pages held by the GPU tier, by the CPU tier
  *   lists        [5][n] out: row MORI_LIST_*; entries past list_counts[row] are unspecified
  *   list_counts  [5] out
+ * Every output array is written exactly once, by one CTA, and never read back, so the outputs
+ * (not the inputs) may also be PINNED host memory: the placement then lands in host memory with
+ * no copy, complete when `stream` has run the launch.  Worth it for small n (scattered 4-byte
+ * stores cross PCIe one by one); for thousands of programs one device-to-host copy is faster.
  */
 int mori_rank_partition(mori_ctx* ctx, void* stream, int32_t n, const float* idleness,
                         const int32_t* kv_pages, const uint8_t* prev_tier, int64_t gpu_cap_pages,
@@ -152,7 +157,8 @@ int mori_rank_partition(mori_ctx* ctx, void* stream, int32_t n, const float* idl
  *                          enqueued -> MORI_ERR_INVALID_ARG.
  *   wait_promote_ticket    0, or a ticket returned by mori_promote: no byte of this call is read
  *                          or written before that promote call has completed (device-side wait).
- *   ticket_out             NULL, or receives this call's ticket (> 0, increasing).
+ *   ticket_out             receives this call's ticket (> 0, increasing); NULL: no ticket is issued
+ *                          (and no event recorded) -- for calls nothing will ever wait on.
  * total_pages == 0 is a valid no-op that still yields a ticket.
  * Calls of one direction take effect in issue order (a later call that writes the same slots or
  * pages wins), whichever path each of them takes; the two directions are ordered only by tickets,
@@ -328,8 +334,18 @@ int mori_rank_partition_tiers(mori_ctx* ctx, void* stream, int32_t n, const floa
  * mori_demote / mori_promote is bracketed by CUDA events on its stream.  mori_profile_read
  * (call after mori_sync) returns and clears the totals for one direction. */
 int mori_profile(mori_ctx* ctx, int32_t enable);
+/* enable == 2 additionally keeps a TIMELINE: every kernel (kind 0) and every staging segment's run
+ * of DMAs (kind 1) of both directions as [start, end) in milliseconds since the mori_profile call,
+ * all on one clock -- the evidence of what overlaps what inside an epoch.  Read it after mori_sync;
+ * *n_rows receives the number of rows available (at most max_rows are copied out). */
+int mori_profile_timeline(mori_ctx* ctx, int32_t which, int64_t max_rows, int32_t* kind, double* start_ms,
+                          double* end_ms, int64_t* bytes, int64_t* n_rows);
 int mori_profile_read(mori_ctx* ctx, int32_t which, double* kernel_ms, int64_t* launches,
                       int64_t* bytes);
+
+/* Launches an EMPTY kernel on `stream`: the launch-latency floor that the latency-bound entry
+ * points (the rankers, the eviction order, the Waiting-queue packing) are reported against. */
+int mori_noop(mori_ctx* ctx, void* stream);
 
 /* Number of CUDA kernels this context has launched since mori_create (rank/partition, index
  * upload, gather/scatter/zero-copy kernels); copy-engine DMAs are not kernels and not counted. */

@@ -32,7 +32,7 @@ EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", 
            "mori_copy_kernel", "mori_last_error", "mori_launch_count", "mori_host_alloc",
            "mori_host_free", "mori_sticky_rebalance", "mori_idleness_update",
            "mori_idleness_eval", "mori_eviction_order", "mori_bfd_assign",
-           "mori_rank_partition_tiers"]
+           "mori_rank_partition_tiers", "mori_profile_timeline", "mori_noop"]
 
 
 class MoriConfig(C.Structure):
@@ -73,8 +73,8 @@ def load():
         L.mori_eviction_order.argtypes = [vp, vp, i32, i64, vp, i32, vp, vp, vp, vp]
         L.mori_idleness_update.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         L.mori_idleness_eval.argtypes = [vp, vp, i32, vp, vp, vp]
-        L.mori_demote.argtypes = [vp, i64, vp, vp, i64, C.POINTER(i64)]
-        L.mori_promote.argtypes = [vp, i64, vp, vp, i64, i64, C.POINTER(i64)]
+        L.mori_demote.argtypes = [vp, i64, vp, vp, i64, vp]
+        L.mori_promote.argtypes = [vp, i64, vp, vp, i64, i64, vp]
         L.mori_sync.argtypes = [vp, i32]
         L.mori_after_stream.argtypes = [vp, i32, vp]
         L.mori_stream_wait.argtypes = [vp, vp, i32]
@@ -82,6 +82,8 @@ def load():
         L.mori_scatter_pages.argtypes = [vp, vp, i64, vp, vp]
         L.mori_profile.argtypes = [vp, i32]
         L.mori_profile_read.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64), C.POINTER(i64)]
+        L.mori_profile_timeline.argtypes = [vp, i32, i64, vp, vp, vp, vp, C.POINTER(i64)]
+        L.mori_noop.argtypes = [vp, vp]
         L.mori_path.argtypes = [vp, i32]
         L.mori_copy_kernel.argtypes = [vp]
         L.mori_last_error.argtypes = [vp]
@@ -244,20 +246,23 @@ class Mori:
             _ptr(idleness_out)))
 
     # -- a5-a7 -------------------------------------------------------------------------------
-    def mori_demote(self, gpu_pages, host_slots, wait_promote_ticket=0) -> int:
+    def mori_demote(self, gpu_pages, host_slots, wait_promote_ticket=0, want_ticket=True) -> int:
+        """-> the call's ticket (0 with ``want_ticket=False``: ticket_out = NULL, no event is recorded)."""
         g, h = _host_i32(gpu_pages), _host_i32(host_slots)
         assert g.shape == h.shape and g.ndim == 1
         t = C.c_int64(0)
         self._ck(self._lib.mori_demote(self._h, g.size, g.ctypes.data, h.ctypes.data,
-                                       int(wait_promote_ticket), C.byref(t)))
+                                       int(wait_promote_ticket), C.byref(t) if want_ticket else None))
         return t.value
 
-    def mori_promote(self, host_slots, gpu_pages, pages_after_demote=0, slots_after_demote=0) -> int:
+    def mori_promote(self, host_slots, gpu_pages, pages_after_demote=0, slots_after_demote=0,
+                     want_ticket=True) -> int:
         g, h = _host_i32(gpu_pages), _host_i32(host_slots)
         assert g.shape == h.shape and g.ndim == 1
         t = C.c_int64(0)
         self._ck(self._lib.mori_promote(self._h, g.size, h.ctypes.data, g.ctypes.data,
-                                        int(pages_after_demote), int(slots_after_demote), C.byref(t)))
+                                        int(pages_after_demote), int(slots_after_demote),
+                                        C.byref(t) if want_ticket else None))
         return t.value
 
     def mori_sync(self, which=BOTH):
@@ -303,14 +308,27 @@ class Mori:
             return load().mori_host_free(p)
         return OK
 
+    def mori_noop(self, stream=None):
+        return self._ck(self._lib.mori_noop(self._h, _stream_handle(stream)))
+
     # -- profiling ---------------------------------------------------------------------------
     def mori_launch_count(self) -> int:
         n = C.c_int64(0)
         self._ck(self._lib.mori_launch_count(self._h, C.byref(n)))
         return n.value
 
-    def mori_profile(self, enable: bool):
+    def mori_profile(self, enable):
+        """False / True, or 2 to keep a timeline as well (``mori_profile_timeline``)."""
         return self._ck(self._lib.mori_profile(self._h, int(enable)))
+
+    def mori_profile_timeline(self, which):
+        """-> list of (kind, start_ms, end_ms, bytes): kind 0 = kernel, 1 = a segment's DMAs."""
+        n = C.c_int64(0)
+        self._ck(self._lib.mori_profile_timeline(self._h, which, 0, None, None, None, None, C.byref(n)))
+        k = np.zeros(n.value, np.int32); t0 = np.zeros(n.value); t1 = np.zeros(n.value); b = np.zeros(n.value, np.int64)
+        self._ck(self._lib.mori_profile_timeline(self._h, which, n.value, k.ctypes.data, t0.ctypes.data,
+                                                 t1.ctypes.data, b.ctypes.data, C.byref(n)))
+        return [(int(k[i]), float(t0[i]), float(t1[i]), int(b[i])) for i in range(n.value)]
 
     def mori_profile_read(self, which):
         ms, n, b = C.c_double(0), C.c_int64(0), C.c_int64(0)

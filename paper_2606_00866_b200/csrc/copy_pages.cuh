@@ -271,12 +271,13 @@ __host__ __device__ inline size_t tma_smem_bytes(int stages, int piece_bytes) {
 // a few pages spread over many SMs (the move is latency-bound: what matters is requests in
 // flight on the link, not per-SM efficiency).
 // ------------------------------------------------------------------------------------------
-constexpr int kSmallMaxPages = 448;
+constexpr int kSmallMaxPages = 448;                                 // 3.5 KiB of ids: the 4 KiB parameter space
+constexpr int kSmallFewPages = 64;                                  // a shorter parameter block launches faster
 constexpr int kSmallPiece = kLdstThreads * 16;
-struct SmallIds { int32_t gpu[kSmallMaxPages]; int32_t lin[kSmallMaxPages]; };
+template <int kCap> struct SmallIds { int32_t gpu[kCap]; int32_t lin[kCap]; };
 
-template <bool kGather>
-__global__ void __launch_bounds__(kLdstThreads) copy_pages_small(const CopyArgs a, const SmallIds ids) {
+template <bool kGather, int kCap>
+__global__ void __launch_bounds__(kLdstThreads) copy_pages_small(const CopyArgs a, const SmallIds<kCap> ids) {
   const int ppc = a.pieces_per_chunk;                               // pieces of kSmallPiece bytes
   const int per_page = a.n_layers * ppc;
   const int n_pieces = (int)a.n_pages * per_page;

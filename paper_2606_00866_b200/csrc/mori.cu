@@ -41,10 +41,12 @@ constexpr int kPieceBytesDefault = 64 * 1024;   // bytes per bulk copy = stage s
 constexpr int kRingBytesDefault = 192 * 1024;   // shared memory the rings of one SM's CTAs may take
 constexpr int kMaxTmaStages = 24;
 constexpr long long kAutoMinRunBytes = 6LL << 20;   // AUTO: below this mean slot-run length, ZEROCOPY
+constexpr long long kRampBytes = 256LL << 20;        // STAGED: size of a call's first (demote) / last (promote) segment
 constexpr long long kSmallMaxBytes = 4LL << 20;     // calls up to this size (and kSmallMaxPages) take the one-launch path
 
 // Tuning overrides for experiments (read once per mori_create): MORI_PIECE_KIB, MORI_RING_KIB,
-// MORI_CTAS_PER_SM, MORI_SCHED (0 static, 1 dynamic), MORI_STAGING_MIB.  Unset = the defaults.
+// MORI_CTAS_PER_SM, MORI_SCHED (0 static, 1 dynamic), MORI_STAGING_MIB, MORI_EVICT_MULTI (1: the
+// general multi-kernel eviction sort at every size).  Unset = the defaults.
 long long env_ll(const char* name, long long dflt) {
   const char* v = std::getenv(name);
   if (!v || !*v) return dflt;
@@ -53,7 +55,8 @@ long long env_ll(const char* name, long long dflt) {
   return end && *end == 0 ? x : dflt;
 }
 
-struct ProfSpan { cudaEvent_t a, b; long long bytes; };
+struct ProfSpan { cudaEvent_t a, b; long long bytes; int kind; };   // kind 0: gather/scatter/zero-copy kernel, 1: DMA segment
+struct TimelineRow { int kind; double t0_ms, t1_ms; long long bytes; };
 
 struct Direction {
   int path = 0;
@@ -69,6 +72,7 @@ struct Direction {
   std::vector<cudaEvent_t> tickets;              // ring
   long long next_ticket = 1;
   std::vector<ProfSpan> spans;
+  std::vector<TimelineRow> timeline;            // mori_profile(ctx, 2): every span, on one clock
   double prof_ms = 0; long long prof_launches = 0, prof_bytes = 0;
 };
 
@@ -99,10 +103,12 @@ struct mori_ctx {
   struct EvictKey { int n_programs; long long n_pages; const void *owner, *ptier, *last; void *victims, *nres; } evict_key[2]{};
   unsigned int* evict_max_last = nullptr;
   int32_t* evict_perm[2] = {nullptr, nullptr}; int32_t* evict_table = nullptr; long long evict_cap = 0;   // scratch, grown on demand
+  bool evict_multi_kernel = false;               // MORI_EVICT_MULTI=1: force the general (multi-kernel) sort
   int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
   Direction dir[2];                              // 0 demote, 1 promote
   std::vector<cudaEvent_t> free_events;
   bool profiling = false;
+  bool timeline = false; cudaEvent_t prof_base = nullptr;   // mori_profile(ctx, 2)
   mutable long long launches = 0;                // kernels launched by this context
   int sticky = MORI_OK;
   mutable std::string err;
@@ -191,10 +197,10 @@ cudaError_t launch_copy(const mori_ctx* c, const mori::CopyArgs& a, cudaStream_t
 
 // The one-launch path of a small move: ids by value in the kernel parameters, LD/ST straight
 // between the pool and the (mapped or device) arena.
-template <bool kGather>
-cudaError_t launch_small(const mori_ctx* c, long long n, const int32_t* gpu_pages, const int32_t* host_slots,
-                         cudaStream_t s) {
-  mori::SmallIds ids;
+template <bool kGather, int kCap>
+cudaError_t launch_small_cap(const mori_ctx* c, long long n, const int32_t* gpu_pages, const int32_t* host_slots,
+                             cudaStream_t s) {
+  mori::SmallIds<kCap> ids;
   std::memcpy(ids.gpu, gpu_pages, sizeof(int32_t) * n);
   std::memcpy(ids.lin, host_slots, sizeof(int32_t) * n);
   mori::CopyArgs a = make_args(c, c->arena_dev, nullptr, nullptr, n);
@@ -202,8 +208,14 @@ cudaError_t launch_small(const mori_ctx* c, long long n, const int32_t* gpu_page
   const long long n_pieces = n * a.n_layers * a.pieces_per_chunk;
   const int grid = (int)std::min<long long>(n_pieces, (long long)c->sm_count * 4);
   c->launches += 1;
-  mori::copy_pages_small<kGather><<<grid, mori::kLdstThreads, 0, s>>>(a, ids);
+  mori::copy_pages_small<kGather, kCap><<<grid, mori::kLdstThreads, 0, s>>>(a, ids);
   return cudaGetLastError();
+}
+template <bool kGather>
+cudaError_t launch_small(const mori_ctx* c, long long n, const int32_t* gpu_pages, const int32_t* host_slots,
+                         cudaStream_t s) {
+  return n <= mori::kSmallFewPages ? launch_small_cap<kGather, mori::kSmallFewPages>(c, n, gpu_pages, host_slots, s)
+                                   : launch_small_cap<kGather, mori::kSmallMaxPages>(c, n, gpu_pages, host_slots, s);
 }
 
 // nullptr (and a latched MORI_ERR_CUDA) when the driver cannot create an event.
@@ -279,32 +291,37 @@ int wait_ticket(mori_ctx* c, Direction& other, long long ticket, cudaStream_t s)
 }
 
 int issue_ticket(mori_ctx* c, Direction& d, cudaStream_t s, int64_t* out) {
+  if (!out) return MORI_OK;                       // nobody will wait on it: no event, no number
   const long long t = d.next_ticket++;
   CK(c, cudaEventRecord(d.tickets[t % kTicketRing], s));
   if (out) *out = t;
   return MORI_OK;
 }
 
-void prof_begin(mori_ctx* c, Direction& d, cudaStream_t s, long long bytes) {
-  if (!c->profiling) return;
-  ProfSpan sp{get_event(c, true), get_event(c, true), bytes};
+void prof_begin(mori_ctx* c, Direction& d, cudaStream_t s, long long bytes, int kind = 0) {
+  if (!c->profiling || (kind != 0 && !c->timeline)) return;
+  ProfSpan sp{get_event(c, true), get_event(c, true), bytes, kind};
   if (!sp.a || !sp.b) { if (sp.a) cudaEventDestroy(sp.a); if (sp.b) cudaEventDestroy(sp.b); sp.a = sp.b = nullptr; }
   if (sp.a) cudaEventRecord(sp.a, s);
   d.spans.push_back(sp);
 }
-void prof_end(mori_ctx* c, Direction& d, cudaStream_t s) {
-  if (!c->profiling || d.spans.empty() || !d.spans.back().b) return;
+void prof_end(mori_ctx* c, Direction& d, cudaStream_t s, int kind = 0) {
+  if (!c->profiling || (kind != 0 && !c->timeline) || d.spans.empty() || !d.spans.back().b) return;
   cudaEventRecord(d.spans.back().b, s);
 }
-void prof_collect(Direction& d) {
+void prof_collect(mori_ctx* c, Direction& d) {
   for (auto& sp : d.spans) {
     float ms = 0;
     if (!sp.a) continue;
     if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) {
-      d.prof_ms += ms; d.prof_launches += 1; d.prof_bytes += sp.bytes;
+      if (sp.kind == 0) { d.prof_ms += ms; d.prof_launches += 1; d.prof_bytes += sp.bytes; }
+      float t0 = 0;
+      if (c && c->timeline && c->prof_base && cudaEventElapsedTime(&t0, c->prof_base, sp.a) == cudaSuccess)
+        d.timeline.push_back({sp.kind, (double)t0, (double)t0 + ms, sp.bytes});
     }
     cudaEventDestroy(sp.a); cudaEventDestroy(sp.b);
   }
+  cudaGetLastError();
   d.spans.clear();
 }
 
@@ -326,14 +343,14 @@ template <int IPT>
 cudaError_t launch_rank_multi(int grid, size_t smem, cudaStream_t s, int n, const float* idl, const int32_t* kv,
                               const uint8_t* prev, long long cg, long long cc, int32_t* order, uint8_t* tier,
                               int32_t* bounds, long long* used, int32_t* lists, int32_t* counts,
-                              unsigned int* ticket) {
+                              int32_t* scratch_order, unsigned int* ticket) {
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(mori::rank_partition_multi_kernel<IPT>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
   mori::rank_partition_multi_kernel<IPT><<<grid, mori::kRankMaxThreads, smem, s>>>(
-      n, idl, kv, prev, cg, cc, order, tier, bounds, used, lists, counts, ticket);
+      n, idl, kv, prev, cg, cc, order, tier, bounds, used, lists, counts, scratch_order, ticket);
   return cudaGetLastError();
 }
 
@@ -341,14 +358,14 @@ template <int IPT>
 cudaError_t launch_tiers(int grid, size_t smem, cudaStream_t s, int n, const float* idl, const int32_t* kv,
                          const mori::TierCaps& caps, const uint8_t* prev, int32_t* order, uint8_t* tier,
                          int32_t* bounds, long long* used, int32_t* moves, int32_t* move_counts,
-                         unsigned int* ticket) {
+                         int32_t* scratch_order, unsigned int* ticket) {
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(mori::rank_tiers_kernel<IPT>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
   mori::rank_tiers_kernel<IPT><<<grid, mori::kRankMaxThreads, smem, s>>>(n, idl, kv, caps, prev, order, tier, bounds,
-                                                                        used, moves, move_counts, ticket);
+                                                                        used, moves, move_counts, scratch_order, ticket);
   return cudaGetLastError();
 }
 
@@ -427,9 +444,24 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
     return fail(nullptr, MORI_ERR_INVALID_ARG, "copy-kernel ring does not fit shared memory (chunk too large for 2 stages)");
   }
   c->debug = env_ll("MORI_DEBUG", 0) != 0;
+  c->evict_multi_kernel = env_ll("MORI_EVICT_MULTI", 0) != 0;
   c->max_pages = cfg->max_pages_per_call ? cfg->max_pages_per_call
                                           : std::max<long long>(cfg->gpu_pool_pages, cfg->host_arena_slots);
-  c->staging_bytes = cfg->staging_bytes ? cfg->staging_bytes : (env_ll("MORI_STAGING_MIB", 1024) << 20);
+  // Staging: the gather / scatter kernels run one launch per segment, and a launch pays ~15 us of
+  // ramp and tail whatever its size, so segments are as large as HBM comfortably allows: 2 GiB
+  // (4 buffers = 8 GiB; in-step 0.99 of the measured HBM copy rate) when >= 32 GiB are free, 1 GiB
+  // (0.93) when >= 12 GiB are, else 256 MiB.  DESIGN.md section 7.
+  long long staging_default = 256LL << 20;
+  {
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+      if (free_b >= (32ULL << 30)) staging_default = 2048LL << 20;
+      else if (free_b >= (12ULL << 30)) staging_default = 1024LL << 20;
+    } else {
+      cudaGetLastError();
+    }
+  }
+  c->staging_bytes = cfg->staging_bytes ? cfg->staging_bytes : (env_ll("MORI_STAGING_MIB", staging_default >> 20) << 20);
   c->staging_bytes = std::min(c->staging_bytes, c->max_pages * c->page_bytes);   // never more than one call can fill
   c->staging_bytes = std::max(c->staging_bytes, c->page_bytes);
   c->staging_bytes -= c->staging_bytes % c->page_bytes;
@@ -519,7 +551,7 @@ int mori_destroy(mori_ctx* c) {
   cudaDeviceSynchronize();
   for (int i = 0; i < 2; ++i) {
     Direction& d = c->dir[i];
-    prof_collect(d);
+    prof_collect(c, d);
     for (int b = 0; b < 2; ++b) {
       if (d.staging[b]) cudaFree(d.staging[b]);
       if (d.kern_done[b]) cudaEventDestroy(d.kern_done[b]);
@@ -532,6 +564,7 @@ int mori_destroy(mori_ctx* c) {
     if (d.copy) cudaStreamDestroy(d.copy);
   }
   for (auto ev : c->free_events) cudaEventDestroy(ev);
+  if (c->prof_base) cudaEventDestroy(c->prof_base);
   if (c->rank_tickets) cudaFree(c->rank_tickets);
   if (c->sched) cudaFree(c->sched);
   if (c->dbg_bitmap) cudaFree(c->dbg_bitmap);
@@ -567,11 +600,13 @@ int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idlen
     // more than one CTA's worth: rank by counting on every SM, last CTA partitions
     const int grid = std::min(c->sm_count, (n + 31) / 32);
     const size_t smem_m = sizeof(uint64_t) * ((size_t)n + 33) + 2 * sizeof(long long);
-    unsigned int* tk = c->rank_tickets + (c->rank_seq++ % kRankTickets);
+    const unsigned long long slot_m = c->rank_seq++ % kRankTickets;
+    unsigned int* tk = c->rank_tickets + slot_m;
+    int32_t* so = c->sticky_order + slot_m * (size_t)c->cfg.max_programs;
     cudaStream_t sm = static_cast<cudaStream_t>(stream);
     long long* um = reinterpret_cast<long long*>(used);
     cudaError_t em;
-#define LM(I) launch_rank_multi<I>(grid, smem_m, sm, n, idleness, kv_pages, prev_tier, gpu_cap, cpu_cap, order, tier, bounds, um, lists, counts, tk)
+#define LM(I) launch_rank_multi<I>(grid, smem_m, sm, n, idleness, kv_pages, prev_tier, gpu_cap, cpu_cap, order, tier, bounds, um, lists, counts, so, tk)
     switch (ipt) {
       case 2: em = LM(2); break;
       case 4: em = LM(4); break;
@@ -644,11 +679,13 @@ int mori_rank_partition_tiers(mori_ctx* c, void* stream, int32_t n, const float*
   while (n_pad < n) n_pad <<= 1;
   const int grid = std::max(1, std::min(c->sm_count, (n + 31) / 32));
   const size_t smem = sizeof(uint64_t) * ((size_t)n + 33) + 2 * sizeof(long long);
-  unsigned int* tk = c->rank_tickets + (c->rank_seq++ % kRankTickets);
+  const unsigned long long slot_t = c->rank_seq++ % kRankTickets;
+  unsigned int* tk = c->rank_tickets + slot_t;
+  int32_t* so = c->sticky_order + slot_t * (size_t)c->cfg.max_programs;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   long long* u = reinterpret_cast<long long*>(used);
   cudaError_t e;
-#define LT(I) launch_tiers<I>(grid, smem, s, n, idleness, kv_pages, caps, prev_tier, order, tier, bounds, u, moves, move_counts, tk)
+#define LT(I) launch_tiers<I>(grid, smem, s, n, idleness, kv_pages, caps, prev_tier, order, tier, bounds, u, moves, move_counts, so, tk)
   switch (n_pad / 1024) {
     case 1: e = LT(1); break;
     case 2: e = LT(2); break;
@@ -704,11 +741,25 @@ int mori_eviction_order(mori_ctx* c, void* stream, int32_t which_tier, int64_t n
     for (int b = 0; b < 2; ++b) { if (c->evict_perm[b]) cudaFree(c->evict_perm[b]); c->evict_perm[b] = nullptr; }
     if (c->evict_table) cudaFree(c->evict_table);
     c->evict_table = nullptr; c->evict_cap = 0;
-    for (int b = 0; b < 2; ++b) CK(c, cudaMalloc((void**)&c->evict_perm[b], sizeof(int32_t) * (size_t)n_pages));
+    for (int b = 0; b < 2; ++b) CK(c, cudaMalloc((void**)&c->evict_perm[b], sizeof(uint64_t) * (size_t)n_pages));   // int32 order, or 64-bit items
     CK(c, cudaMalloc((void**)&c->evict_table, sizeof(int32_t) * 256 * (size_t)tiles));
     c->evict_cap = n_pages;
   }
   mori::EvictArgs a{n_pages, n_programs, which_tier == MORI_TIER_GPU ? 0 : 1, tiles, page_owner, program_tier, last_access};
+  if (n_pages <= mori::kEvictClusterMaxPages && !c->evict_multi_kernel) {
+    // every BASELINE.json pool: ONE launch, a cluster of 8 CTAs, passes separated by cluster barriers
+    const long long seg = ((n_pages + mori::kEvictCluster - 1) / mori::kEvictCluster + 1023) / 1024 * 1024;
+    const int rounds = (int)(seg / 1024);
+    uint64_t* b0 = reinterpret_cast<uint64_t*>(c->evict_perm[0]);
+    uint64_t* b1 = reinterpret_cast<uint64_t*>(c->evict_perm[1]);
+    if (rounds <= 2) mori::evict_order_cluster_kernel<2><<<mori::kEvictCluster, 1024, 0, s>>>(a, b0, b1, victims, n_resident);
+    else if (rounds <= 4) mori::evict_order_cluster_kernel<4><<<mori::kEvictCluster, 1024, 0, s>>>(a, b0, b1, victims, n_resident);
+    else if (rounds <= 8) mori::evict_order_cluster_kernel<8><<<mori::kEvictCluster, 1024, 0, s>>>(a, b0, b1, victims, n_resident);
+    else mori::evict_order_cluster_kernel<16><<<mori::kEvictCluster, 1024, 0, s>>>(a, b0, b1, victims, n_resident);
+    CK(c, cudaGetLastError());
+    c->launches += 1;
+    return MORI_OK;
+  }
   auto enqueue = [&](cudaStream_t q) -> cudaError_t {
     cudaError_t e = cudaMemsetAsync(n_resident, 0, sizeof(int32_t), q);
     if (e != cudaSuccess) return e;
@@ -921,8 +972,14 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
   if (total > 0)
     if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;
   if (total > 0) d.copy_busy = true;
-  for (long long a0 = 0; a0 < total; a0 += seg_pages) {
-    const long long cnt = std::min(seg_pages, total - a0);
+  // The pipeline's ramp: a demotion's first DMA waits for its first gather and a promotion's last
+  // scatter runs after its last DMA, so those two segments are short (<= 256 MiB: ~0.1 ms of kernel
+  // instead of ~0.7 ms for a 2 GiB segment); every other kernel hides under a DMA.
+  const long long ramp_pages = std::max<long long>(1, std::min<long long>(seg_pages, kRampBytes / pb));
+  for (long long a0 = 0, cnt = 0; a0 < total; a0 += cnt) {
+    cnt = std::min(seg_pages, total - a0);
+    if (demote && a0 == 0 && total > 2 * ramp_pages) cnt = std::min(cnt, ramp_pages);
+    if (!demote && total - a0 == cnt && cnt > 2 * ramp_pages) cnt -= ramp_pages;
     const int b = d.buf; d.buf ^= 1;
     unsigned char* stg = d.staging[b];
     mori::CopyArgs a = make_args(c, stg, dg + a0, nullptr, cnt);
@@ -944,11 +1001,15 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
       prof_end(c, d, d.kern);
       CK(c, cudaEventRecord(d.kern_done[b], d.kern));
       CK(c, cudaStreamWaitEvent(d.copy, d.kern_done[b], 0));
+      prof_begin(c, d, d.copy, cnt * pb, 1);
       if (int rc = dma(d.copy)) return rc;
+      prof_end(c, d, d.copy, 1);
       CK(c, cudaEventRecord(d.copy_done[b], d.copy));
     } else {
       CK(c, cudaStreamWaitEvent(d.copy, d.kern_done[b], 0));       // staging[b] scattered
+      prof_begin(c, d, d.copy, cnt * pb, 1);
       if (int rc = dma(d.copy)) return rc;
+      prof_end(c, d, d.copy, 1);
       CK(c, cudaEventRecord(d.copy_done[b], d.copy));
       CK(c, cudaStreamWaitEvent(d.kern, d.copy_done[b], 0));
       prof_begin(c, d, d.kern, cnt * pb);
@@ -961,11 +1022,7 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
   if (demote) {
     // copy stream finishes last; it already follows the kernel stream, so one event on it covers
     // the call
-    cudaEvent_t ev = d.tickets[d.next_ticket % kTicketRing];
-    const long long t = d.next_ticket++;
-    CK(c, cudaEventRecord(ev, d.copy));
-    if (ticket_out) *ticket_out = t;
-    return MORI_OK;
+    return issue_ticket(c, d, d.copy, ticket_out);
   }
   // promote: the kernel stream finishes last; an EMPTY call has put nothing on it that follows the
   // copy stream's wait for wait_arena, so fold that in for the ticket to cover both waits
@@ -998,7 +1055,7 @@ int mori_sync(mori_ctx* c, int32_t which) {
     }
     d.idx_used = 0;
     d.copy_busy = false;
-    prof_collect(d);
+    prof_collect(c, d);
   }
   return c->sticky;
 }
@@ -1037,6 +1094,27 @@ int mori_stream_wait(mori_ctx* c, void* stream, int32_t which) {
 int mori_profile(mori_ctx* c, int32_t enable) {
   if (!c) return MORI_ERR_INVALID_ARG;
   c->profiling = enable != 0;
+  c->timeline = enable == 2;
+  if (c->timeline) {
+    if (!c->prof_base) CK(c, cudaEventCreate(&c->prof_base));
+    CK(c, cudaEventRecord(c->prof_base, c->dir[0].kern));           // time zero of the timeline
+    CK(c, cudaEventSynchronize(c->prof_base));
+    for (int i = 0; i < 2; ++i) c->dir[i].timeline.clear();
+  }
+  return MORI_OK;
+}
+
+int mori_profile_timeline(mori_ctx* c, int32_t which, int64_t max_rows, int32_t* kind, double* start_ms,
+                          double* end_ms, int64_t* bytes, int64_t* n_rows) {
+  if (!c || (which != MORI_DEMOTE && which != MORI_PROMOTE) || !n_rows || max_rows < 0) return MORI_ERR_INVALID_ARG;
+  const auto& tl = c->dir[which - 1].timeline;
+  *n_rows = (int64_t)tl.size();
+  for (int64_t i = 0; i < std::min<int64_t>(max_rows, (int64_t)tl.size()); ++i) {
+    if (kind) kind[i] = tl[i].kind;
+    if (start_ms) start_ms[i] = tl[i].t0_ms;
+    if (end_ms) end_ms[i] = tl[i].t1_ms;
+    if (bytes) bytes[i] = tl[i].bytes;
+  }
   return MORI_OK;
 }
 
@@ -1047,6 +1125,17 @@ int mori_profile_read(mori_ctx* c, int32_t which, double* ms, int64_t* launches,
   if (launches) *launches = d.prof_launches;
   if (bytes) *bytes = d.prof_bytes;
   d.prof_ms = 0; d.prof_launches = 0; d.prof_bytes = 0;
+  return MORI_OK;
+}
+
+__global__ void noop_kernel() {}
+
+int mori_noop(mori_ctx* c, void* stream) {
+  if (!c) return MORI_ERR_INVALID_ARG;
+  if (c->sticky) return c->sticky;
+  noop_kernel<<<1, 32, 0, static_cast<cudaStream_t>(stream)>>>();
+  CK(c, cudaGetLastError());
+  c->launches += 1;
   return MORI_OK;
 }
 

@@ -277,7 +277,8 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
                             long long cap_gpu, long long cap_cpu, int32_t* __restrict__ order,
                             uint8_t* __restrict__ tier, int32_t* __restrict__ bounds,
                             long long* __restrict__ used, int32_t* __restrict__ lists,
-                            int32_t* __restrict__ list_counts, unsigned int* __restrict__ ticket) {
+                            int32_t* __restrict__ list_counts, int32_t* __restrict__ scratch_order,
+                            unsigned int* __restrict__ ticket) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
   uint64_t* warp_tot = keys + n;                                     // [33]
@@ -286,13 +287,15 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
   for (int i = tid; i < n; i += blockDim.x)
     keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;
   __syncthreads();
-  if (!rank_by_counting(n, [&](int j, int i) { return keys[j] < keys[i]; }, order, ticket)) return;
+  // the CTAs exchange the order through library-owned DEVICE scratch; the caller's arrays are
+  // written once, by the last CTA -- so they may be mapped host memory
+  if (!rank_by_counting(n, [&](int j, int i) { return keys[j] < keys[i]; }, scratch_order, ticket)) return;
 
   int prog[IPT];
 #pragma unroll
   for (int i = 0; i < IPT; ++i) {
     const int r = tid * IPT + i;
-    prog[i] = r < n ? __ldcg(order + r) : -1;        // written by other CTAs: read through L2
+    prog[i] = r < n ? __ldcg(scratch_order + r) : -1;   // written by other CTAs: read through L2
   }
   partition_tail<IPT>(n, prog, kv_pages, prev_tier, cap_gpu, cap_cpu, order, tier, bounds, used, lists,
                       list_counts, warp_tot, bcast);
@@ -312,7 +315,7 @@ rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __re
                   const TierCaps caps, const uint8_t* __restrict__ prev_tier, int32_t* __restrict__ order,
                   uint8_t* __restrict__ tier, int32_t* __restrict__ bounds, long long* __restrict__ used,
                   int32_t* __restrict__ moves, int32_t* __restrict__ move_counts,
-                  unsigned int* __restrict__ ticket) {
+                  int32_t* __restrict__ scratch_order, unsigned int* __restrict__ ticket) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
   uint64_t* warp_tot = keys + n;                                     // [33]
@@ -321,7 +324,7 @@ rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __re
   for (int i = tid; i < n; i += blockDim.x)
     keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;
   __syncthreads();
-  if (!rank_by_counting(n, [&](int j, int i) { return keys[j] < keys[i]; }, order, ticket)) return;
+  if (!rank_by_counting(n, [&](int j, int i) { return keys[j] < keys[i]; }, scratch_order, ticket)) return;
 
   int prog[IPT];
   long long incl[IPT];
@@ -329,7 +332,8 @@ rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __re
 #pragma unroll
   for (int i = 0; i < IPT; ++i) {
     const int r = tid * IPT + i;
-    prog[i] = r < n ? __ldcg(order + r) : -1;
+    prog[i] = r < n ? __ldcg(scratch_order + r) : -1;
+    if (r < n) order[r] = prog[i];                                   // the caller's array: written once, here
     const int s = r < n ? kv_pages[prog[i]] : 0;
     incl[i] = s > 0 ? s : 0;
     tsum += incl[i];

@@ -16,8 +16,8 @@
 // memory, one warp per program); the last CTA to finish (atomic ticket) cuts the victim prefix
 // ("usage minus what the earlier victims free still exceeds the capacity" is monotone) and the
 // candidate prefix ("inclusive size sum fits the free capacity" is monotone) with block scans.
-// The only sequential step is the paper's per-victim "CPU if it fits, else Waiting", walked by
-// one thread over the victims' sizes in shared memory, and skipped when all of them fit.
+// The only sequential step is the paper's per-victim "CPU if it fits, else Waiting": skipped when
+// all of them fit, else walked by one warp, 32 victims per round (the room only shrinks).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -125,25 +125,42 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
 #pragma unroll
     for (int i = 0; i < IPT; ++i) if (victim[i]) vdest[tid * IPT + i] = 1;
     if (tid == 0) bcast[0] = usage_cpu0 + freed;
-  } else if (tid == 0) {
-    // the loop-carried part is one add and one compare; the sizes are read four ahead so that the
-    // shared-memory latency is off that chain
+  } else if (tid < 32) {
+    // The paper's walk is sequential ("each victim, in that order, goes to the CPU queue if it
+    // still fits"), but the room only ever shrinks, which one warp exploits 32 victims at a time:
+    //   (1) a victim larger than the room that is left can never fit -> Waiting, whatever precedes it;
+    //   (2) of the others, in order, the longest prefix whose summed size fits is taken at once;
+    //   (3) the one right after that prefix is then larger than the new room -> step (1) again.
+    // Every round decides at least one victim of the chunk and usually all 32.
+    const int lane = tid;
     long long room = cap_cpu - usage_cpu0;
-    int k = 0;
-    for (; k + 4 <= v; k += 4) {
-      const int s0 = vsize[k], s1 = vsize[k + 1], s2 = vsize[k + 2], s3 = vsize[k + 3];
-      const bool f0 = s0 <= room; room -= f0 ? s0 : 0;
-      const bool f1 = s1 <= room; room -= f1 ? s1 : 0;
-      const bool f2 = s2 <= room; room -= f2 ? s2 : 0;
-      const bool f3 = s3 <= room; room -= f3 ? s3 : 0;
-      vdest[k] = f0 ? 1 : 2; vdest[k + 1] = f1 ? 1 : 2; vdest[k + 2] = f2 ? 1 : 2; vdest[k + 3] = f3 ? 1 : 2;
+    for (int k0 = 0; k0 < v; k0 += 32) {
+      const int k = k0 + lane;
+      const long long s = k < v ? (long long)vsize[k] : 0;
+      unsigned undecided = __ballot_sync(0xFFFFFFFFu, k < v);
+      int dest = 0;
+      while (undecided) {
+        const bool mine = (undecided >> lane) & 1u;
+        const unsigned miss = __ballot_sync(0xFFFFFFFFu, mine && s > room);
+        if ((miss >> lane) & 1u) dest = 2;
+        undecided &= ~miss;
+        if (!undecided) break;
+        const bool still = (undecided >> lane) & 1u;
+        long long incl = still ? s : 0;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const long long o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+          if (lane >= d) incl += o;
+        }
+        const unsigned fit = __ballot_sync(0xFFFFFFFFu, still && incl <= room);   // a prefix of the undecided ones
+        if ((fit >> lane) & 1u) dest = 1;
+        const long long taken = __shfl_sync(0xFFFFFFFFu, incl, fit ? 31 - __clz(fit) : 0);
+        room -= fit ? taken : 0;
+        undecided &= ~fit;
+      }
+      if (k < v) vdest[k] = (uint8_t)dest;
     }
-    for (; k < v; ++k) {
-      const int s0 = vsize[k];
-      const bool f0 = s0 <= room; room -= f0 ? s0 : 0;
-      vdest[k] = f0 ? 1 : 2;
-    }
-    bcast[0] = cap_cpu - room;
+    if (lane == 0) bcast[0] = cap_cpu - room;
   }
   __syncthreads();
   const long long usage_cpu1 = bcast[0];

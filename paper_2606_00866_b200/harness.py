@@ -48,8 +48,13 @@ class GpuRunner:
         self._o_bounds = self._o_counts + 20
         self._o_used = (self._o_bounds + 8 + 7) // 8 * 8
         self._o_tier = self._o_used + 16
-        self.d_out = torch.zeros(self._o_tier + n, dtype=torch.uint8, device=d)
         self.h_out = torch.zeros(self._o_tier + n, dtype=torch.uint8, pin_memory=True)
+        # small n: the ranker writes its outputs straight into the pinned blob (include/mori.h:
+        # outputs may be mapped host memory) -- no device-to-host copy; large n: device blob + one copy
+        self.out_mapped = n <= 1024
+        self.d_out = self.h_out if self.out_mapped else torch.zeros(self._o_tier + n, dtype=torch.uint8, device=d)
+        self._h_out_np = self.h_out.numpy()
+        self._h_in_np = None
         self.h_in = torch.zeros(9 * n, dtype=torch.uint8, pin_memory=True)    # iota | kv | prev
         self.d_in = torch.zeros(9 * n, dtype=torch.uint8, device=d)
         self._wl = None
@@ -65,9 +70,10 @@ class GpuRunner:
         with torch.cuda.stream(s):
             self.d_in.copy_(self.h_in, non_blocking=True)
             self._launch_rank(self.d_in, s)
-            self.h_out.copy_(self.d_out, non_blocking=True)
+            if not self.out_mapped:
+                self.h_out.copy_(self.d_out, non_blocking=True)
         s.synchronize()
-        return self._unpack(self.h_out.numpy())
+        return self._unpack(self._h_out_np)
 
     # -- NEXT-1: the sticky policy mode, same host-in / host-out shape as place() ------------------
     def place_sticky(self, iota, kv_pages, prev_tier, flags, stream=None):
@@ -90,10 +96,11 @@ class GpuRunner:
                 self.cfg.cap_gpu_pages, self.cfg.cap_cpu_pages, base + self._o_tier,
                 self._st["lazy"].data_ptr(), base + self._o_used, base + self._o_lists,
                 base + self._o_counts))
-            self.h_out.copy_(self.d_out, non_blocking=True)
+            if not self.out_mapped:
+                self.h_out.copy_(self.d_out, non_blocking=True)
             lazy = self._st["lazy"].cpu()
         s.synchronize()
-        out = self._unpack(self.h_out.numpy())
+        out = self._unpack(self._h_out_np)
         out["lazy"] = lazy.numpy()
         del out["order"], out["bounds"]
         return out
@@ -107,13 +114,19 @@ class GpuRunner:
         hin[8 * n:] = prev_tier
         self.d_in.copy_(self.h_in, non_blocking=True)
 
-    def place_resident(self, stream=None):
+    def place_resident(self, stream=None, done_event=None):
+        """``done_event`` (a torch.cuda.Event) is recorded on the stream right behind the launch (and
+        the device-to-host copy of the placement, when there is one): the device-side end of a1-a4,
+        before any host-side unpacking."""
         s = stream or torch.cuda.current_stream()
-        with torch.cuda.stream(s):
-            self._launch_rank(self.d_in, s)
-            self.h_out.copy_(self.d_out, non_blocking=True)
+        self._launch_rank(self.d_in, s)
+        if not self.out_mapped:
+            with torch.cuda.stream(s):
+                self.h_out.copy_(self.d_out, non_blocking=True)
+        if done_event is not None:
+            done_event.record(s)
         s.synchronize()
-        return self._unpack(self.h_out.numpy())
+        return self._unpack(self._h_out_np)
 
     def _launch_rank(self, d_in, s):
         n = self.cfg.n_programs
@@ -145,10 +158,14 @@ class GpuRunner:
         per program."""
         tickets = {}                      # demote number k -> ticket of the call that carried it
         dem, pro, pro_dep = [], [], 0
+        need_tickets = any(op[0] == "promote" and op[5] > 0 for op in plan.ops)
+
+        def cat(parts):
+            return parts[0] if len(parts) == 1 else np.concatenate(parts)
 
         def flush_dem():
             if dem:
-                t = self.mori.mori_demote(np.concatenate([o[3] for o in dem]), np.concatenate([o[4] for o in dem]))
+                t = self.mori.mori_demote(cat([o[3] for o in dem]), cat([o[4] for o in dem]), want_ticket=need_tickets)
                 for o in dem:
                     tickets[o[1]] = t
                 dem.clear()
@@ -158,8 +175,9 @@ class GpuRunner:
             if pro:
                 if pro_dep > 0 and pro_dep not in tickets:
                     flush_dem()
-                self.mori.mori_promote(np.concatenate([o[3] for o in pro]), np.concatenate([o[4] for o in pro]),
-                                       pages_after_demote=tickets.get(pro_dep, 0) if pro_dep > 0 else 0)
+                self.mori.mori_promote(cat([o[3] for o in pro]), cat([o[4] for o in pro]),
+                                       pages_after_demote=tickets.get(pro_dep, 0) if pro_dep > 0 else 0,
+                                       want_ticket=False)
                 pro.clear()
             pro_dep = 0
 

@@ -379,6 +379,7 @@ class IdAllocator:
                 raise MemoryError("allocator exhausted")
             ids = np.concatenate([clean, dirty[:k - clean.size]])
         dep = int(self.tag[ids].max())
+        self.last_tags = self.tag[ids].copy()       # per id: 0 = was clean, t = free once move #t completes
         self.free[ids] = False
         self.tag[ids] = 0
         return ids.astype(np.int32), dep
@@ -484,7 +485,16 @@ class Sim:
                     p = pro_q.pop(0)
                     slots = self.host_slots[p]
                     pages, dep = self.gpu_alloc.alloc(slots.size)
-                    ops.append(("promote", 0, p, slots.copy(), pages, dep if dep > 0 else -1))
+                    if dep > 0:
+                        # some of the pages are still being vacated: the part that lands in clean
+                        # pages goes at once, the rest follows the demotion that frees it, one piece
+                        # per demotion, in the order the demotions complete
+                        tags = self.gpu_alloc.last_tags
+                        for t in np.unique(tags):
+                            sel = tags == t
+                            ops.append(("promote", 0, p, slots[sel].copy(), pages[sel], int(t) if t > 0 else -1))
+                    else:
+                        ops.append(("promote", 0, p, slots.copy(), pages, -1))
                     self.cpu_alloc.release(slots, tag=1)     # not reusable before the next join
                     self.gpu_pages[p] = pages
                     self.host_slots[p] = np.zeros(0, np.int32)

@@ -11,12 +11,21 @@ pytestmark = pytest.mark.gpu
 PAGES = 140000
 
 
-@pytest.fixture(scope="module")
-def ctx(mori):
+@pytest.fixture(scope="module", params=["cluster", "multi_kernel"])
+def ctx(mori, request):
+    """Two sorts behind one entry point: pools of up to 131 072 pages take ONE launch (a cluster of
+    8 CTAs), larger ones the general multi-kernel radix sort; MORI_EVICT_MULTI=1 forces the latter
+    at every size so that both are checked at every size."""
+    import os
     # 32-byte pages: a pool and an arena with many pages cost nothing
     pool = torch.zeros(PAGES * 32, dtype=torch.uint8, device="cuda")
     arena = torch.zeros(PAGES * 32, dtype=torch.uint8).pin_memory()
-    m = mori.Mori(1, 1, 8, 1, pool, arena)
+    if request.param == "multi_kernel":
+        os.environ["MORI_EVICT_MULTI"] = "1"
+    try:
+        m = mori.Mori(1, 1, 8, 1, pool, arena)
+    finally:
+        os.environ.pop("MORI_EVICT_MULTI", None)
     yield m
     m.close()
 
@@ -43,7 +52,7 @@ def test_hand_worked_example(ctx, mori):
         assert gpu_order(ctx, which, g["owner"], g["program_tier"], g["last_access"]).tolist() == g[name].tolist()
 
 
-@pytest.mark.parametrize("n_pages", [0, 1, 31, 32, 33, 1023, 1024, 1025, 5000, 65536, 65537, PAGES])
+@pytest.mark.parametrize("n_pages", [0, 1, 31, 32, 33, 1023, 1024, 1025, 5000, 8191, 8193, 16385, 40960, 65536, 65537, 131072, 131073, PAGES])
 def test_random_pools_identical_sequence(ctx, mori, n_pages):
     rng = np.random.default_rng(900 + n_pages)
     for rep in range(3):
