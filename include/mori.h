@@ -275,7 +275,9 @@ int mori_idleness_eval(mori_ctx* ctx, void* stream, int32_t n, const double* ope
  * CPU DRAM evicts inactive first, then busy, then idle; "within each type, LRU breaks ties".
  * A page's type is its owner's placement: MORI_TIER_GPU busy, MORI_TIER_CPU idle,
  * anything else inactive.  Equal last_access inside a type: lower page id first.
- * DEVICE pointers; a fixed sequence of kernels on `stream`; asynchronous.
+ * DEVICE pointers; asynchronous on `stream`: ONE launch (a cluster of 16 CTAs, 8 where the device does not
+ * allow that size) for pools of up to 262 144 (131 072) pages, a fixed sequence of kernels replayed as a CUDA
+ * graph beyond that.
  *
  *   which_tier    MORI_TIER_GPU: n_pages <= gpu_pool_pages;  MORI_TIER_CPU: n_pages <= host_arena_slots
  *   page_owner    [n_pages] int32 program slot, or < 0 for a free page (free pages are not listed)

@@ -146,7 +146,7 @@ evict_scatter_kernel(EvictArgs a, int pass, const int32_t* __restrict__ perm_in,
 // Pass 0 also counts the resident pages and finds the largest last-access value; passes whose
 // byte of it is zero for every resident page are skipped outright (tick-sized counters: 2 passes
 // instead of 5).
-constexpr int kEvictCluster = 8;
+constexpr int kEvictCluster = 8;                                    // portable cluster size
 constexpr int kEvictClusterMaxPages = kEvictCluster * 1024 * 16;
 
 __device__ __forceinline__ uint64_t evict_item(const EvictArgs& a, int page, bool& resident, unsigned& last) {
@@ -162,13 +162,15 @@ __device__ __forceinline__ int evict_item_digit(uint64_t item, int pass) {
   return pass == 4 ? (int)(item >> 62) : (int)((item >> (30 + 8 * pass)) & 0xFF);
 }
 
+// The cluster size is a launch attribute (8, or 16 where the device allows the non-portable size).
 template <int R>
-__global__ void __cluster_dims__(kEvictCluster, 1, 1) __launch_bounds__(1024, 1)
+__global__ void __launch_bounds__(1024, 1)
 evict_order_cluster_kernel(EvictArgs a, uint64_t* __restrict__ buf0, uint64_t* __restrict__ buf1,
                            int32_t* __restrict__ victims, int32_t* __restrict__ n_resident) {
   namespace cg = cooperative_groups;
   cg::cluster_group cluster = cg::this_cluster();
   const int crank = (int)cluster.block_rank();
+  const int csize = (int)cluster.num_blocks();
   __shared__ int wc[32][257];
   __shared__ int tot[256];
   __shared__ int s_stat[2];                                          // resident pages, max last access (this CTA)
@@ -176,7 +178,7 @@ evict_order_cluster_kernel(EvictArgs a, uint64_t* __restrict__ buf0, uint64_t* _
   __shared__ uint64_t warp_tot[33];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const long long N = a.n_pages;
-  const int seg = (int)(((N + kEvictCluster - 1) / kEvictCluster + 1023) / 1024 * 1024);
+  const int seg = (int)(((N + csize - 1) / csize + 1023) / 1024 * 1024);
   const int per_warp = seg / 32, rounds = per_warp / 32;             // rounds <= R (host checks)
   const long long first = (long long)crank * seg + (long long)warp * per_warp + lane;
 
@@ -206,12 +208,15 @@ evict_order_cluster_kernel(EvictArgs a, uint64_t* __restrict__ buf0, uint64_t* _
     const bool last_pass = pass == 4;
     for (int e = tid; e < 32 * 257; e += 1024) (&wc[0][0])[e] = 0;
     __syncthreads();
-    // ---- sweep A: per-warp digit counts --------------------------------------------------------
+    // ---- sweep A: per-warp digit counts (the lanes with the same digit are remembered for sweep B) --
+    unsigned peers_of[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
+      peers_of[r] = 0;
       if (r < rounds) {
         const int d = item[r] == ~0ull ? 256 : evict_item_digit(item[r], pass);
         const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
+        peers_of[r] = peers;
         if (d < 256 && lane == __ffs(peers) - 1) wc[warp][d] += __popc(peers);
         __syncwarp();
       }
@@ -226,14 +231,14 @@ evict_order_cluster_kernel(EvictArgs a, uint64_t* __restrict__ buf0, uint64_t* _
     // ---- exchange: where this CTA's items of every digit start -----------------------------------
     int all = 0, below = 0;
     if (tid < 256) {
-      for (int c = 0; c < kEvictCluster; ++c) {
+      for (int c = 0; c < csize; ++c) {
         const int v = *cluster.map_shared_rank(&tot[tid], c);
         all += v; below += c < crank ? v : 0;
       }
     }
     if (pass == 0 && tid == 0) {
       int res = 0; unsigned mx = 0;
-      for (int c = 0; c < kEvictCluster; ++c) {
+      for (int c = 0; c < csize; ++c) {
         const int* st = cluster.map_shared_rank(&s_stat[0], c);
         res += st[0]; mx = max(mx, (unsigned)st[1]);
       }
@@ -251,7 +256,7 @@ evict_order_cluster_kernel(EvictArgs a, uint64_t* __restrict__ buf0, uint64_t* _
     for (int r = 0; r < R; ++r) {
       if (r < rounds) {
         const int d = item[r] == ~0ull ? 256 : evict_item_digit(item[r], pass);
-        const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
+        const unsigned peers = peers_of[r];
         const int leader = __ffs(peers) - 1;
         int start = 0;
         if (d < 256 && lane == leader) { start = wc[warp][d]; wc[warp][d] = start + __popc(peers); }

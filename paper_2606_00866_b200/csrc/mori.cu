@@ -104,9 +104,12 @@ struct mori_ctx {
   unsigned int* evict_max_last = nullptr;
   int32_t* evict_perm[2] = {nullptr, nullptr}; int32_t* evict_table = nullptr; long long evict_cap = 0;   // scratch, grown on demand
   bool evict_multi_kernel = false;               // MORI_EVICT_MULTI=1: force the general (multi-kernel) sort
+  int evict_cluster_want = 16;
+  int evict_cluster = 8;                         // CTAs of the one-launch eviction sort's cluster (8, or 16 where allowed)
   int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
   Direction dir[2];                              // 0 demote, 1 promote
   std::vector<cudaEvent_t> free_events;
+  std::vector<cudaEvent_t> free_timing_events;   // profiling spans reuse their events (creating one costs microseconds)
   bool profiling = false;
   bool timeline = false; cudaEvent_t prof_base = nullptr;   // mori_profile(ctx, 2)
   mutable long long launches = 0;                // kernels launched by this context
@@ -222,6 +225,7 @@ cudaError_t launch_small(const mori_ctx* c, long long n, const int32_t* gpu_page
 cudaEvent_t get_event(mori_ctx* c, bool timing) {
   cudaEvent_t e = nullptr;
   if (!timing && !c->free_events.empty()) { e = c->free_events.back(); c->free_events.pop_back(); return e; }
+  if (timing && !c->free_timing_events.empty()) { e = c->free_timing_events.back(); c->free_timing_events.pop_back(); return e; }
   const cudaError_t rc = cudaEventCreateWithFlags(&e, timing ? cudaEventDefault : cudaEventDisableTiming);
   if (rc != cudaSuccess) {
     c->sticky = MORI_ERR_CUDA;
@@ -319,7 +323,8 @@ void prof_collect(mori_ctx* c, Direction& d) {
       if (c && c->timeline && c->prof_base && cudaEventElapsedTime(&t0, c->prof_base, sp.a) == cudaSuccess)
         d.timeline.push_back({sp.kind, (double)t0, (double)t0 + ms, sp.bytes});
     }
-    cudaEventDestroy(sp.a); cudaEventDestroy(sp.b);
+    if (c) { c->free_timing_events.push_back(sp.a); c->free_timing_events.push_back(sp.b); }
+    else { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   }
   cudaGetLastError();
   d.spans.clear();
@@ -445,6 +450,7 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
   }
   c->debug = env_ll("MORI_DEBUG", 0) != 0;
   c->evict_multi_kernel = env_ll("MORI_EVICT_MULTI", 0) != 0;
+  c->evict_cluster_want = (int)env_ll("MORI_EVICT_CLUSTER", 16);
   c->max_pages = cfg->max_pages_per_call ? cfg->max_pages_per_call
                                           : std::max<long long>(cfg->gpu_pool_pages, cfg->host_arena_slots);
   // Staging: the gather / scatter kernels run one launch per segment, and a launch pays ~15 us of
@@ -481,12 +487,47 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
     }                                                                                         \
   } while (0)
 
+  // CUDA loads kernels lazily, on their first launch (tens of microseconds each): touch the hot
+  // path's kernels now so that no epoch pays for it -- a small move is a single ~10 us launch.
+  {
+    cudaFuncAttributes fa;
+    const void* hot[] = {(const void*)mori::copy_pages_small<true, mori::kSmallFewPages>,
+                         (const void*)mori::copy_pages_small<false, mori::kSmallFewPages>,
+                         (const void*)mori::copy_pages_small<true, mori::kSmallMaxPages>,
+                         (const void*)mori::copy_pages_small<false, mori::kSmallMaxPages>,
+                         (const void*)mori::copy_pages_tma<true>, (const void*)mori::copy_pages_tma<false>,
+                         (const void*)mori::copy_pages_ldst<true>, (const void*)mori::copy_pages_ldst<false>,
+                         (const void*)upload_idx_kernel, (const void*)mori::rank_partition_kernel<1>,
+                         (const void*)mori::rank_partition_multi_kernel<2>, (const void*)mori::rank_partition_multi_kernel<4>,
+                         (const void*)mori::rank_partition_multi_kernel<8>};
+    for (const void* f : hot) CKC(cudaFuncGetAttributes(&fa, f));
+  }
   // The attribute is per function and PROCESS-wide: every context sets it to the device's opt-in
   // maximum, so contexts with different ring sizes never lower it under one another.
   CKC(cudaFuncSetAttribute(mori::copy_pages_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
   CKC(cudaFuncSetAttribute(mori::copy_pages_tma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
   CKC(cudaMalloc((void**)&c->rank_tickets, sizeof(unsigned int) * kRankTickets));
   CKC(cudaMemset(c->rank_tickets, 0, sizeof(unsigned int) * kRankTickets));
+  if (c->evict_cluster_want >= 16) {
+    // a cluster of 16 CTAs is a non-portable size: allowed per kernel, and only if the device can
+    // co-schedule it (cudaOccupancyMaxActiveClusters); otherwise the portable 8
+    bool ok = true;
+    const void* ks[] = {(const void*)mori::evict_order_cluster_kernel<2>, (const void*)mori::evict_order_cluster_kernel<4>,
+                        (const void*)mori::evict_order_cluster_kernel<8>, (const void*)mori::evict_order_cluster_kernel<16>};
+    for (const void* k : ks) ok = ok && cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+    if (ok) {
+      cudaLaunchConfig_t lc{};
+      lc.gridDim = dim3(16); lc.blockDim = dim3(1024);
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = 16; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      lc.attrs = at; lc.numAttrs = 1;
+      int n_clusters = 0;
+      ok = cudaOccupancyMaxActiveClusters(&n_clusters, mori::evict_order_cluster_kernel<8>, &lc) == cudaSuccess && n_clusters >= 1;
+    }
+    cudaGetLastError();
+    c->evict_cluster = ok ? 16 : 8;
+  }
   if (env_ll("MORI_SCHED", 1) != 0) {
     CKC(cudaMalloc((void**)&c->sched, sizeof(unsigned int) * 2 * kSchedRing));
     CKC(cudaMemset(c->sched, 0, sizeof(unsigned int) * 2 * kSchedRing));
@@ -564,6 +605,7 @@ int mori_destroy(mori_ctx* c) {
     if (d.copy) cudaStreamDestroy(d.copy);
   }
   for (auto ev : c->free_events) cudaEventDestroy(ev);
+  for (auto ev : c->free_timing_events) cudaEventDestroy(ev);
   if (c->prof_base) cudaEventDestroy(c->prof_base);
   if (c->rank_tickets) cudaFree(c->rank_tickets);
   if (c->sched) cudaFree(c->sched);
@@ -598,7 +640,7 @@ int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idlen
   const int threads = n_pad / ipt;
   if (n > mori::kRankMaxThreads) {
     // more than one CTA's worth: rank by counting on every SM, last CTA partitions
-    const int grid = std::min(c->sm_count, (n + 31) / 32);
+    const int grid = std::min(c->sm_count, (n + 7) / 8);
     const size_t smem_m = sizeof(uint64_t) * ((size_t)n + 33) + 2 * sizeof(long long);
     const unsigned long long slot_m = c->rank_seq++ % kRankTickets;
     unsigned int* tk = c->rank_tickets + slot_m;
@@ -639,7 +681,7 @@ int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idl
     return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
   int n_pad = 1024;
   while (n_pad < n) n_pad <<= 1;
-  const int grid = std::max(1, std::min(c->sm_count, (n + 31) / 32));
+  const int grid = std::max(1, std::min(c->sm_count, (n + 7) / 8));
   const size_t smem = sizeof(uint64_t) * (2 * (size_t)n + 33) + 4 * sizeof(long long);
   const unsigned long long slot = c->rank_seq++ % kRankTickets;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -677,7 +719,7 @@ int mori_rank_partition_tiers(mori_ctx* c, void* stream, int32_t n, const float*
   }
   int n_pad = 1024;
   while (n_pad < n) n_pad <<= 1;
-  const int grid = std::max(1, std::min(c->sm_count, (n + 31) / 32));
+  const int grid = std::max(1, std::min(c->sm_count, (n + 7) / 8));
   const size_t smem = sizeof(uint64_t) * ((size_t)n + 33) + 2 * sizeof(long long);
   const unsigned long long slot_t = c->rank_seq++ % kRankTickets;
   unsigned int* tk = c->rank_tickets + slot_t;
@@ -707,7 +749,7 @@ int mori_bfd_assign(mori_ctx* c, void* stream, int32_t m, const int32_t* size, c
   if (n_replicas < 1 || n_replicas > mori::kBfdMaxReplicas) return fail(c, MORI_ERR_UNSUPPORTED, "n_replicas must be 1..32");
   if (!free_pages || !free_out || (m > 0 && (!size || !idleness || !flags || !replica)))
     return fail(c, MORI_ERR_INVALID_ARG, "NULL array");
-  const int grid = std::max(1, std::min(c->sm_count, (m + 31) / 32));
+  const int grid = std::max(1, std::min(c->sm_count, (m + 7) / 8));
   const size_t smem = sizeof(uint64_t) * 2 * (size_t)std::max(m, 1);
   const unsigned long long slot = c->rank_seq++ % kRankTickets;
   if (smem > 48 * 1024)
@@ -746,16 +788,25 @@ int mori_eviction_order(mori_ctx* c, void* stream, int32_t which_tier, int64_t n
     c->evict_cap = n_pages;
   }
   mori::EvictArgs a{n_pages, n_programs, which_tier == MORI_TIER_GPU ? 0 : 1, tiles, page_owner, program_tier, last_access};
-  if (n_pages <= mori::kEvictClusterMaxPages && !c->evict_multi_kernel) {
+  if (n_pages <= (long long)c->evict_cluster * 1024 * 16 && n_pages <= 2 * mori::kEvictClusterMaxPages && !c->evict_multi_kernel) {
     // every BASELINE.json pool: ONE launch, a cluster of 8 CTAs, passes separated by cluster barriers
-    const long long seg = ((n_pages + mori::kEvictCluster - 1) / mori::kEvictCluster + 1023) / 1024 * 1024;
+    const int csize = c->evict_cluster;
+    const long long seg = ((n_pages + csize - 1) / csize + 1023) / 1024 * 1024;
     const int rounds = (int)(seg / 1024);
     uint64_t* b0 = reinterpret_cast<uint64_t*>(c->evict_perm[0]);
     uint64_t* b1 = reinterpret_cast<uint64_t*>(c->evict_perm[1]);
-    if (rounds <= 2) mori::evict_order_cluster_kernel<2><<<mori::kEvictCluster, 1024, 0, s>>>(a, b0, b1, victims, n_resident);
-    else if (rounds <= 4) mori::evict_order_cluster_kernel<4><<<mori::kEvictCluster, 1024, 0, s>>>(a, b0, b1, victims, n_resident);
-    else if (rounds <= 8) mori::evict_order_cluster_kernel<8><<<mori::kEvictCluster, 1024, 0, s>>>(a, b0, b1, victims, n_resident);
-    else mori::evict_order_cluster_kernel<16><<<mori::kEvictCluster, 1024, 0, s>>>(a, b0, b1, victims, n_resident);
+    cudaLaunchConfig_t lc{};
+    lc.gridDim = dim3(csize); lc.blockDim = dim3(1024); lc.dynamicSmemBytes = 0; lc.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = csize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.attrs = at; lc.numAttrs = 1;
+    cudaError_t le;
+    if (rounds <= 2) le = cudaLaunchKernelEx(&lc, mori::evict_order_cluster_kernel<2>, a, b0, b1, victims, n_resident);
+    else if (rounds <= 4) le = cudaLaunchKernelEx(&lc, mori::evict_order_cluster_kernel<4>, a, b0, b1, victims, n_resident);
+    else if (rounds <= 8) le = cudaLaunchKernelEx(&lc, mori::evict_order_cluster_kernel<8>, a, b0, b1, victims, n_resident);
+    else le = cudaLaunchKernelEx(&lc, mori::evict_order_cluster_kernel<16>, a, b0, b1, victims, n_resident);
+    CK(c, le);
     CK(c, cudaGetLastError());
     c->launches += 1;
     return MORI_OK;

@@ -62,10 +62,22 @@ __device__ __forceinline__ uint64_t block_excl_scan(uint64_t v, uint64_t* warp_t
 // exactly one CTA, the LAST to finish (atomic ticket, reset for the next launch), after every
 // CTA's order[] writes are visible to it (read them with __ldcg): that CTA carries on with the
 // part of the algorithm that needs the whole order.  `less(j, i)` says key_j < key_i.
+// The tail of every rank-by-counting kernel: true in exactly one CTA, the LAST to finish.
+__device__ __forceinline__ bool last_cta_ticket(unsigned int* __restrict__ ticket) {
+  __shared__ unsigned int s_ticket;
+  __threadfence();                                   // this CTA's order[] writes are visible ...
+  __syncthreads();
+  if (threadIdx.x == 0) s_ticket = atomicAdd(ticket, 1u);    // ... before its ticket is
+  __syncthreads();
+  if (s_ticket != gridDim.x - 1) return false;
+  if (threadIdx.x == 0) *ticket = 0;                 // ready for the next launch that uses this counter
+  __threadfence();
+  return true;
+}
+
 template <class Less>
 __device__ __forceinline__ bool rank_by_counting(int n, Less less, int32_t* __restrict__ order,
                                                  unsigned int* __restrict__ ticket) {
-  __shared__ unsigned int s_ticket;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
   const int per = (n + gridDim.x - 1) / gridDim.x;
   const int lo = blockIdx.x * per, hi = min(n, lo + per);
@@ -76,14 +88,36 @@ __device__ __forceinline__ bool rank_by_counting(int n, Less less, int32_t* __re
     for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
     if (lane == 0) order[c] = i;
   }
-  __threadfence();                                   // this CTA's order[] writes are visible ...
-  __syncthreads();
-  if (tid == 0) s_ticket = atomicAdd(ticket, 1u);    // ... before its ticket is
-  __syncthreads();
-  if (s_ticket != gridDim.x - 1) return false;
-  if (tid == 0) *ticket = 0;                         // ready for the next launch that uses this counter
-  __threadfence();
-  return true;
+  return last_cta_ticket(ticket);
+}
+
+// The same for unique 128-bit keys (sticky_rebalance, bfd_assign), where the counting loop is what
+// the launch costs: n^2 compares, bound by instruction issue.  Keys sit in shared memory as one
+// 16-byte word each (x = low half, y = high half) -- one LDS.128 per compare -- and the compare is
+// the borrow of a 128-bit subtraction (four carry-chained ISETPs), branch-free, four keys in flight.
+__device__ __forceinline__ int lt128(const ulonglong2& a, const ulonglong2& b) {
+  return (((unsigned __int128)a.y << 64) | a.x) < (((unsigned __int128)b.y << 64) | b.x) ? 1 : 0;
+}
+__device__ __forceinline__ bool rank_by_counting128(int n, const ulonglong2* __restrict__ keys,
+                                                    int32_t* __restrict__ order, unsigned int* __restrict__ ticket) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+  const int per = (n + gridDim.x - 1) / gridDim.x;
+  const int lo = blockIdx.x * per, hi = min(n, lo + per);
+  for (int i = lo + warp; i < hi; i += n_warps) {
+    const ulonglong2 ki = keys[i];
+    int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
+    int j = lane;
+    for (; j + 96 < n; j += 128) {
+      const ulonglong2 k0 = keys[j], k1 = keys[j + 32], k2 = keys[j + 64], k3 = keys[j + 96];
+      c0 += lt128(k0, ki); c1 += lt128(k1, ki); c2 += lt128(k2, ki); c3 += lt128(k3, ki);
+    }
+    for (; j < n; j += 32) c0 += lt128(keys[j], ki);
+    int c = (c0 + c1) + (c2 + c3);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
+    if (lane == 0) order[c] = i;
+  }
+  return last_cta_ticket(ticket);
 }
 
 // Steps a2-a4 for one CTA whose thread t owns ranks [t*IPT, (t+1)*IPT): prog[i] is the program at

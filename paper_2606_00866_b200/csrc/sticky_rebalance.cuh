@@ -36,7 +36,8 @@ __device__ __forceinline__ int sticky_group(int prev, int fl) {
   return (fl & kFlagNew) ? 3 : 2;
 }
 
-__device__ __forceinline__ void sticky_key(int p, float iota, int s, int prev, int fl, uint64_t& hi, uint64_t& lo) {
+__device__ __forceinline__ void sticky_key(int p, float iota, int s, int prev, int fl, unsigned long long& hi,
+                                           unsigned long long& lo) {
   const uint32_t ik = idleness_key(iota);
   const int g = sticky_group(prev, fl);
   if (g == 0) {                       // Acting first, then most idle first (later in the total order)
@@ -57,25 +58,24 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
                         int32_t* __restrict__ lists, int32_t* __restrict__ list_counts,
                         int32_t* __restrict__ order, unsigned int* __restrict__ ticket) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  uint64_t* khi = reinterpret_cast<uint64_t*>(smem_raw);             // [n]
-  uint64_t* klo = khi + n;                                           // [n]
-  uint64_t* warp_tot = klo + n;                                      // [33]
+  ulonglong2* keys = reinterpret_cast<ulonglong2*>(smem_raw);        // [n] (x = low half, y = high half)
+  uint64_t* warp_tot = reinterpret_cast<uint64_t*>(keys + n);        // [33]
   long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [4]
   const int tid = threadIdx.x;
 
   for (int p = tid; p < n; p += blockDim.x) {
     const int pv = prev_tier[p];
-    sticky_key(p, idleness[p], kv_pages[p], pv == 0 ? 0 : (pv == 1 ? 1 : 2), flags[p], khi[p], klo[p]);
+    unsigned long long hi64, lo64;
+    sticky_key(p, idleness[p], kv_pages[p], pv == 0 ? 0 : (pv == 1 ? 1 : 2), flags[p], hi64, lo64);
+    keys[p] = make_ulonglong2(lo64, hi64);
   }
   __syncthreads();
   // ---- position of every program = number of smaller 128-bit keys; the last CTA goes on ---------
-  if (!rank_by_counting(n, [&](int j, int i) { return khi[j] < khi[i] || (khi[j] == khi[i] && klo[j] < klo[i]); },
-                        order, ticket))
-    return;
+  if (!rank_by_counting128(n, keys, order, ticket)) return;
 
   // ---- this thread's positions ------------------------------------------------------------------
-  int32_t* vsize = reinterpret_cast<int32_t*>(khi);                  // [n] victims' sizes, by position
-  uint8_t* vdest = reinterpret_cast<uint8_t*>(klo);                  // [n] 1 = CPU queue, 2 = Waiting
+  int32_t* vsize = reinterpret_cast<int32_t*>(keys);                 // [n] victims' sizes, by position
+  uint8_t* vdest = reinterpret_cast<uint8_t*>(vsize + n);            // [n] 1 = CPU queue, 2 = Waiting
   int prog[IPT], grp[IPT], was[IPT], fl[IPT];
   long long sz[IPT];
   long long sum_g = 0, sum_c = 0;

@@ -6,6 +6,7 @@ and one libmori context.  No oracle here, no CPU fallback: placement comes from
 """
 from __future__ import annotations
 
+import ctypes as C
 from typing import Optional
 
 import numpy as np
@@ -149,35 +150,33 @@ class GpuRunner:
                     lists=[lists2d[k, :counts[k]].copy() for k in range(5)])
 
     # -- a5-a7 ---------------------------------------------------------------------------------
-    def execute(self, plan: W.EpochPlan, sync=True, merge=True):
-        """Issues the epoch's moves.  A move is a flat list of pages (include/mori.h), so the
-        demotions of an epoch go out as ONE ``mori_demote`` per stretch of the plan that no promotion
-        depends on, and the promotions likewise as one ``mori_promote`` per stretch with the same
-        dependency: fewer calls, fewer ragged last staging segments, and the page order inside a
-        call is the plan's (the paper's move order, P:L206 / L208).  ``merge=False`` issues one call
-        per program."""
-        tickets = {}                      # demote number k -> ticket of the call that carried it
+    def prepare(self, plan: W.EpochPlan, merge=True):
+        """Turns the epoch's moves into the argument lists of the calls that will carry them (host
+        work, like the allocator that produced the tables).  A move is a flat list of pages
+        (include/mori.h), so the demotions of an epoch go out as ONE ``mori_demote`` per stretch of
+        the plan that no promotion depends on, and the promotions likewise as one ``mori_promote``
+        per stretch with the same dependency: fewer calls, fewer ragged last staging segments, and
+        the page order inside a call is the plan's (the paper's move order, P:L206 / L208).
+        ``merge=False``: one call per program.  -> (steps, need_tickets) for ``issue``."""
+        steps = []                        # ("d", pages, slots, n, [k ...]) | ("p", slots, pages, n, dep) | ("sync",)
         dem, pro, pro_dep = [], [], 0
-        need_tickets = any(op[0] == "promote" and op[5] > 0 for op in plan.ops)
+        flushed = set()
 
         def cat(parts):
-            return parts[0] if len(parts) == 1 else np.concatenate(parts)
+            return np.ascontiguousarray(parts[0] if len(parts) == 1 else np.concatenate(parts), dtype=np.int32)
 
         def flush_dem():
             if dem:
-                t = self.mori.mori_demote(cat([o[3] for o in dem]), cat([o[4] for o in dem]), want_ticket=need_tickets)
-                for o in dem:
-                    tickets[o[1]] = t
+                g, h = cat([o[3] for o in dem]), cat([o[4] for o in dem])
+                steps.append(("d", g, h, g.size, [o[1] for o in dem]))
+                flushed.update(o[1] for o in dem)
                 dem.clear()
 
         def flush_pro():
             nonlocal pro_dep
             if pro:
-                if pro_dep > 0 and pro_dep not in tickets:
-                    flush_dem()
-                self.mori.mori_promote(cat([o[3] for o in pro]), cat([o[4] for o in pro]),
-                                       pages_after_demote=tickets.get(pro_dep, 0) if pro_dep > 0 else 0,
-                                       want_ticket=False)
+                h, g = cat([o[3] for o in pro]), cat([o[4] for o in pro])
+                steps.append(("p", h, g, g.size, pro_dep))
                 pro.clear()
             pro_dep = 0
 
@@ -190,7 +189,7 @@ class GpuRunner:
                 dep = op[5] if op[5] > 0 else 0
                 if pro and dep != pro_dep:        # a different dependency: its own call
                     flush_pro()
-                if dep > 0 and dep not in tickets:
+                if dep > 0 and dep not in flushed:
                     flush_dem()                   # the demotion it follows ends its call here, so the
                                                   # promotion waits for that much and no more
                 pro.append(op)
@@ -199,12 +198,38 @@ class GpuRunner:
                     flush_pro()
             elif op[0] == "sync_all":
                 flush_dem(); flush_pro()
-                self.mori.mori_sync(binding.BOTH)
-                tickets.clear()
+                steps.append(("sync",))
+                flushed.clear()
         # both directions start together: the demote call first (it is what vacates pages)
         flush_dem(); flush_pro()
+        return steps, any(st[0] == "p" and st[4] > 0 for st in steps)
+
+    def issue(self, prepared, sync=True):
+        """The C-ABI calls of one epoch, nothing else: one ``mori_demote`` / ``mori_promote`` per
+        prepared step, tickets handed from the demotion that vacates pages to the promotion that
+        lands in them."""
+        steps, need_tickets = prepared
+        lib, h_ctx = self.mori._lib, self.mori._h
+        tickets = {}
+        t = C.c_int64(0)
+        tp = C.byref(t) if need_tickets else None
+        for st in steps:
+            if st[0] == "d":
+                self.mori._ck(lib.mori_demote(h_ctx, st[3], st[1].ctypes.data, st[2].ctypes.data, 0, tp))
+                for k in st[4]:
+                    tickets[k] = t.value
+            elif st[0] == "p":
+                self.mori._ck(lib.mori_promote(h_ctx, st[3], st[1].ctypes.data, st[2].ctypes.data,
+                                               tickets.get(st[4], 0) if st[4] > 0 else 0, 0, None))
+            else:
+                self.mori.mori_sync(binding.BOTH)
+                tickets.clear()
         if sync:
             self.mori.mori_sync(binding.BOTH)
+
+    def execute(self, plan: W.EpochPlan, sync=True, merge=True):
+        """``prepare`` + ``issue``."""
+        self.issue(self.prepare(plan, merge=merge), sync=sync)
 
     # -- input generation on the device (workload helper library; not the hot path) ------------
     def _keys_pages(self, triples):

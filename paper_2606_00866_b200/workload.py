@@ -396,7 +396,9 @@ class IdAllocator:
 class EpochPlan:
     """What one epoch does, as tables.  ``ops`` is the issue order:
     ("demote", k, program, gpu_pages, host_slots)          k = 1, 2, ... within the epoch
-    ("promote", 0, program, host_slots, gpu_pages, dep)    dep = k of the demote it must follow, or -1
+    ("promote", 0, program, host_slots, gpu_pages, dep, first)   dep = k of the demote it must follow, or -1;
+                                                           first = logical page of the program the lists start at
+                                                           (a promotion is split by the demotion that frees its pages)
     ("sync_all",)                                          the host must join both streams here
     ``fills`` = [(uid, first_logical_page, gpu_pages)] executed after the epoch's sync."""
     iota: np.ndarray
@@ -489,12 +491,14 @@ class Sim:
                         # some of the pages are still being vacated: the part that lands in clean
                         # pages goes at once, the rest follows the demotion that frees it, one piece
                         # per demotion, in the order the demotions complete
-                        tags = self.gpu_alloc.last_tags
+                        tags = self.gpu_alloc.last_tags              # non-decreasing along the logical pages
                         for t in np.unique(tags):
-                            sel = tags == t
-                            ops.append(("promote", 0, p, slots[sel].copy(), pages[sel], int(t) if t > 0 else -1))
+                            sel = np.flatnonzero(tags == t)
+                            assert sel[-1] - sel[0] + 1 == sel.size     # a contiguous range of logical pages
+                            ops.append(("promote", 0, p, slots[sel].copy(), pages[sel], int(t) if t > 0 else -1,
+                                        int(sel[0])))
                     else:
-                        ops.append(("promote", 0, p, slots.copy(), pages, -1))
+                        ops.append(("promote", 0, p, slots.copy(), pages, -1, 0))
                     self.cpu_alloc.release(slots, tag=1)     # not reusable before the next join
                     self.gpu_pages[p] = pages
                     self.host_slots[p] = np.zeros(0, np.int32)

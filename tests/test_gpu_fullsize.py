@@ -97,8 +97,9 @@ def test_full_size_epochs_sampled_parity(mori, idx, f_busy):
             uid = int(sim.trace.uid[op[2]])
             promote = op[0] == "promote"
             slots, pages = (op[3], op[4]) if promote else (op[4], op[3])
+            first = op[6] if promote else 0                  # a promotion may cover a range of the program's pages
             js = _sample(len(pages), rng)
-            exp = _oracle_pages(seed, uid, js, sh, promote)
+            exp = _oracle_pages(seed, uid, [first + j for j in js], sh, promote)
             for want_page, j in zip(exp, js):
                 if promote:     # read the destination page back by a plain strided copy
                     have = pv[:, int(pages[j])].cpu().numpy()

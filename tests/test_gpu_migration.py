@@ -175,7 +175,7 @@ def test_cfg1_epochs_full_mirror(mori, path):
         _epochs_with_mirror(mori, W.get_config(1), seed, 20, path, 2)
 
 
-@pytest.mark.parametrize("idx,scale,epochs", [(2, 128, 20), (3, 128, 12), (4, 128, 16), (5, 128, 16)])
+@pytest.mark.parametrize("idx,scale,epochs", [(2, 128, 20), (3, 128, 12), (4, 128, 10), (5, 128, 10)])
 @pytest.mark.parametrize("path,kernel", [(1, 1), (2, 2)])
 def test_scaled_twins_epochs_full_mirror(mori, idx, scale, epochs, path, kernel):
     moved = _epochs_with_mirror(mori, W.get_config(idx, scale), 866, epochs, path, kernel)

@@ -79,7 +79,7 @@ def test_argument_errors(ctx, mori):
             ctx.mori_rank_partition_tiers(4, z, z, caps, z, z, z, z)
 
 
-@pytest.mark.parametrize("idx,scale,mid_frac,epochs", [(2, 64, 0.5, 30), (3, 128, 0.4, 20)])
+@pytest.mark.parametrize("idx,scale,mid_frac,epochs", [(2, 128, 0.5, 30), (3, 128, 0.4, 20)])
 def test_three_tier_epochs_all_three_pools_byte_exact(mori, idx, scale, mid_frac, epochs):
     """A whole epoch across three pools ("a second idleness threshold ... an intermediate
     tier"): mori_rank_partition_tiers decides (tiers and both move lists bit-exact vs the oracle),
