@@ -1,29 +1,37 @@
 #!/usr/bin/env python
 """bench.py -- the MORI hot path on B200, measured (driver contract: one JSON line on stdout).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--f-busy F] [--impl ours|reference]
+    python bench.py --leg copy_sweep          (auxiliary: the gather/scatter kernel alone and in-step)
 
 A *step* is one scheduling epoch: every row of SURVEY.md section 8(a) once --
 ``mori_rank_partition`` (a1-a4), ``mori_demote`` / ``mori_promote`` for every program the placement
 moves (a5, a6, concurrently in both link directions) and ``mori_sync`` (a7) -- on the seeded
 synthetic workload of BASELINE.json ``configs[1]`` (cfg 2, Llama-3-8B-shaped KV, 64 programs,
 60 GiB device pool, 128 GiB pinned arena).  Everything on the path runs in
-libmori.so (CUDA, sm_100a) through its C ABI; there is no CPU fallback.
+libmori.so (CUDA, sm_100a) through its C ABI; there is no CPU fallback.  After the headline config
+a single-GPU run measures every other BASELINE.json config the same way (``per_config``).
 
 Numbers on the line (DESIGN.md section 7 says how each is derived):
   value        migrated KV bytes / time of K epochs, GB/s.  The KV pool and the rank/partition
                inputs are resident in HBM when the timed region starts; timed on the device with
-               CUDA events (region A: rank/partition + read-back of the move lists, region B:
-               all demotes/promotes up to the join).  The page/slot allocator between A and B is
-               harness code (it stands in for the serving engine's allocator) and is not timed.
+               CUDA events (region A: rank/partition up to the arrival of its move lists in host
+               memory, region B: all demotes/promotes up to the join).  The page/slot allocator
+               between A and B, and the concatenation of its tables into the calls' arguments, are
+               harness code (they stand in for the serving engine's allocator) and are not timed.
+  frac_of_measured_link_peak, roofline_frac   the two headline fractions, right behind ``value``.
   e2e          the same epochs' metric through the public API from HOST buffers: idleness / size /
                previous-tier arrays copied host->device, lists device->host, host page tables
                into mori_demote / mori_promote, the allocator included, one timed region.
   roofline     the gather/scatter kernel of the STAGED path (the only HBM-bound kernel), timed
                live by the library's CUDA events around every launch inside the timed steps.
+  per_config   one record per BASELINE.json config: GB/s, fraction of the measured link peak, scale,
+               the ranker's capacities, in-step and standalone gather/scatter fractions.
   link         measured pinned-memcpy peaks of this box (denominators) and the achieved fractions.
   gather_scatter  the device halves alone (pool <-> contiguous device buffer), >= 4 GiB per launch.
-  cpu_baseline the CPU oracle (oracle/, as it stands) on this box's host cores, bounded sample.
+  rank_partition, eviction_order   the latency-bound entry points against the launch floor (mori_noop).
+  cpu_baseline the CPU oracle (oracle/, as it stands) on this box's host cores, 1 thread and all
+               cores, bounded sample, on the scaled twin of every config.
 """
 from __future__ import annotations
 
@@ -107,7 +115,7 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def measure_link_peak(arena, nbytes=GIB, reps=5, stream_chunks=1):
+def measure_link_peak(arena, nbytes=GIB, reps=5, stream_chunks=1, joined=False):
     """Pinned cudaMemcpyAsync of ONE contiguous buffer: D2H alone, H2D alone, both at once on
     two streams -- the host-link denominators (GB/s).  Uses the first bytes of the arena before
     the workload touches it, and a scratch device buffer."""
@@ -133,6 +141,14 @@ def measure_link_peak(arena, nbytes=GIB, reps=5, stream_chunks=1):
                 with torch.cuda.stream(s2):
                     d2.copy_(h2, non_blocking=True)
                 cur.wait_stream(s1); cur.wait_stream(s2)
+            elif joined:                                 # one direction, issued the way an epoch's transfers are:
+                s1.wait_event(e0)                        # on a side stream, joined to the timing stream on both ends
+                with torch.cuda.stream(s1):
+                    if do_d2h:
+                        h1.copy_(d1, non_blocking=True)
+                    else:
+                        d2.copy_(h2, non_blocking=True)
+                cur.wait_stream(s1)
             elif do_d2h:                                 # one direction: the copy alone between the two events
                 h1.copy_(d1, non_blocking=True)
             else:
@@ -531,12 +547,16 @@ def measure_config(args, cfg, seed, arena, link, steps, warmup, local, barrier, 
         sm = measure_link_peak(arena, nbytes=mean_b, reps=10)
         ach = sum(x["dem"] + x["pro"] for x in moving) / (sum(x["ms"] for x in moving) * 1e-3) / 1e9
         ach_b = sum(x["dem"] + x["pro"] for x in moving) / (sum(x["ms_b"] for x in moving) * 1e-3) / 1e9
+        smj = measure_link_peak(arena, nbytes=mean_b, reps=10, joined=True) if mean_b < (64 << 20) else sm
         out["size_matched"] = {"bytes": mean_b, "d2h_GBps": sm["d2h"], "h2d_GBps": sm["h2d"],
+                               "d2h_joined_GBps": smj["d2h"], "transfer_region_over_d2h_joined": ach_b / smj["d2h"],
                                "epochs_GBps": ach, "epochs_over_d2h": ach / sm["d2h"],
                                "transfer_region_GBps": ach_b, "transfer_region_over_d2h": ach_b / sm["d2h"],
                                "note": "one-direction denominator: epochs that move both ways can exceed it; "
                                        "`epochs` = rank/partition + transfers, `transfer_region` = the demote/promote "
-                                       "calls up to the join only (what a plain memcpy of the same bytes competes with)"}
+                                       "calls up to the join only (what a plain memcpy of the same bytes competes with); "
+                                       "`joined` = the same memcpy issued on a side stream and joined to the timing stream "
+                                       "on both ends, as an epoch's transfers are"}
 
     # ---- roofline of the HBM-bound kernel, from the library's per-launch CUDA events ---------------
     ncu = _load_ncu_traffic()
@@ -590,7 +610,9 @@ def _per_config_record(m, link, scale):
         rec["size_matched"] = {"bytes": smx["bytes"], "pinned_memcpy_GBps": smx["d2h_GBps"],
                                "epochs_GBps": smx["epochs_GBps"], "frac": smx["epochs_over_d2h"],
                                "transfer_region_GBps": smx["transfer_region_GBps"],
-                               "transfer_region_frac": smx["transfer_region_over_d2h"]}
+                               "transfer_region_frac": smx["transfer_region_over_d2h"],
+                               "pinned_memcpy_joined_GBps": smx["d2h_joined_GBps"],
+                               "transfer_region_frac_of_joined_memcpy": smx["transfer_region_over_d2h_joined"]}
     if m["roofline"]:
         rec["in_step_gather_scatter_frac_of_measured_hbm"] = m["roofline"]["frac"]
         rec["in_step_launches"] = m["roofline"]["launches"]

@@ -501,6 +501,16 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
                          (const void*)mori::rank_partition_multi_kernel<2>, (const void*)mori::rank_partition_multi_kernel<4>,
                          (const void*)mori::rank_partition_multi_kernel<8>};
     for (const void* f : hot) CKC(cudaFuncGetAttributes(&fa, f));
+    // ... and the one-launch movers really run once, on nothing (n_pages = 0): the first launch of a
+    // kernel costs tens of microseconds more than the next, which for a 272 KiB move is the move
+    mori::CopyArgs z{};
+    z.n_layers = 1; z.chunk_bytes = 16; z.piece_bytes = 16; z.pieces_per_chunk = 1; z.stages = 2; z.store_lag = 1;
+    mori::copy_pages_small<true, mori::kSmallFewPages><<<1, mori::kLdstThreads>>>(z, mori::SmallIds<mori::kSmallFewPages>{});
+    mori::copy_pages_small<false, mori::kSmallFewPages><<<1, mori::kLdstThreads>>>(z, mori::SmallIds<mori::kSmallFewPages>{});
+    mori::copy_pages_small<true, mori::kSmallMaxPages><<<1, mori::kLdstThreads>>>(z, mori::SmallIds<mori::kSmallMaxPages>{});
+    mori::copy_pages_small<false, mori::kSmallMaxPages><<<1, mori::kLdstThreads>>>(z, mori::SmallIds<mori::kSmallMaxPages>{});
+    CKC(cudaGetLastError());
+    CKC(cudaDeviceSynchronize());
   }
   // The attribute is per function and PROCESS-wide: every context sets it to the device's opt-in
   // maximum, so contexts with different ring sizes never lower it under one another.
@@ -641,7 +651,7 @@ int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idlen
   if (n > mori::kRankMaxThreads) {
     // more than one CTA's worth: rank by counting on every SM, last CTA partitions
     const int grid = std::min(c->sm_count, (n + 7) / 8);
-    const size_t smem_m = sizeof(uint64_t) * ((size_t)n + 33) + 2 * sizeof(long long);
+    const size_t smem_m = sizeof(uint64_t) * ((size_t)n + 66) + 2 * sizeof(long long);
     const unsigned long long slot_m = c->rank_seq++ % kRankTickets;
     unsigned int* tk = c->rank_tickets + slot_m;
     int32_t* so = c->sticky_order + slot_m * (size_t)c->cfg.max_programs;
@@ -659,7 +669,7 @@ int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idlen
     c->launches += 1;
     return MORI_OK;
   }
-  const size_t smem = sizeof(uint64_t) * (n_pad + 33) + 2 * sizeof(long long);
+  const size_t smem = sizeof(uint64_t) * (n_pad + 66) + 2 * sizeof(long long);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   cudaError_t e;
   long long* u = reinterpret_cast<long long*>(used);
@@ -682,7 +692,7 @@ int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idl
   int n_pad = 1024;
   while (n_pad < n) n_pad <<= 1;
   const int grid = std::max(1, std::min(c->sm_count, (n + 7) / 8));
-  const size_t smem = sizeof(uint64_t) * (2 * (size_t)n + 33) + 4 * sizeof(long long);
+  const size_t smem = sizeof(uint64_t) * (2 * (size_t)n + 99) + 4 * sizeof(long long);
   const unsigned long long slot = c->rank_seq++ % kRankTickets;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   long long* u = reinterpret_cast<long long*>(used);

@@ -54,6 +54,48 @@ __device__ __forceinline__ uint64_t block_excl_scan(uint64_t v, uint64_t* warp_t
   return warp_tot[warp] + incl - v;
 }
 
+// The same for N values per thread at once (one set of barriers for all of them): v[] come in as
+// the thread's values and go out as their exclusive prefixes, total[] gets the sums.  warp_tot is
+// 33 * N words of shared memory.
+template <int N>
+__device__ __forceinline__ void block_excl_scan_n(uint64_t (&v)[N], uint64_t* warp_tot, uint64_t (&total)[N]) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  uint64_t incl[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    incl[k] = v[k];
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      uint64_t o = __shfl_up_sync(0xFFFFFFFFu, incl[k], d);
+      if (lane >= d) incl[k] += o;
+    }
+  }
+  __syncthreads();  // warp_tot may still be read from a previous scan
+  if (lane == 31) {
+#pragma unroll
+    for (int k = 0; k < N; ++k) warp_tot[33 * k + warp] = incl[k];
+  }
+  __syncthreads();
+  if (warp < N) {                                    // warp k scans the warp totals of value k
+    uint64_t* wt = warp_tot + 33 * warp;
+    uint64_t w = lane < n_warps ? wt[lane] : 0;
+    uint64_t wi = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      uint64_t o = __shfl_up_sync(0xFFFFFFFFu, wi, d);
+      if (lane >= d) wi += o;
+    }
+    if (lane < n_warps) wt[lane] = wi - w;
+    if (lane == 31) wt[32] = wi;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    total[k] = warp_tot[33 * k + 32];
+    v[k] = warp_tot[33 * k + warp] + incl[k] - v[k];
+  }
+}
+
 // Ranking by counting, shared by every kernel that orders more keys than one CTA sorts well
 // (rank_partition_multi, rank_tiers, sticky_rebalance, bfd_assign).  Keys are unique, so
 // position(i) = #{j : key_j < key_i}.  Every CTA holds all n keys in its shared memory (built by
@@ -121,7 +163,7 @@ __device__ __forceinline__ bool rank_by_counting128(int n, const ulonglong2* __r
 }
 
 // Steps a2-a4 for one CTA whose thread t owns ranks [t*IPT, (t+1)*IPT): prog[i] is the program at
-// rank t*IPT + i (or -1 past n).  warp_tot = 33 words, bcast = 2 words of shared memory.
+// rank t*IPT + i (or -1 past n).  warp_tot = 66 words, bcast = 2 words of shared memory.
 template <int IPT>
 __device__ __forceinline__ void partition_tail(
     int n, const int (&prog)[IPT], const int32_t* __restrict__ kv_pages,
@@ -213,9 +255,10 @@ __device__ __forceinline__ void partition_tail(
 
   // ---- a4: compaction by rank.  Ascending lists take the exclusive count below; descending
   //          lists (demote, drop: most idle first) take total - inclusive count ------------------
-  uint64_t ptot, rtot;
-  uint64_t pex = block_excl_scan(packed, warp_tot, &ptot);
-  uint64_t rex = block_excl_scan(rsv, warp_tot, &rtot);
+  uint64_t pr[2] = {packed, rsv}, prt[2];
+  block_excl_scan_n<2>(pr, warp_tot, prt);                           // warp_tot: 66 words
+  uint64_t pex = pr[0], rex = pr[1];
+  const uint64_t ptot = prt[0], rtot = prt[1];
 #pragma unroll
   for (int i = 0; i < IPT; ++i) {
     const int k = cls[i];
@@ -246,8 +289,8 @@ rank_partition_kernel(int n, int n_pad, const float* __restrict__ idleness,
                       int32_t* __restrict__ list_counts) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n_pad]
-  uint64_t* warp_tot = keys + n_pad;                                 // [33]
-  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
+  uint64_t* warp_tot = keys + n_pad;                                 // [2][33]
+  long long* bcast = reinterpret_cast<long long*>(warp_tot + 66);    // [2]
   const int tid = threadIdx.x, nt = blockDim.x;
 
   // ---- a1: keys ------------------------------------------------------------------------------
@@ -315,8 +358,8 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
                             unsigned int* __restrict__ ticket) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
-  uint64_t* warp_tot = keys + n;                                     // [33]
-  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [2]
+  uint64_t* warp_tot = keys + n;                                     // [2][33]
+  long long* bcast = reinterpret_cast<long long*>(warp_tot + 66);    // [2]
   const int tid = threadIdx.x;
   for (int i = tid; i < n; i += blockDim.x)
     keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;

@@ -59,8 +59,8 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
                         int32_t* __restrict__ order, unsigned int* __restrict__ ticket) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ulonglong2* keys = reinterpret_cast<ulonglong2*>(smem_raw);        // [n] (x = low half, y = high half)
-  uint64_t* warp_tot = reinterpret_cast<uint64_t*>(keys + n);        // [33]
-  long long* bcast = reinterpret_cast<long long*>(warp_tot + 33);    // [4]
+  uint64_t* warp_tot = reinterpret_cast<uint64_t*>(keys + n);        // [3][33]
+  long long* bcast = reinterpret_cast<long long*>(warp_tot + 99);    // [4]
   const int tid = threadIdx.x;
 
   for (int p = tid; p < n; p += blockDim.x) {
@@ -99,10 +99,11 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
   __syncthreads();                                                   // keys are dead: smem is reused below
 
   // ---- demotion: victims = the prefix of group 0 whose predecessors do not free enough ----------
-  uint64_t tot_g, tot_c, tot;
-  long long run = (long long)block_excl_scan((uint64_t)sum_g, warp_tot, &tot_g);   // freed BEFORE this thread
-  block_excl_scan((uint64_t)sum_c, warp_tot, &tot_c);
-  const long long usage_gpu0 = (long long)tot_g, usage_cpu0 = (long long)tot_c;
+  uint64_t tot;
+  uint64_t sc2[2] = {(uint64_t)sum_g, (uint64_t)sum_c}, tt2[2];
+  block_excl_scan_n<2>(sc2, warp_tot, tt2);                          // one set of barriers for both sums
+  long long run = (long long)sc2[0];                                 // freed BEFORE this thread
+  const long long usage_gpu0 = (long long)tt2[0], usage_cpu0 = (long long)tt2[1];
   bool victim[IPT];
   int n_v = 0;
   long long freed_mine = 0;
@@ -115,10 +116,10 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
       vsize[tid * IPT + i] = (int32_t)sz[i];
     }
   }
-  block_excl_scan((uint64_t)n_v, warp_tot, &tot);
-  const int v = (int)tot;                                            // victims are positions [0, v)
-  block_excl_scan((uint64_t)freed_mine, warp_tot, &tot);
-  const long long freed = (long long)tot;
+  uint64_t vf2[2] = {(uint64_t)n_v, (uint64_t)freed_mine};
+  block_excl_scan_n<2>(vf2, warp_tot, tt2);
+  const int v = (int)tt2[0];                                         // victims are positions [0, v)
+  const long long freed = (long long)tt2[1];
 
   // ---- each victim: CPU queue if it fits, else Waiting, in victim order -----------------
   if (usage_cpu0 + freed <= cap_cpu) {                               // all of them fit
@@ -187,12 +188,12 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
     }
     if (victim[i]) packed += vdest[tid * IPT + i] == 1 ? 1ull : (1ull << 32);
   }
-  uint64_t ptot;
-  uint64_t pex = block_excl_scan(packed, warp_tot, &ptot);
-  block_excl_scan((uint64_t)up_g, warp_tot, &tot);
-  const long long promoted_pages = (long long)tot;
-  block_excl_scan((uint64_t)down_c, warp_tot, &tot);
-  const long long promoted_from_cpu = (long long)tot;
+  uint64_t pud[3] = {packed, (uint64_t)up_g, (uint64_t)down_c}, tt3[3];
+  block_excl_scan_n<3>(pud, warp_tot, tt3);
+  uint64_t pex = pud[0];
+  const uint64_t ptot = tt3[0];
+  const long long promoted_pages = (long long)tt3[1];
+  const long long promoted_from_cpu = (long long)tt3[2];
 
   // ---- outputs ----------------------------------------------------------------------------------
 #pragma unroll

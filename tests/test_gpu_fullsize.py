@@ -23,6 +23,13 @@ def _mem_available():
     return 0
 
 
+def _mem_total():
+    for line in open("/proc/meminfo"):
+        if line.startswith("MemTotal:"):
+            return int(line.split()[1]) * 1024
+    return 0
+
+
 def _sample(n, rng, k=4):
     js = {0, n - 1} | {int(x) for x in rng.integers(0, n, size=min(k, n))}
     return sorted(js)
@@ -69,6 +76,8 @@ def test_full_size_epochs_sampled_parity(mori, idx, f_busy):
     scale = _scale_that_fits(idx)
     print(f"cfg {idx}: scale {scale} (MemAvailable {_mem_available() / GIB:.0f} GiB)")
     assert scale <= 2, "this box cannot hold even the half-size arena"
+    if idx in (2, 3, 5) and _mem_total() >= 190 * GIB:
+        assert scale == 1, f"cfg {idx} must run as written on a 196 GiB host (MemAvailable {_mem_available() / GIB:.0f} GiB)"
     cfg = W.get_config(idx, scale, f_busy)
     sh = cfg.shape
     arena_bytes = cfg.cpu_pool_pages * sh.page_bytes
