@@ -79,8 +79,9 @@ def test_argument_errors(ctx, mori):
             ctx.mori_rank_partition_tiers(4, z, z, caps, z, z, z, z)
 
 
-@pytest.mark.parametrize("idx,scale,mid_frac,epochs", [(2, 128, 0.5, 30), (3, 128, 0.4, 20)])
-def test_three_tier_epochs_all_three_pools_byte_exact(mori, idx, scale, mid_frac, epochs):
+@pytest.mark.parametrize("idx,scale,mid_frac,epochs,slack_div", [(2, 128, 0.5, 30, 2), (3, 128, 0.4, 20, 2),
+                                                                   (2, 128, 0.35, 32, 0)])
+def test_three_tier_epochs_all_three_pools_byte_exact(mori, idx, scale, mid_frac, epochs, slack_div):
     """A whole epoch across three pools ("a second idleness threshold ... an intermediate
     tier"): mori_rank_partition_tiers decides (tiers and both move lists bit-exact vs the oracle),
     mori_demote / mori_promote of the three pair-contexts move the bytes (pool <-> device-resident
@@ -94,14 +95,17 @@ def test_three_tier_epochs_all_three_pools_byte_exact(mori, idx, scale, mid_frac
     seed = 866
     mid_ids = int(cfg.gpu_pool_pages * mid_frac)
     pool_ids = [cfg.gpu_pool_pages, mid_ids, cfg.cpu_pool_pages]
-    caps = [cfg.cap_gpu_pages, max(0, mid_ids - cfg.max_program_pages // 2), cfg.cap_cpu_pages]
+    # slack_div = 0: the ranker is given every middle slot, so the planner must split epochs into
+    # phases separated by joins (an id freed in a phase is not reused before the next join)
+    slack = cfg.max_program_pages // slack_div if slack_div else 0
+    caps = [cfg.cap_gpu_pages, max(0, mid_ids - slack), cfg.cap_cpu_pages]
     sim = W.SimTiers(cfg, seed, pool_ids, caps)
     r = TierRunner(cfg, seed, mid_ids, staging_bytes=max(sh.page_bytes * 3, 1 << 20))
     r.host.zero_()
     pool_m = np.zeros(sh.n_layers * pool_ids[0] * sh.chunk_bytes, np.uint8)
     mid_m = np.zeros(mid_ids * sh.page_bytes, np.uint8)
     host_m = np.zeros(pool_ids[2] * sh.page_bytes, np.uint8)
-    pairs, moved = set(), 0
+    pairs, moved, joins = set(), 0, 0
     for e in range(epochs):
         plan = sim.begin_epoch()
         want = oracle.rank_partition_tiers(plan.iota, plan.kv_pages, caps, plan.prev_tier)
@@ -122,9 +126,12 @@ def test_three_tier_epochs_all_three_pools_byte_exact(mori, idx, scale, mid_frac
         assert np.array_equal(r.pool.cpu().numpy(), pool_m), (e, "GPU pool")
         assert np.array_equal(r.mid.cpu().numpy(), mid_m), (e, "middle arena")
         assert np.array_equal(r.host.numpy(), host_m), (e, "host arena")
+        joins += sum(1 for op in plan.ops if op[0] == "sync_all")
         for op in plan.ops:
             if op[0] == "move":
                 pairs.add((op[2], op[3]))
                 moved += len(op[4])
     r.close()
     assert moved > 0 and {(0, 1), (1, 0), (1, 2)} <= pairs, pairs
+    if slack_div == 0:
+        assert joins > 0

@@ -209,14 +209,19 @@ def _small_cfg2():
     return replace(W.get_config(2, 128), shape=W.KVShape(4, 2, 32, 16))
 
 
-def test_three_pool_epochs_keep_every_resident_page_intact():
+@pytest.mark.parametrize("mid_ids,mid_slack", [(160, None), (120, 0)])
+def test_three_pool_epochs_keep_every_resident_page_intact(mid_ids, mid_slack):
+    """mid_slack = physical middle slots the ranker is NOT given (None: one largest program).  With no
+    slack at all the planner must split epochs into phases separated by joins (ids freed in a phase
+    are not reused before the next join); the bytes must come out right either way."""
     cfg = _small_cfg2()
-    mid_ids, mid_cap = 160, 160 - cfg.max_program_pages
+    mid_cap = mid_ids - (cfg.max_program_pages if mid_slack is None else mid_slack)
     pool_ids = [cfg.gpu_pool_pages, mid_ids, cfg.cpu_pool_pages]
     caps = [cfg.cap_gpu_pages, mid_cap, cfg.cap_cpu_pages]
-    seen = {"pairs": set(), "pages": 0}
+    seen = {"pairs": set(), "pages": 0, "joins": 0}
 
     def on_epoch(e, sim, plan, res, mirrors):
+        seen["joins"] += sum(1 for op in plan.ops if op[0] == "sync_all")
         for op in plan.ops:
             if op[0] == "move":
                 seen["pairs"].add((op[2], op[3]))
@@ -230,6 +235,8 @@ def test_three_pool_epochs_keep_every_resident_page_intact():
     assert seen["pages"] > 500
     # the hierarchy was really exercised: bytes went down and up between all neighbouring pairs
     assert {(0, 1), (1, 0), (1, 2)} <= seen["pairs"], seen["pairs"]
+    if mid_slack == 0:
+        assert seen["joins"] >= 5, "a middle pool with no slack must force mid-epoch joins"
 
 
 def test_three_pool_epochs_with_an_empty_middle_tier_are_the_two_pool_epochs():
