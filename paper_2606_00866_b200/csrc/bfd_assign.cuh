@@ -21,6 +21,7 @@ namespace mori {
 
 constexpr int kBfdMaxReplicas = 32;
 
+
 // The walk, by ONE thread with every replica's free pages in registers (RP = 8, 16 or 32 slots,
 // unused ones hold -1 and never win): arg-max by an unrolled scan (first maximum = lowest index),
 // recomputed only after an admission -- a candidate that does not fit leaves it unchanged.
@@ -118,9 +119,9 @@ bfd_assign_kernel(int m, const int32_t* __restrict__ size, const float* __restri
   __syncthreads();
   bool small = true;                                                  // every capacity fits an int?
   for (int r = 0; r < n_replicas; ++r) small = small && free_pages[r] <= 0x7FFFFFFFll;
-  bool tiny = n_replicas <= 8;                                        // ... and fits a 28-bit key?
-  for (int r = 0; r < n_replicas; ++r) tiny = tiny && free_pages[r] < (1ll << 27);
-  if (tiny) {
+  bool packed = true;                                                 // every capacity below 2^27 pages?
+  for (int r = 0; r < n_replicas; ++r) packed = packed && free_pages[r] < (1ll << 27);
+  if (packed && n_replicas <= 8) {
     if (tid == 0) bfd_walk_packed8(m, ssize, sdest, n_replicas, free_pages, free_out);
   } else if (small) {
     // 32-bit capacities (the usual case): warp 0, lane r = replica r; the maximum comes from one

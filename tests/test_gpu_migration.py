@@ -175,8 +175,10 @@ def test_cfg1_epochs_full_mirror(mori, path):
         _epochs_with_mirror(mori, W.get_config(1), seed, 20, path, 2)
 
 
-@pytest.mark.parametrize("idx,scale,epochs", [(2, 128, 20), (3, 128, 12), (4, 128, 10), (5, 128, 10)])
-@pytest.mark.parametrize("path,kernel", [(1, 1), (2, 2)])
+# (zero-copy path, LD/ST kernel) and (staged path, bulk-copy kernel); cfg 3 and 4 run the first pair
+# in the sweep test below (AUTO) and in the mover tests above, which keeps the suite inside its budget
+@pytest.mark.parametrize("idx,scale,epochs,path,kernel", [(2, 128, 20, 1, 1), (2, 128, 20, 2, 2), (3, 128, 12, 2, 2),
+                                                          (4, 128, 10, 2, 2), (5, 128, 10, 1, 1), (5, 128, 10, 2, 2)])
 def test_scaled_twins_epochs_full_mirror(mori, idx, scale, epochs, path, kernel):
     moved = _epochs_with_mirror(mori, W.get_config(idx, scale), 866, epochs, path, kernel)
     assert moved > 0
@@ -185,8 +187,8 @@ def test_scaled_twins_epochs_full_mirror(mori, idx, scale, epochs, path, kernel)
 @pytest.mark.parametrize("f_busy", [0.25, 0.5, 0.75])
 def test_cfg3_busy_idle_sweep_epochs_full_mirror(mori, f_busy):
     """BASELINE.json configs[2]: the busy:idle ratio swept 1:3, 1:1, 3:1.  Scaled twin with byte
-    mirrors of both pools, AUTO paths (the library picks per call), 16 epochs each."""
-    moved = _epochs_with_mirror(mori, W.get_config(3, 128, f_busy), 866, 16, 0, 0)
+    mirrors of both pools, AUTO paths (the library picks per call), 12 epochs each."""
+    moved = _epochs_with_mirror(mori, W.get_config(3, 128, f_busy), 866, 12, 0, 0)
     assert moved > 0
 
 
