@@ -151,58 +151,9 @@ class GpuRunner:
 
     # -- a5-a7 ---------------------------------------------------------------------------------
     def prepare(self, plan: W.EpochPlan, merge=True):
-        """Turns the epoch's moves into the argument lists of the calls that will carry them (host
-        work, like the allocator that produced the tables).  A move is a flat list of pages
-        (include/mori.h), so the demotions of an epoch go out as ONE ``mori_demote`` per stretch of
-        the plan that no promotion depends on, and the promotions likewise as one ``mori_promote``
-        per stretch with the same dependency: fewer calls, fewer ragged last staging segments, and
-        the page order inside a call is the plan's (the paper's move order, P:L206 / L208).
-        ``merge=False``: one call per program.  -> (steps, need_tickets) for ``issue``."""
-        steps = []                        # ("d", pages, slots, n, [k ...]) | ("p", slots, pages, n, dep) | ("sync",)
-        dem, pro, pro_dep = [], [], 0
-        flushed = set()
-
-        def cat(parts):
-            return np.ascontiguousarray(parts[0] if len(parts) == 1 else np.concatenate(parts), dtype=np.int32)
-
-        def flush_dem():
-            if dem:
-                g, h = cat([o[3] for o in dem]), cat([o[4] for o in dem])
-                steps.append(("d", g, h, g.size, [o[1] for o in dem]))
-                flushed.update(o[1] for o in dem)
-                dem.clear()
-
-        def flush_pro():
-            nonlocal pro_dep
-            if pro:
-                h, g = cat([o[3] for o in pro]), cat([o[4] for o in pro])
-                steps.append(("p", h, g, g.size, pro_dep))
-                pro.clear()
-            pro_dep = 0
-
-        for op in plan.ops:
-            if op[0] == "demote":
-                dem.append(op)
-                if not merge:
-                    flush_dem()
-            elif op[0] == "promote":
-                dep = op[5] if op[5] > 0 else 0
-                if pro and dep != pro_dep:        # a different dependency: its own call
-                    flush_pro()
-                if dep > 0 and dep not in flushed:
-                    flush_dem()                   # the demotion it follows ends its call here, so the
-                                                  # promotion waits for that much and no more
-                pro.append(op)
-                pro_dep = dep
-                if not merge:
-                    flush_pro()
-            elif op[0] == "sync_all":
-                flush_dem(); flush_pro()
-                steps.append(("sync",))
-                flushed.clear()
-        # both directions start together: the demote call first (it is what vacates pages)
-        flush_dem(); flush_pro()
-        return steps, any(st[0] == "p" and st[4] > 0 for st in steps)
+        """The argument lists of the calls that will carry the epoch's moves (host work, like the
+        allocator that produced the tables): ``workload.plan_calls``.  -> (steps, need_tickets)."""
+        return W.plan_calls(plan, merge=merge)
 
     def issue(self, prepared, sync=True):
         """The C-ABI calls of one epoch, nothing else: one ``mori_demote`` / ``mori_promote`` per

@@ -1,9 +1,12 @@
 """Seeded synthetic inputs for the MORI hot path: configs, agent trace, page contents, allocator.
 
 This module is the ONE piece shared by the CPU oracle's tests and the CUDA path's tests/bench.
-It holds none of the method's arithmetic: no ranking, no partition, no page movement.  It makes
-inputs (idleness scores, KV sizes, page tables, page bytes) and turns a placement that SOMEONE
-ELSE computed into page/slot tables.  It imports neither ``oracle`` nor the CUDA binding.
+It holds no ranking, no partition and no page movement.  It makes inputs (idleness scores, KV
+sizes, page tables, page bytes) and turns a placement that SOMEONE ELSE computed into page/slot
+tables and call lists.  It imports neither ``oracle`` nor the CUDA binding.  One formula of the
+paper does live here, because the trace must produce the hot path's input: ``windowed_idleness``,
+Eq. (1) in float64.  Neither ``oracle/oracle.c`` nor ``csrc/idleness.cuh`` calls or shares it (each
+states Eq. (1) itself); the oracle's pins use it as one more independent evaluation.
 
 Recipe (BASELINE.json ``configs``): the paper replays private coding-agent
 traces that are not available; a two-phase synthetic trace stands in, shaped by what
@@ -409,6 +412,66 @@ class EpochPlan:
     fills: list = field(default_factory=list)
     demote_pages: int = 0
     promote_pages: int = 0
+
+
+def plan_calls(plan: "EpochPlan", merge: bool = True):
+    """Turns the epoch's moves into the argument lists of the mover calls that will carry them.
+    A move is a flat list of pages (include/mori.h), so the demotions of an epoch go out as ONE
+    demote call per stretch of the plan that no promotion depends on, and the promotions likewise
+    as one promote call per stretch with the same dependency: fewer calls, fewer ragged last staging
+    segments, and the page order inside a call is the plan's (the paper's move order, P:L206 /
+    L208).  ``merge=False``: one call per program.
+
+    -> (steps, need_tickets); steps, in issue order:
+         ("d", gpu_pages i32[], host_slots i32[], n, [k ...])   k = the plan's demote numbers it carries
+         ("p", host_slots i32[], gpu_pages i32[], n, dep)       dep = demote number it must follow, or 0
+         ("sync",)                                              the host joins both directions here
+    A promotion's ``dep`` is always carried by a demote step issued BEFORE it."""
+    steps = []
+    dem, pro, pro_dep = [], [], 0
+    flushed = set()
+
+    def cat(parts):
+        return np.ascontiguousarray(parts[0] if len(parts) == 1 else np.concatenate(parts), dtype=np.int32)
+
+    def flush_dem():
+        if dem:
+            g, h = cat([o[3] for o in dem]), cat([o[4] for o in dem])
+            steps.append(("d", g, h, g.size, [o[1] for o in dem]))
+            flushed.update(o[1] for o in dem)
+            dem.clear()
+
+    def flush_pro():
+        nonlocal pro_dep
+        if pro:
+            h, g = cat([o[3] for o in pro]), cat([o[4] for o in pro])
+            steps.append(("p", h, g, g.size, pro_dep))
+            pro.clear()
+        pro_dep = 0
+
+    for op in plan.ops:
+        if op[0] == "demote":
+            dem.append(op)
+            if not merge:
+                flush_dem()
+        elif op[0] == "promote":
+            dep = op[5] if op[5] > 0 else 0
+            if pro and dep != pro_dep:        # a different dependency: its own call
+                flush_pro()
+            if dep > 0 and dep not in flushed:
+                flush_dem()                   # the demotion it follows ends its call here, so the
+                                              # promotion waits for that much and no more
+            pro.append(op)
+            pro_dep = dep
+            if not merge:
+                flush_pro()
+        elif op[0] == "sync_all":
+            flush_dem(); flush_pro()
+            steps.append(("sync",))
+            flushed.clear()
+    # both directions start together: the demote call first (it is what vacates pages)
+    flush_dem(); flush_pro()
+    return steps, any(st[0] == "p" and st[4] > 0 for st in steps)
 
 
 class Sim:

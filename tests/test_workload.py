@@ -183,3 +183,53 @@ def test_alloc_run_gives_one_contiguous_clean_run_or_falls_back():
     with pytest.raises(MemoryError):
         a.alloc_run(5)
     assert a.alloc_run(0)[0].size == 0
+
+
+def test_plan_calls_keeps_order_bytes_and_dependencies():
+    """The merged call lists carry exactly the plan's pages, each direction in plan order, and a
+    promotion that lands in pages a demotion vacates is issued after the call that carries it."""
+    import oracle
+    cfg = W.get_config(3, 32, 0.5)          # the config whose promotions do depend on demotions
+    sim = W.Sim(cfg, 866)
+    seen_dep = seen_split = 0
+    for e in range(120):
+        plan = sim.begin_epoch()
+        res = oracle.rank_partition(plan.iota, plan.kv_pages, plan.prev_tier, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+        sim.apply_placement(res["tier"], res["lists"])
+        for merge in (True, False):
+            steps, need = W.plan_calls(plan, merge=merge)
+            dem_ops = [op for op in plan.ops if op[0] == "demote"]
+            pro_ops = [op for op in plan.ops if op[0] == "promote"]
+            d_steps = [st for st in steps if st[0] == "d"]
+            p_steps = [st for st in steps if st[0] == "p"]
+            cat = lambda xs: np.concatenate(xs) if xs else np.zeros(0, np.int32)
+            assert np.array_equal(cat([st[1] for st in d_steps]), cat([op[3] for op in dem_ops]))
+            assert np.array_equal(cat([st[2] for st in d_steps]), cat([op[4] for op in dem_ops]))
+            # promotions: same multiset of (slot, page) pairs, and plan order inside every dependency class
+            got = np.stack([cat([st[1] for st in p_steps]), cat([st[2] for st in p_steps])]) if p_steps else np.zeros((2, 0))
+            want = np.stack([cat([op[3] for op in pro_ops]), cat([op[4] for op in pro_ops])]) if pro_ops else np.zeros((2, 0))
+            assert sorted(map(tuple, got.T.tolist())) == sorted(map(tuple, want.T.tolist()))
+            carried = set()
+            for st in steps:
+                if st[0] == "d":
+                    carried.update(st[4])
+                elif st[0] == "p" and st[4] > 0:
+                    assert st[4] in carried, "a dependent promotion was issued before its demotion"
+                elif st[0] == "sync":
+                    carried.clear()
+            assert need == any(op[5] > 0 for op in pro_ops)
+            if not merge:
+                assert len(d_steps) == len(dem_ops) and len(p_steps) == len(pro_ops)
+        seen_dep += any(op[0] == "promote" and op[5] > 0 for op in plan.ops)
+        per_prog = {}
+        for op in plan.ops:
+            if op[0] == "promote":
+                per_prog.setdefault(op[2], []).append(op)
+        for ops in per_prog.values():          # a split promotion covers its program's pages once, in order
+            if len(ops) > 1:
+                seen_split += 1
+                firsts = [op[6] for op in ops]
+                assert firsts == sorted(firsts) and firsts[0] == 0
+                assert all(firsts[i] + len(ops[i][3]) == firsts[i + 1] for i in range(len(ops) - 1))
+        sim.end_epoch()
+    assert seen_dep > 0 and seen_split > 0, "the trace never produced a dependent promotion"
