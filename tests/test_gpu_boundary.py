@@ -188,3 +188,40 @@ def test_eviction_order_alternating_tiers_keeps_both_graphs(mori):
             want = oracle.eviction_order(0 if which == mori.TIER_GPU else 1, owner, ptier, last)
             assert np.array_equal(vic.cpu().numpy()[:int(nres.item())], want), (rep, which)
     m.close()
+
+
+def test_profile_timeline_and_launch_floor(mori):
+    """mori_profile(ctx, 2) keeps every kernel and every staging segment's DMAs of a call as
+    [start, end) on one clock; mori_noop is one (empty) launch."""
+    L, H, D, T, P, S = 2, 8, 128, 16, 256, 256                  # 128 KiB pages
+    chunk = 2 * H * T * D * 2
+    m, pool, arena, pool_m, arena_m, _ = _ctx(mori, L, H, D, T, P, S, path=2, kernel=2, staging=40 * L * chunk, seed=8)
+    g = np.arange(100, dtype=np.int32)
+    h = np.arange(100, dtype=np.int32)
+    m.mori_profile(2)
+    m.mori_demote(g, h)
+    m.mori_promote(h, (g + 120).astype(np.int32))
+    m.mori_sync(mori.BOTH)
+    for which in (mori.DEMOTE, mori.PROMOTE):
+        rows = m.mori_profile_timeline(which)
+        kern = [r for r in rows if r[0] == 0]
+        dma = [r for r in rows if r[0] == 1]
+        assert len(kern) == len(dma) == 3                        # segments of 40, 40, 20 pages
+        assert sum(r[3] for r in kern) == sum(r[3] for r in dma) == 100 * L * chunk
+        assert all(0 <= r[1] < r[2] for r in rows)
+        for k, d in zip(sorted(kern, key=lambda r: r[1]), sorted(dma, key=lambda r: r[1])):
+            if which == mori.DEMOTE:
+                assert k[2] <= d[1] + 1e-3                       # a segment's DMA follows its gather
+            else:
+                assert d[2] <= k[1] + 1e-3                       # a segment's scatter follows its DMA
+    ms, launches, nbytes = m.mori_profile_read(mori.DEMOTE)
+    assert launches == 3 and nbytes == 100 * L * chunk           # kernels only, as with mori_profile(1)
+    m.mori_profile(False)
+    l0 = m.mori_launch_count()
+    m.mori_noop()
+    torch.cuda.synchronize()
+    assert m.mori_launch_count() - l0 == 1
+    oracle.demote(L, chunk, pool_m, arena_m, g, h)
+    oracle.promote(L, chunk, pool_m, arena_m, h, (g + 120).astype(np.int32))
+    assert np.array_equal(arena.numpy(), arena_m) and np.array_equal(pool.cpu().numpy(), pool_m)
+    m.close()
