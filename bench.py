@@ -928,6 +928,84 @@ def copy_kernel_sweep(args):
                                   "random page ids, consecutive slots", "rows": rows}))
 
 
+def three_tier_leg(args):
+    """`--leg three_tier`: the movers of a three-tier hierarchy (GPU pool, a middle arena in device memory
+    -- a second buffer of this GPU standing in for a peer GPU's HBM -- and the pinned host arena;
+    P:L339-351) one pair and one direction at a time, 4 GiB per move, then whole epochs driven by
+    mori_rank_partition_tiers.  cfg 2 at scale 4.  One JSON line."""
+    import torch
+    from paper_2606_00866_b200 import binding, workload as W
+    from paper_2606_00866_b200.harness import TierRunner
+    cfg = W.get_config(2, args.scale or 4)
+    sh = cfg.shape
+    mid_ids = cfg.gpu_pool_pages // 2
+    arena = binding.Mori.mori_host_alloc(cfg.cpu_pool_pages * sh.page_bytes)
+    r = TierRunner(cfg, SEED, mid_ids, host_arena=arena)
+    r.pool.random_(0, 255)
+    rng = np.random.default_rng(SEED)
+    n = int(min(4 * GIB // sh.page_bytes, mid_ids, cfg.gpu_pool_pages // 2, cfg.cpu_pool_pages // 2))
+    cur = torch.cuda.current_stream()
+    pairs = {}
+    for name, ctx, n_fast, n_slow in (("pool_mid", r.pool_mid, cfg.gpu_pool_pages, mid_ids),
+                                      ("pool_host", r.pool_host, cfg.gpu_pool_pages, cfg.cpu_pool_pages),
+                                      ("mid_host", r.mid_host, mid_ids, cfg.cpu_pool_pages)):
+        fast = rng.permutation(n_fast)[:n].astype(np.int32)          # scattered ids in the faster pool
+        slow = np.arange(n, dtype=np.int32)                          # one run of slots in the slower one
+        ent = {}
+        for direction in ("down", "up"):
+            ts = []
+            for _ in range(4):
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(cur)
+                ctx.mori_after_stream(binding.BOTH, cur)
+                if direction == "down":
+                    ctx.mori_demote(fast, slow, want_ticket=False)
+                else:
+                    ctx.mori_promote(slow, fast, want_ticket=False)
+                ctx.mori_stream_wait(cur, binding.BOTH)
+                e1.record(cur)
+                ctx.mori_sync(binding.BOTH)
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1) * 1e-3)
+            ent[direction + "_GBps"] = n * sh.page_bytes / float(np.median(ts[1:])) / 1e9
+        ent["GiB_per_move"] = n * sh.page_bytes / GIB
+        pairs[name] = ent
+    # whole epochs: placement by mori_rank_partition_tiers, bytes by the three pair-contexts
+    r.pool.zero_()
+    pool_ids = [cfg.gpu_pool_pages, mid_ids, cfg.cpu_pool_pages]
+    caps = [cfg.cap_gpu_pages, mid_ids - cfg.max_program_pages // 2, cfg.cap_cpu_pages]
+    sim = W.SimTiers(cfg, SEED, pool_ids, caps)
+    moved = {}
+    t_move, epochs = 0.0, 0
+    for e in range(args.warmup + args.steps):
+        plan = sim.begin_epoch()
+        got = r.place(plan.iota, plan.kv_pages, plan.prev_tier, caps)
+        sim.apply_placement(got["tier"], got["moves"])
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r.execute(plan)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        sim.end_epoch()
+        r.fill(plan.fills)
+        if e >= args.warmup:
+            t_move += dt; epochs += 1
+            for op in plan.ops:
+                if op[0] == "move":
+                    k = f"{op[2]}->{op[3]}"
+                    moved[k] = moved.get(k, 0) + len(op[4]) * sh.page_bytes
+    tot = sum(moved.values())
+    r.close()
+    binding.Mori.mori_host_free(arena)
+    print(json.dumps({"leg": "three_tier", "workload": cfg.name, "tiers": "0 = GPU pool, 1 = middle arena (device memory of the "
+                      "SAME GPU: stands in for peer HBM; NVLink bandwidth unmeasured, one GPU), 2 = pinned host arena",
+                      "pools_GiB": [x * sh.page_bytes / GIB for x in pool_ids], "pairs": pairs,
+                      "epochs": {"timed": epochs, "moved_GiB_by_pair": {k: v / GIB for k, v in sorted(moved.items())},
+                                 "GBps_all_pairs_host_timed": tot / t_move / 1e9 if t_move > 0 else 0.0,
+                                 "note": "host wall-clock around TierRunner.execute (three contexts, joins included)"}}))
+
+
 def launch_floor(m, cur, reps=200):
     """The floor the latency-bound entry points are judged against: an EMPTY kernel (mori_noop)
     launched through the same binding on the same stream -- device microseconds per call over `reps`
@@ -1166,7 +1244,7 @@ def main():
     ap.add_argument("--verbose", action="store_true", help="per-step lines on stderr")
     ap.add_argument("--timeline", default=None, metavar="FILE",
                     help="write the per-stream event timeline of every timed step of the headline config to FILE (JSON)")
-    ap.add_argument("--leg", default=None, choices=["copy_sweep"],
+    ap.add_argument("--leg", default=None, choices=["copy_sweep", "three_tier"],
                     help="run one auxiliary measurement leg instead of the bench line (copy_sweep: the gather/scatter "
                          "kernel alone and in-step for several ring geometries; profiles/ cites it)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -1175,6 +1253,8 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.leg == "copy_sweep":
         copy_kernel_sweep(args)
+    elif args.leg == "three_tier":
+        three_tier_leg(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

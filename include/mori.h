@@ -65,10 +65,13 @@ enum { MORI_LIST_DEMOTE = 0, MORI_LIST_PROMOTE = 1, MORI_LIST_DROP = 2, MORI_LIS
  *              cudaMemcpyAsync DMAs staging -> arena on a copy stream, double-buffered
  *              (promote: DMA arena -> staging, then scatter kernel staging -> pool).
  *   COPYENGINE no kernel: one strided cudaMemcpy2DAsync per logical page (baseline).
- *   AUTO       chosen per call from the slot table: STAGED when the runs of
- *              consecutive host slots average >= 6 MiB (large DMAs reach 97-100 % of the measured
- *              link peak), ZEROCOPY otherwise (a DMA per 2 MiB run reaches 89 %, SM-driven
- *              zero-copy 92 % whatever the fragmentation).  mori_path() reports STAGED. */
+ *   AUTO       chosen per call from the slot table: a call of at most 448
+ *              pages and 4 MiB is ONE launch of a kernel that carries the page and slot ids in its
+ *              parameters and copies straight between the pool and the mapped arena (no index
+ *              upload, no staging, no DMA); otherwise STAGED when the runs of consecutive host slots
+ *              average >= 6 MiB (large DMAs reach 97-100 % of the measured link peak), ZEROCOPY
+ *              below that (a DMA per 2 MiB run reaches 89 %, SM-driven zero-copy 92 % whatever the
+ *              fragmentation).  mori_path() reports STAGED. */
 enum { MORI_PATH_AUTO = 0, MORI_PATH_ZEROCOPY = 1, MORI_PATH_STAGED = 2, MORI_PATH_COPYENGINE = 3 };
 /* Device copy kernel used by STAGED paths and by mori_gather_pages / mori_scatter_pages. */
 enum { MORI_KERNEL_AUTO = 0, MORI_KERNEL_LDST = 1, MORI_KERNEL_TMA = 2 };
