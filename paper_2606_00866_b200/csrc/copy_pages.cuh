@@ -169,13 +169,8 @@ constexpr int kTmaThreads = 64;   // warp 0 lane 0 = load issuer, warp 1 lane 0 
 template <bool kGather>
 __device__ __forceinline__ void chunk_addresses(const CopyArgs& a, long long w, const unsigned char*& src,
                                                 unsigned char*& dst) {
-#ifdef MORI_MAP_LAYER_SLOW
-  const int l = (int)(w / a.n_pages);
-  const long long k = w - (long long)l * a.n_pages;
-#else
   const long long k = w / a.n_layers;
   const int l = (int)(w - k * a.n_layers);
-#endif
   const long long g = a.gpu_pages[k];
   const long long e = a.lin_idx ? (long long)a.lin_idx[k] : k;
   unsigned char* pp = a.pool + ((long long)l * a.pool_pages + g) * a.chunk_bytes;
