@@ -233,3 +233,73 @@ def test_plan_calls_keeps_order_bytes_and_dependencies():
                 assert all(firsts[i] + len(ops[i][3]) == firsts[i + 1] for i in range(len(ops) - 1))
         sim.end_epoch()
     assert seen_dep > 0 and seen_split > 0, "the trace never produced a dependent promotion"
+
+
+def test_two_tier_planner_never_aliases_pages_without_a_ticket():
+    """What the movers rely on: within an epoch, a promotion lands either in pages nothing is
+    reading (free before the epoch's moves began, or freed before the last join) or in pages freed
+    by exactly the demotion it names as its dependency; a demotion writes slots nothing reads."""
+    import oracle
+    for idx, scale, fb in ((3, 32, 0.5), (2, 64, None), (5, 64, None)):
+        cfg = W.get_config(idx, scale, fb)
+        sim = W.Sim(cfg, 867)
+        for e in range(60):
+            plan = sim.begin_epoch()
+            res = oracle.rank_partition(plan.iota, plan.kv_pages, plan.prev_tier, cfg.cap_gpu_pages, cfg.cap_cpu_pages)
+            sim.apply_placement(res["tier"], res["lists"])
+            freed_by = {}                       # gpu page -> demote number that vacates it (since the last join)
+            slots_read = set()                  # host slots a promotion of this phase reads
+            slots_written = set()
+            for op in plan.ops:
+                if op[0] == "sync_all":
+                    freed_by.clear(); slots_read.clear(); slots_written.clear()
+                elif op[0] == "demote":
+                    for g in op[3]:
+                        assert int(g) not in freed_by
+                        freed_by[int(g)] = op[1]
+                    assert not (set(map(int, op[4])) & (slots_read | slots_written)), "a demotion writes a slot in use"
+                    slots_written.update(map(int, op[4]))
+                else:
+                    deps = {freed_by[int(g)] for g in op[4] if int(g) in freed_by}
+                    assert deps <= ({op[5]} if op[5] > 0 else set()), (e, deps, op[5])
+                    assert not (set(map(int, op[3])) & slots_written), "a promotion reads a slot written this phase"
+                    slots_read.update(map(int, op[3]))
+            sim.end_epoch()
+            # every program's pages / slots are its own
+            allg = np.concatenate([p for p in sim.gpu_pages if p.size] or [np.zeros(0, np.int32)])
+            allh = np.concatenate([p for p in sim.host_slots if p.size] or [np.zeros(0, np.int32)])
+            assert np.unique(allg).size == allg.size and np.unique(allh).size == allh.size
+            assert allg.size <= cfg.gpu_pool_pages and allh.size <= cfg.cpu_pool_pages
+
+
+def test_tier_planner_never_reuses_an_id_freed_in_the_same_phase():
+    """SimTiers promises the three pair-movers that no id freed by a move is handed out again before
+    the next join, and that every program's ids stay disjoint in every pool."""
+    import oracle
+    cfg = W.get_config(2, 64)
+    for mid_ids, slack in ((cfg.gpu_pool_pages // 2, cfg.max_program_pages // 2), (cfg.gpu_pool_pages // 3, 0)):
+        pool_ids = [cfg.gpu_pool_pages, mid_ids, cfg.cpu_pool_pages]
+        caps = [cfg.cap_gpu_pages, mid_ids - slack, cfg.cap_cpu_pages]
+        sim = W.SimTiers(cfg, 868, pool_ids, caps)
+        for e in range(50):
+            plan = sim.begin_epoch()
+            res = oracle.rank_partition_tiers(plan.iota, plan.kv_pages, caps, plan.prev_tier)
+            sim.apply_placement(res["tier"], res["moves"])
+            freed = [set(), set(), set()]
+            for op in plan.ops:
+                if op[0] == "sync_all":
+                    freed = [set(), set(), set()]
+                else:
+                    _, p, frm, to, src, dst = op
+                    assert frm != to and len(src) == len(dst)
+                    assert not (set(map(int, dst)) & freed[to]), (e, "id reused before a join")
+                    freed[frm].update(map(int, src))
+            sim.end_epoch()
+            for t, tri in enumerate(sim.resident()):
+                ids = np.concatenate([x[2] for x in tri]) if tri else np.zeros(0, np.int32)
+                assert np.unique(ids).size == ids.size and ids.size <= pool_ids[t]
+                assert ids.size == 0 or (ids.min() >= 0 and ids.max() < pool_ids[t])
+            # the label and the location agree for every program that holds bytes
+            for p in range(cfg.n_programs):
+                if sim.where[p] >= 0:
+                    assert sim.where[p] == sim.tier[p], (e, p)
