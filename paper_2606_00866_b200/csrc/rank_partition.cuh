@@ -96,69 +96,146 @@ __device__ __forceinline__ void block_excl_scan_n(uint64_t (&v)[N], uint64_t* wa
   }
 }
 
+// Per-program byte outputs (tier, lazy) are produced in RANK order but indexed by PROGRAM: as
+// scattered one-byte global stores they cost a memory transaction each (n = 4096: ~2 us from the one
+// SM that runs the tail).  They are staged in shared memory instead and written out coalesced.
+__device__ __forceinline__ void flush_bytes(const uint8_t* s, uint8_t* __restrict__ g, int n) {
+  __syncthreads();
+  for (int i = threadIdx.x; i < n; i += blockDim.x) g[i] = s[i];
+}
+
 // Ranking by counting, shared by every kernel that orders more keys than one CTA sorts well
 // (rank_partition_multi, rank_tiers, sticky_rebalance, bfd_assign).  Keys are unique, so
 // position(i) = #{j : key_j < key_i}.  Every CTA holds all n keys in its shared memory (built by
-// the caller, __syncthreads() done); this CTA ranks the items of its slice -- one warp per item,
-// lanes striding j, shuffle reduction -- and writes order[position] = item.  Returns true in
-// exactly one CTA, the LAST to finish (atomic ticket, reset for the next launch), after every
-// CTA's order[] writes are visible to it (read them with __ldcg): that CTA carries on with the
-// part of the algorithm that needs the whole order.  `less(j, i)` says key_j < key_i.
+// the caller, __syncthreads() done); this CTA ranks the items of its slice -- one warp per K items,
+// lanes striding j, shuffle reduction -- and writes order[position] = item (rank_by_counting64 /
+// rank_by_counting128 below).  They return true in exactly one CTA, the LAST to finish (atomic
+// ticket, reset for the next launch), after every CTA's order[] writes are visible to it (read them
+// with __ldcg): that CTA carries on with the part of the algorithm that needs the whole order.
 // The tail of every rank-by-counting kernel: true in exactly one CTA, the LAST to finish.
 __device__ __forceinline__ bool last_cta_ticket(unsigned int* __restrict__ ticket) {
   __shared__ unsigned int s_ticket;
-  __threadfence();                                   // this CTA's order[] writes are visible ...
-  __syncthreads();
-  if (threadIdx.x == 0) s_ticket = atomicAdd(ticket, 1u);    // ... before its ticket is
-  __syncthreads();
-  if (s_ticket != gridDim.x - 1) return false;
-  if (threadIdx.x == 0) *ticket = 0;                 // ready for the next launch that uses this counter
-  __threadfence();
-  return true;
-}
-
-template <class Less>
-__device__ __forceinline__ bool rank_by_counting(int n, Less less, int32_t* __restrict__ order,
-                                                 unsigned int* __restrict__ ticket) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
-  const int per = (n + gridDim.x - 1) / gridDim.x;
-  const int lo = blockIdx.x * per, hi = min(n, lo + per);
-  for (int i = lo + warp; i < hi; i += n_warps) {
-    int c = 0;
-    for (int j = lane; j < n; j += 32) c += less(j, i) ? 1 : 0;
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
-    if (lane == 0) order[c] = i;
+  __syncthreads();                                   // the CTA's order[] writes are ordered before thread 0 ...
+  if (threadIdx.x == 0) {
+    __threadfence();                                 // ... whose ONE fence (fences are cumulative) makes them
+    s_ticket = atomicAdd(ticket, 1u);                // visible device-wide before the ticket is taken
+    if (s_ticket == gridDim.x - 1) {
+      *ticket = 0;                                   // ready for the next launch that uses this counter
+      __threadfence();                               // every other CTA's writes are visible to this one now
+    }
   }
-  return last_cta_ticket(ticket);
+  __syncthreads();
+  return s_ticket == gridDim.x - 1;
 }
 
-// The same for unique 128-bit keys (sticky_rebalance, bfd_assign), where the counting loop is what
-// the launch costs: n^2 compares, bound by instruction issue.  Keys sit in shared memory as one
-// 16-byte word each (x = low half, y = high half) -- one LDS.128 per compare -- and the compare is
-// the borrow of a 128-bit subtraction (four carry-chained ISETPs), branch-free, four keys in flight.
-__device__ __forceinline__ int lt128(const ulonglong2& a, const ulonglong2& b) {
-  return (((unsigned __int128)a.y << 64) | a.x) < (((unsigned __int128)b.y << 64) | b.x) ? 1 : 0;
+// Unique 128-bit keys (sticky_rebalance, bfd_assign) sit in shared memory as one 16-byte word each
+// (x = low half, y = high half) -- one LDS.128 per key read -- and the compare is the borrow of a
+// 128-bit subtraction (four carry-chained ISETPs), branch-free.
+// acc -= (a < b): a < b <=> a - b borrows, so one carry chain over the 32-bit words and a final
+// subtract-with-borrow INTO the accumulator: five instructions per 128-bit compare-and-count (the
+// compiler's own 128-bit compare takes ten, and the counting loop is bound by instruction issue),
+// three per 64-bit one.  The count is -acc.
+__device__ __forceinline__ void count_lt128(int& acc, const ulonglong2& a, const ulonglong2& b) {
+  asm("{\n\t.reg .u32 t;\n\t"
+      "sub.cc.u32 t, %1, %5;\n\t"
+      "subc.cc.u32 t, %2, %6;\n\t"
+      "subc.cc.u32 t, %3, %7;\n\t"
+      "subc.cc.u32 t, %4, %8;\n\t"
+      "subc.u32 %0, %0, 0;\n\t}"
+      : "+r"(acc)
+      : "r"((unsigned int)a.x), "r"((unsigned int)(a.x >> 32)), "r"((unsigned int)a.y), "r"((unsigned int)(a.y >> 32)),
+        "r"((unsigned int)b.x), "r"((unsigned int)(b.x >> 32)), "r"((unsigned int)b.y), "r"((unsigned int)(b.y >> 32)));
+}
+__device__ __forceinline__ void count_lt64(int& acc, uint64_t a, uint64_t b) {
+  asm("{\n\t.reg .u32 t;\n\t"
+      "sub.cc.u32 t, %1, %3;\n\t"
+      "subc.cc.u32 t, %2, %4;\n\t"
+      "subc.u32 %0, %0, 0;\n\t}"
+      : "+r"(acc)
+      : "r"((unsigned int)a), "r"((unsigned int)(a >> 32)), "r"((unsigned int)b), "r"((unsigned int)(b >> 32)));
+}
+
+// K programs per warp pass: every key read from shared memory is compared against K keys held in
+// registers, so the loop's shared-memory traffic -- what bounds it: n^2 reads of 16 bytes per launch,
+// 268 MB at n = 4096 against ~36 TB/s over 148 SMs -- drops K-fold.
+template <int K>
+__device__ __forceinline__ void count_positions128(int n, const ulonglong2* __restrict__ keys,
+                                                   int32_t* __restrict__ order, int lo, int hi) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  for (int i0 = lo + warp * K; i0 < hi; i0 += n_warps * K) {
+    ulonglong2 ki[K];
+    int c[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) { ki[k] = keys[min(i0 + k, n - 1)]; c[k] = 0; }
+    int j = lane;
+    for (; j + 32 < n; j += 64) {
+      const ulonglong2 k0 = keys[j], k1 = keys[j + 32];
+#pragma unroll
+      for (int k = 0; k < K; ++k) { count_lt128(c[k], k0, ki[k]); count_lt128(c[k], k1, ki[k]); }
+    }
+    for (; j < n; j += 32) {
+      const ulonglong2 k0 = keys[j];
+#pragma unroll
+      for (int k = 0; k < K; ++k) count_lt128(c[k], k0, ki[k]);
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      int v = -c[k];
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, d);
+      if (lane == 0 && i0 + k < hi) order[v] = i0 + k;
+    }
+  }
 }
 __device__ __forceinline__ bool rank_by_counting128(int n, const ulonglong2* __restrict__ keys,
                                                     int32_t* __restrict__ order, unsigned int* __restrict__ ticket) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
   const int per = (n + gridDim.x - 1) / gridDim.x;
   const int lo = blockIdx.x * per, hi = min(n, lo + per);
-  for (int i = lo + warp; i < hi; i += n_warps) {
-    const ulonglong2 ki = keys[i];
-    int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
+  if (per >= 48) count_positions128<4>(n, keys, order, lo, hi);
+  else if (per >= 16) count_positions128<2>(n, keys, order, lo, hi);
+  else count_positions128<1>(n, keys, order, lo, hi);
+  return last_cta_ticket(ticket);
+}
+
+// The same for unique 64-bit keys (rank_partition_multi, rank_tiers).
+template <int K>
+__device__ __forceinline__ void count_positions64(int n, const uint64_t* __restrict__ keys,
+                                                  int32_t* __restrict__ order, int lo, int hi) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  for (int i0 = lo + warp * K; i0 < hi; i0 += n_warps * K) {
+    uint64_t ki[K];
+    int c[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) { ki[k] = keys[min(i0 + k, n - 1)]; c[k] = 0; }
     int j = lane;
     for (; j + 96 < n; j += 128) {
-      const ulonglong2 k0 = keys[j], k1 = keys[j + 32], k2 = keys[j + 64], k3 = keys[j + 96];
-      c0 += lt128(k0, ki); c1 += lt128(k1, ki); c2 += lt128(k2, ki); c3 += lt128(k3, ki);
-    }
-    for (; j < n; j += 32) c0 += lt128(keys[j], ki);
-    int c = (c0 + c1) + (c2 + c3);
+      const uint64_t k0 = keys[j], k1 = keys[j + 32], k2 = keys[j + 64], k3 = keys[j + 96];
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
-    if (lane == 0) order[c] = i;
+      for (int k = 0; k < K; ++k) {
+        count_lt64(c[k], k0, ki[k]); count_lt64(c[k], k1, ki[k]); count_lt64(c[k], k2, ki[k]); count_lt64(c[k], k3, ki[k]);
+      }
+    }
+    for (; j < n; j += 32) {
+      const uint64_t k0 = keys[j];
+#pragma unroll
+      for (int k = 0; k < K; ++k) count_lt64(c[k], k0, ki[k]);
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      int v = -c[k];
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, d);
+      if (lane == 0 && i0 + k < hi) order[v] = i0 + k;
+    }
   }
+}
+__device__ __forceinline__ bool rank_by_counting64(int n, const uint64_t* __restrict__ keys,
+                                                   int32_t* __restrict__ order, unsigned int* __restrict__ ticket) {
+  const int per = (n + gridDim.x - 1) / gridDim.x;
+  const int lo = blockIdx.x * per, hi = min(n, lo + per);
+  if (per >= 48) count_positions64<4>(n, keys, order, lo, hi);
+  else if (per >= 16) count_positions64<2>(n, keys, order, lo, hi);
+  else count_positions64<1>(n, keys, order, lo, hi);
   return last_cta_ticket(ticket);
 }
 
@@ -170,7 +247,7 @@ __device__ __forceinline__ void partition_tail(
     const uint8_t* __restrict__ prev_tier, long long cap_gpu, long long cap_cpu,
     int32_t* __restrict__ order, uint8_t* __restrict__ tier, int32_t* __restrict__ bounds,
     long long* __restrict__ used, int32_t* __restrict__ lists, int32_t* __restrict__ list_counts,
-    uint64_t* warp_tot, long long* bcast) {
+    uint64_t* warp_tot, long long* bcast, uint8_t* s_tier /* n bytes of (dead) shared memory */) {
   const int tid = threadIdx.x;
   // ---- a2: footprints in rank order + exclusive prefix sum (int64) ----------------------------
   long long sz[IPT];
@@ -236,7 +313,7 @@ __device__ __forceinline__ void partition_tail(
     cls[i] = -1;
     if (r < n) {
       const int now = r < b_gpu ? 0 : (r < b_cpu ? 1 : 2);
-      tier[prog[i]] = (uint8_t)now;
+      s_tier[prog[i]] = (uint8_t)now;
       order[r] = prog[i];
       if (prev_tier != nullptr) {
         const int pv = prev_tier[prog[i]];
@@ -251,6 +328,7 @@ __device__ __forceinline__ void partition_tail(
       }
     }
   }
+  flush_bytes(s_tier, tier, n);
   if (prev_tier == nullptr) return;
 
   // ---- a4: compaction by rank.  Ascending lists take the exclusive count below; descending
@@ -336,7 +414,7 @@ rank_partition_kernel(int n, int n_pad, const float* __restrict__ idleness,
     prog[i] = r < n ? (int)(uint32_t)keys[r] : -1;
   }
   partition_tail<IPT>(n, prog, kv_pages, prev_tier, cap_gpu, cap_cpu, order, tier, bounds, used, lists,
-                      list_counts, warp_tot, bcast);
+                      list_counts, warp_tot, bcast, reinterpret_cast<uint8_t*>(keys));   // the keys are dead
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -366,7 +444,7 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
   __syncthreads();
   // the CTAs exchange the order through library-owned DEVICE scratch; the caller's arrays are
   // written once, by the last CTA -- so they may be mapped host memory
-  if (!rank_by_counting(n, [&](int j, int i) { return keys[j] < keys[i]; }, scratch_order, ticket)) return;
+  if (!rank_by_counting64(n, keys, scratch_order, ticket)) return;
 
   int prog[IPT];
 #pragma unroll
@@ -375,7 +453,7 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
     prog[i] = r < n ? __ldcg(scratch_order + r) : -1;   // written by other CTAs: read through L2
   }
   partition_tail<IPT>(n, prog, kv_pages, prev_tier, cap_gpu, cap_cpu, order, tier, bounds, used, lists,
-                      list_counts, warp_tot, bcast);
+                      list_counts, warp_tot, bcast, reinterpret_cast<uint8_t*>(keys));   // the keys are dead
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -401,7 +479,7 @@ rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __re
   for (int i = tid; i < n; i += blockDim.x)
     keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;
   __syncthreads();
-  if (!rank_by_counting(n, [&](int j, int i) { return keys[j] < keys[i]; }, scratch_order, ticket)) return;
+  if (!rank_by_counting64(n, keys, scratch_order, ticket)) return;
 
   int prog[IPT];
   long long incl[IPT];
@@ -449,8 +527,10 @@ rank_tiers_kernel(int n, const float* __restrict__ idleness, const int32_t* __re
     b_prev = b;
     __syncthreads();                                                 // bcast is rewritten next round
   }
+  uint8_t* s_tier = reinterpret_cast<uint8_t*>(keys);                // the keys are dead (barriers above)
 #pragma unroll
-  for (int i = 0; i < IPT; ++i) if (prog[i] >= 0) tier[prog[i]] = (uint8_t)my_tier[i];
+  for (int i = 0; i < IPT; ++i) if (prog[i] >= 0) s_tier[prog[i]] = (uint8_t)my_tier[i];
+  flush_bytes(s_tier, tier, n);
   if (prev_tier == nullptr) return;
 
   // move lists (the two-tier rule of P:L206 / L208 carried over): DOWN the hierarchy most idle

@@ -76,6 +76,8 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
   // ---- this thread's positions ------------------------------------------------------------------
   int32_t* vsize = reinterpret_cast<int32_t*>(keys);                 // [n] victims' sizes, by position
   uint8_t* vdest = reinterpret_cast<uint8_t*>(vsize + n);            // [n] 1 = CPU queue, 2 = Waiting
+  uint8_t* s_tier = vdest + n;                                       // [n] per-PROGRAM outputs, staged (flush_bytes)
+  uint8_t* s_lazy = s_tier + n;                                      // [n]
   int prog[IPT], grp[IPT], was[IPT], fl[IPT];
   long long sz[IPT];
   long long sum_g = 0, sum_c = 0;
@@ -202,14 +204,16 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
     int now = was[i], row = -1;
     if (victim[i]) { now = vdest[tid * IPT + i]; row = now == 1 ? 0 : 2; }
     else if (promoted[i]) { now = 0; row = was[i] == 1 ? 1 : 3; }
-    tier[prog[i]] = (uint8_t)now;
-    lazy[prog[i]] = (uint8_t)(victim[i] && !(fl[i] & kFlagActing));
+    s_tier[prog[i]] = (uint8_t)now;
+    s_lazy[prog[i]] = (uint8_t)(victim[i] && !(fl[i] & kFlagActing));
     if (row >= 0) {
       const int pos = (int)((pex >> (16 * row)) & 0xFFFF);
       pex += 1ull << (16 * row);
       lists[(size_t)row * n + pos] = prog[i];
     }
   }
+  flush_bytes(s_tier, tier, n);
+  flush_bytes(s_lazy, lazy, n);
   if (tid < 4) list_counts[tid] = (int)((ptot >> (16 * tid)) & 0xFFFF);
   if (tid == 4) list_counts[4] = 0;
   if (tid == 0) {
