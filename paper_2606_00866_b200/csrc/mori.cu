@@ -512,6 +512,19 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
     CKC(cudaGetLastError());
     CKC(cudaDeviceSynchronize());
   }
+  auto warm_streams = [&]() -> cudaError_t {      // first use of a stream / an event costs microseconds too
+    mori::CopyArgs z{};
+    z.n_layers = 1; z.chunk_bytes = 16; z.piece_bytes = 16; z.pieces_per_chunk = 1; z.stages = 2; z.store_lag = 1;
+    for (int i = 0; i < 2; ++i) {
+      Direction& d = c->dir[i];
+      if (!d.kern) continue;
+      mori::copy_pages_small<true, mori::kSmallFewPages><<<1, mori::kLdstThreads, 0, d.kern>>>(z, mori::SmallIds<mori::kSmallFewPages>{});
+      cudaEventRecord(d.tickets[0], d.kern);
+      cudaStreamWaitEvent(d.copy, d.tickets[0], 0);
+    }
+    cudaError_t e = cudaGetLastError();
+    return e != cudaSuccess ? e : cudaDeviceSynchronize();
+  };
   // The attribute is per function and PROCESS-wide: every context sets it to the device's opt-in
   // maximum, so contexts with different ring sizes never lower it under one another.
   CKC(cudaFuncSetAttribute(mori::copy_pages_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
@@ -593,6 +606,7 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
       }
     }
   }
+  CKC(warm_streams());
 #undef CKC
   return MORI_OK;
 }
