@@ -41,7 +41,7 @@ constexpr int kPieceBytesDefault = 64 * 1024;   // bytes per bulk copy = stage s
 constexpr int kRingBytesDefault = 192 * 1024;   // shared memory the rings of one SM's CTAs may take
 constexpr int kMaxTmaStages = 24;
 constexpr long long kAutoMinRunBytes = 6LL << 20;   // AUTO: below this mean slot-run length, ZEROCOPY
-constexpr long long kRampBytes = 256LL << 20;        // STAGED: size of a call's first (demote) / last (promote) segment
+constexpr long long kRampBytes = 512LL << 20;        // STAGED: size of a call's first (demote) / last (promote) segment
 constexpr long long kSmallMaxBytes = 4LL << 20;     // calls up to this size (and kSmallMaxPages) take the one-launch path
 
 // Tuning overrides for experiments (read once per mori_create): MORI_PIECE_KIB, MORI_RING_KIB,
@@ -1048,13 +1048,19 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
     if (int rc = stage_indices(c, d, total, gpu_pages, host_slots, &dg, &dh)) return rc;
   if (total > 0) d.copy_busy = true;
   // The pipeline's ramp: a demotion's first DMA waits for its first gather and a promotion's last
-  // scatter runs after its last DMA, so those two segments are short (<= 256 MiB: ~0.1 ms of kernel
-  // instead of ~0.7 ms for a 2 GiB segment); every other kernel hides under a DMA.
+  // scatter runs after its last DMA, so those two segments are short (<= 512 MiB: ~0.17 ms of kernel
+  // instead of ~0.65 ms for a 2 GiB segment); every other kernel hides under a DMA.
+  // The rest of the call is cut into EQUAL segments (6.1 GiB = ramp + 3 x 1.95 GiB, not ramp + 2 + 2 +
+  // 1.85 + a 0.1 GiB tail whose launch would be all ramp and tail).
   const long long ramp_pages = std::max<long long>(1, std::min<long long>(seg_pages, kRampBytes / pb));
-  for (long long a0 = 0, cnt = 0; a0 < total; a0 += cnt) {
-    cnt = std::min(seg_pages, total - a0);
-    if (demote && a0 == 0 && total > 2 * ramp_pages) cnt = std::min(cnt, ramp_pages);
-    if (!demote && total - a0 == cnt && cnt > 2 * ramp_pages) cnt -= ramp_pages;
+  const long long ramp = total > 2 * ramp_pages ? ramp_pages : 0;
+  const long long body = total - ramp;
+  const long long n_body = (body + seg_pages - 1) / seg_pages;              // segments of the body
+  long long seg_i = 0;
+  for (long long a0 = 0, cnt = 0; a0 < total; a0 += cnt, ++seg_i) {
+    const long long bi = demote ? seg_i - (ramp ? 1 : 0) : seg_i;           // index within the body, or outside it
+    if (bi < 0 || bi >= n_body) cnt = ramp;                                 // the ramp: first (demote) / last (promote)
+    else cnt = body / n_body + (bi < body % n_body ? 1 : 0);
     const int b = d.buf; d.buf ^= 1;
     unsigned char* stg = d.staging[b];
     mori::CopyArgs a = make_args(c, stg, dg + a0, nullptr, cnt);
