@@ -55,7 +55,6 @@ class GpuRunner:
         self.out_mapped = n <= 1024
         self.d_out = self.h_out if self.out_mapped else torch.zeros(self._o_tier + n, dtype=torch.uint8, device=d)
         self._h_out_np = self.h_out.numpy()
-        self._h_in_np = None
         self.h_in = torch.zeros(9 * n, dtype=torch.uint8, pin_memory=True)    # iota | kv | prev
         self.d_in = torch.zeros(9 * n, dtype=torch.uint8, device=d)
         self._wl = None

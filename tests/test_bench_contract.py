@@ -66,3 +66,18 @@ def test_link_bounds():
         assert bench.memcpy_model_seconds(d * G, p * G, link) >= bench.ideal_seconds(d * G, p * G, link) * (1 - 1e-12)
     d = 57.2 / (57.2 + 55.6) * 10 * G; p = 55.6 / (57.2 + 55.6) * 10 * G
     assert np.isclose(bench.memcpy_model_seconds(d, p, link), 10 * G / 99.8e9)
+
+
+def test_roofline_traffic_comes_from_a_tracked_ncu_summary():
+    """bench.py prints `roofline.traffic` from profiles/ncu_traffic.json (no constant in the code): the
+    file must name its source capture and launch, and its ratio must be read + write over 2 x bytes."""
+    sys.path.insert(0, ROOT)
+    import bench
+    t = bench._load_ncu_traffic()
+    for k in ("dram_bytes_per_launch", "dram_bytes_read", "dram_bytes_write", "algorithmic_bytes_same_launch",
+              "ratio", "launch", "source", "kernel"):
+        assert k in t, k
+    assert np.isclose(t["dram_bytes_per_launch"], t["dram_bytes_read"] + t["dram_bytes_write"])
+    assert np.isclose(t["ratio"], t["dram_bytes_per_launch"] / t["algorithmic_bytes_same_launch"], atol=5e-4)
+    assert 0.9 < t["ratio"] < 1.1
+    assert os.path.exists(os.path.join(ROOT, t["source"].split(" ")[0]))
