@@ -736,13 +736,18 @@ def run_ours(args):
         t0 = time.perf_counter()
         try:
             c2 = W.get_config(idx, sc, fb)
-            m2 = measure_config(args, c2, seed, arena_full[:c2.cpu_pool_pages * c2.shape.page_bytes], link,
+            # the box is one GPU of a shared host and its pinned-memcpy rate drifts within a run: every leg
+            # is held against peaks measured right before it (both sets are printed)
+            link2 = measure_link_peak(arena_full, reps=3)
+            m2 = measure_config(args, c2, seed, arena_full[:c2.cpu_pool_pages * c2.shape.page_bytes], link2,
                                 args.per_config_steps if idx != 1 else c2.epochs - 4, 4, local, barrier,
                                 do_e2e=(idx == 1), gather_reps=0 if (args.no_gather_leg or idx == 1) else 5,
                                 clocks_on=False)
             m2["runner"].close()
             m2["runner"] = None
-            rec = _per_config_record(m2, link, sc)
+            rec = _per_config_record(m2, link2, sc)
+            rec["link_peaks_GBps_before_leg"] = {k: link2[k] for k in ("d2h", "h2d", "bidir_sum")}
+            rec["frac_of_link_peak_measured_at_start"] = link_report(m2["steps"], link)["frac_of_measured_link_peak"]
             rec["leg_seconds"] = time.perf_counter() - t0
             per_config.append(rec)
             del m2
