@@ -84,9 +84,14 @@ typedef struct {
   int64_t gpu_pool_pages;
   void*   host_arena;        /* PINNED, caller-owned, 16-byte aligned; may be NULL if neither
                                 mori_demote nor mori_promote is used.  May instead be DEVICE
-                                memory (this GPU's, or a peer GPU's with peer access enabled:
-                                the intermediate tier of P:L347): both directions then run as
-                                one full-grid kernel, path_* are ignored */
+                                memory (this GPU's, or a peer GPU's -- mori_create turns peer
+                                access on, or fails with MORI_ERR_UNSUPPORTED if the two GPUs are
+                                not peers: the intermediate tier of P:L347): both directions then
+                                run as one full-grid kernel, path_* are ignored.  A DEVICE arena
+                                described as a pool of ONE layer (n_layers = 1, n_kv_heads = L * H:
+                                a slot is then one chunk) can in turn be the gpu_pool of a second
+                                context whose host_arena is pinned memory: the arena <-> arena
+                                mover of a three-tier hierarchy */
   int64_t host_arena_slots;
   int32_t max_programs;      /* 1 .. MORI_MAX_PROGRAMS */
   int32_t path_demote;       /* MORI_PATH_* */

@@ -576,6 +576,19 @@ int mori_create(const mori_config* cfg, mori_ctx** out) {
     // for, and both directions are the one-kernel path at full grid.
     cudaPointerAttributes at{};
     if (cudaPointerGetAttributes(&at, cfg->host_arena) == cudaSuccess && at.type == cudaMemoryTypeDevice) {
+      if (at.device != dev) {
+        // a peer GPU's HBM: this GPU's SMs reach it over NVLink once peer access is on
+        int can = 0;
+        CKC(cudaDeviceCanAccessPeer(&can, dev, at.device));
+        if (!can) {
+          g_create_error = "host_arena is memory of GPU " + std::to_string(at.device) + ", which GPU " +
+                           std::to_string(dev) + " cannot access as a peer";
+          mori_destroy(c); *out = nullptr; return MORI_ERR_UNSUPPORTED;
+        }
+        const cudaError_t pe = cudaDeviceEnablePeerAccess(at.device, 0);
+        if (pe != cudaSuccess && pe != cudaErrorPeerAccessAlreadyEnabled) CKC(pe);
+        cudaGetLastError();
+      }
       c->arena_is_device = true;
       c->arena_dev = static_cast<unsigned char*>(cfg->host_arena);
       for (int i = 0; i < 2; ++i) { c->dir[i].path = MORI_PATH_ZEROCOPY; c->dir[i].auto_path = false; }
