@@ -678,7 +678,7 @@ int mori_rank_partition(mori_ctx* c, void* stream, int32_t n, const float* idlen
   if (n > mori::kRankMaxThreads) {
     // more than one CTA's worth: rank by counting on every SM, last CTA partitions
     const int grid = std::min(c->sm_count, (n + 7) / 8);
-    const size_t smem_m = sizeof(uint64_t) * ((size_t)n + 66) + 2 * sizeof(long long);
+    const size_t smem_m = sizeof(uint64_t) * ((size_t)n + 66) + 2 * sizeof(long long) + 5 * (size_t)n;   // keys, scan scratch, staged sizes and tiers
     const unsigned long long slot_m = c->rank_seq++ % kRankTickets;
     unsigned int* tk = c->rank_tickets + slot_m;
     int32_t* so = c->sticky_order + slot_m * (size_t)c->cfg.max_programs;
@@ -719,7 +719,7 @@ int mori_sticky_rebalance(mori_ctx* c, void* stream, int32_t n, const float* idl
   int n_pad = 1024;
   while (n_pad < n) n_pad <<= 1;
   const int grid = std::max(1, std::min(c->sm_count, (n + 7) / 8));
-  const size_t smem = sizeof(uint64_t) * (2 * (size_t)n + 99) + 4 * sizeof(long long);
+  const size_t smem = sizeof(uint64_t) * (2 * (size_t)n + 99) + 4 * sizeof(long long) + 6 * (size_t)n;   // keys, scan scratch, staged inputs
   const unsigned long long slot = c->rank_seq++ % kRankTickets;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   long long* u = reinterpret_cast<long long*>(used);

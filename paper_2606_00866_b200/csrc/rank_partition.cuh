@@ -438,9 +438,16 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
   uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);            // [n]
   uint64_t* warp_tot = keys + n;                                     // [2][33]
   long long* bcast = reinterpret_cast<long long*>(warp_tot + 66);    // [2]
+  // sizes and previous tiers, kept for the last CTA's tail: there they are read in RANK order, which
+  // from global memory is a scattered gather (one transaction per program) and from here is free
+  int32_t* s_kv = reinterpret_cast<int32_t*>(bcast + 2);             // [n]
+  uint8_t* s_prev = reinterpret_cast<uint8_t*>(s_kv + n);            // [n]
   const int tid = threadIdx.x;
-  for (int i = tid; i < n; i += blockDim.x)
+  for (int i = tid; i < n; i += blockDim.x) {
     keys[i] = ((uint64_t)idleness_key(idleness[i]) << 32) | (uint32_t)i;
+    s_kv[i] = kv_pages[i];
+    if (prev_tier != nullptr) s_prev[i] = prev_tier[i];
+  }
   __syncthreads();
   // the CTAs exchange the order through library-owned DEVICE scratch; the caller's arrays are
   // written once, by the last CTA -- so they may be mapped host memory
@@ -452,8 +459,8 @@ rank_partition_multi_kernel(int n, const float* __restrict__ idleness,
     const int r = tid * IPT + i;
     prog[i] = r < n ? __ldcg(scratch_order + r) : -1;   // written by other CTAs: read through L2
   }
-  partition_tail<IPT>(n, prog, kv_pages, prev_tier, cap_gpu, cap_cpu, order, tier, bounds, used, lists,
-                      list_counts, warp_tot, bcast, reinterpret_cast<uint8_t*>(keys));   // the keys are dead
+  partition_tail<IPT>(n, prog, s_kv, prev_tier != nullptr ? s_prev : nullptr, cap_gpu, cap_cpu, order, tier, bounds,
+                      used, lists, list_counts, warp_tot, bcast, reinterpret_cast<uint8_t*>(keys));   // the keys are dead
 }
 
 // ---------------------------------------------------------------------------------------------

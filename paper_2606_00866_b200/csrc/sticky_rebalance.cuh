@@ -61,12 +61,18 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
   ulonglong2* keys = reinterpret_cast<ulonglong2*>(smem_raw);        // [n] (x = low half, y = high half)
   uint64_t* warp_tot = reinterpret_cast<uint64_t*>(keys + n);        // [3][33]
   long long* bcast = reinterpret_cast<long long*>(warp_tot + 99);    // [4]
+  // the per-program inputs, kept for the last CTA's tail: there they are read in RANK order, which
+  // from global memory is a scattered gather (one transaction per program) and from here is free
+  int32_t* s_kv = reinterpret_cast<int32_t*>(bcast + 4);             // [n]
+  uint8_t* s_prev = reinterpret_cast<uint8_t*>(s_kv + n);            // [n]
+  uint8_t* s_fl = s_prev + n;                                        // [n]
   const int tid = threadIdx.x;
 
   for (int p = tid; p < n; p += blockDim.x) {
-    const int pv = prev_tier[p];
+    const int pv = prev_tier[p], kvp = kv_pages[p], flg = flags[p];
+    s_kv[p] = kvp; s_prev[p] = (uint8_t)pv; s_fl[p] = (uint8_t)flg;
     unsigned long long hi64, lo64;
-    sticky_key(p, idleness[p], kv_pages[p], pv == 0 ? 0 : (pv == 1 ? 1 : 2), flags[p], hi64, lo64);
+    sticky_key(p, idleness[p], kvp, pv == 0 ? 0 : (pv == 1 ? 1 : 2), flg, hi64, lo64);
     keys[p] = make_ulonglong2(lo64, hi64);
   }
   __syncthreads();
@@ -87,12 +93,12 @@ sticky_rebalance_kernel(int n, const float* __restrict__ idleness, const int32_t
     prog[i] = -1; grp[i] = 7; was[i] = 2; fl[i] = 0; sz[i] = 0;
     if (r < n) {
       const int p = __ldcg(order + r);
-      const int pv = prev_tier[p];
+      const int pv = s_prev[p];
       prog[i] = p;
       was[i] = pv == 0 ? 0 : (pv == 1 ? 1 : 2);
-      fl[i] = flags[p];
+      fl[i] = s_fl[p];
       grp[i] = sticky_group(was[i], fl[i]);
-      const int s = kv_pages[p];
+      const int s = s_kv[p];
       sz[i] = s > 0 ? s : 0;
       if (was[i] == 0) sum_g += sz[i];
       if (was[i] == 1) sum_c += sz[i];
