@@ -300,6 +300,30 @@ int mori_eviction_order(mori_ctx* ctx, void* stream, int32_t which_tier, int64_t
                         const uint32_t* last_access, int32_t* victims, int32_t* n_resident);
 
 /*
+ * The same order for callers that cannot allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no context, and no cudaMalloc / cudaFree / allocating
+ * library routine on any call -- mori_eviction_order allocates its sort scratch on first use, this
+ * entry point keeps it in a file-scope static __device__ array instead (2 x MORI_NOALLOC_MAX_PAGES
+ * x 8 bytes = 1 MiB, held by every GPU that loads the library until the process exits).
+ *
+ *   Runs on the CURRENT device, one launch (the cluster kernel of mori_eviction_order) on `stream`;
+ *   arguments, order and outputs exactly as mori_eviction_order (which_tier: MORI_TIER_GPU / _CPU).
+ *   n_pages      0 .. MORI_NOALLOC_MAX_PAGES; more -> MORI_ERR_CAPACITY, nothing enqueued
+ *   why          NULL, or receives a pointer to a static string that says what was wrong (valid for
+ *                ever; "" on success)
+ * The first call on a device looks the scratch up (cudaGetSymbolAddress) and picks the cluster
+ * size: make it outside graph capture (n_pages = 0 does only that).  Every call on a device shares
+ * the one scratch array, which keeps the previous call's contents: nothing in it needs to start at
+ * zero (each pass overwrites every entry it later reads), but two calls that OVERLAP on the GPU --
+ * different streams, no ordering between them -- race on it.  Calls on one stream are safe.
+ */
+#define MORI_NOALLOC_MAX_PAGES 65536 /* cfg 2's arena, the largest BASELINE.json pool */
+int mori_eviction_order_noalloc(void* stream, int32_t which_tier, int64_t n_pages,
+                                const int32_t* page_owner, int32_t n_programs,
+                                const uint8_t* program_tier, const uint32_t* last_access,
+                                int32_t* victims, int32_t* n_resident, const char** why);
+
+/*
  * NEXT-4(i): which replica admits each Waiting-queue promotion: "Waiting-
  * queue promotions use Best-Fit-Decreasing bin packing across replicas, selecting the replica
  * with the most available capacity first" (CPU-queue promotions keep their replica and are not

@@ -32,7 +32,7 @@ EXPORTS = ["mori_create", "mori_destroy", "mori_rank_partition", "mori_demote", 
            "mori_copy_kernel", "mori_last_error", "mori_launch_count", "mori_host_alloc",
            "mori_host_free", "mori_sticky_rebalance", "mori_idleness_update",
            "mori_idleness_eval", "mori_eviction_order", "mori_bfd_assign",
-           "mori_rank_partition_tiers", "mori_profile_timeline", "mori_noop"]
+           "mori_rank_partition_tiers", "mori_profile_timeline", "mori_noop", "mori_eviction_order_noalloc"]
 
 
 class MoriConfig(C.Structure):
@@ -84,6 +84,7 @@ def load():
         L.mori_profile_read.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64), C.POINTER(i64)]
         L.mori_profile_timeline.argtypes = [vp, i32, i64, vp, vp, vp, vp, C.POINTER(i64)]
         L.mori_noop.argtypes = [vp, vp]
+        L.mori_eviction_order_noalloc.argtypes = [vp, i32, i64, vp, i32, vp, vp, vp, vp, C.POINTER(C.c_char_p)]
         L.mori_path.argtypes = [vp, i32]
         L.mori_copy_kernel.argtypes = [vp]
         L.mori_last_error.argtypes = [vp]
@@ -232,6 +233,23 @@ class Mori:
             self._h, _stream_handle(stream), int(which_tier), int(page_owner.numel()), _ptr(page_owner),
             int(program_tier.numel()), _ptr(program_tier), _ptr(last_access), _ptr(victims),
             _ptr(n_resident)))
+
+    NOALLOC_MAX_PAGES = 65536
+
+    @staticmethod
+    def mori_eviction_order_noalloc(which_tier, page_owner, program_tier, last_access, victims, n_resident,
+                                    stream=None):
+        """The typed eviction order with NO allocation on any call and no context: the sort scratch
+        is a 1 MiB static device array (include/mori.h).  At most ``NOALLOC_MAX_PAGES`` pages; calls
+        that overlap on the GPU race on the shared scratch.  Same tensors as ``mori_eviction_order``."""
+        why = C.c_char_p()
+        rc = load().mori_eviction_order_noalloc(
+            _stream_handle(stream), int(which_tier), int(page_owner.numel()), _ptr(page_owner),
+            int(program_tier.numel()), _ptr(program_tier), _ptr(last_access), _ptr(victims), _ptr(n_resident),
+            C.byref(why))
+        if rc != OK:
+            raise MoriError(rc, (why.value or b"").decode())
+        return rc
 
     # -- NEXT-2: Eq. (1) on the device -------------------------------------------------------
     def mori_idleness_update(self, prog, kind, reasoning, acting, stream=None):

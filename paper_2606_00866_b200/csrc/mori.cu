@@ -391,7 +391,110 @@ cudaError_t launch_sticky(int grid, size_t smem, cudaStream_t s, int n, const fl
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------------
+// mori_eviction_order_noalloc: the sort scratch of the one-launch eviction order as a file-scope
+// array, so that the entry point never allocates.  2 buffers of MORI_NOALLOC_MAX_PAGES 64-bit
+// items = 1 MiB, held by every GPU that loads the library until the process exits.  In HOST code
+// this name is a stand-in, not a device address: the address comes from cudaGetSymbolAddress, once
+// per device with that device current (noalloc_setup below).
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned long long g_noalloc_evict_scratch[2 * MORI_NOALLOC_MAX_PAGES];
+
+namespace {
+constexpr int kNoallocMaxDevices = 64;
+struct NoallocDev { bool ready = false; unsigned long long* scratch = nullptr; int cluster = 8; };
+NoallocDev g_noalloc_dev[kNoallocMaxDevices];
+std::mutex g_noalloc_mu;
+
+// Once per device, with that device current.  No allocation: a symbol lookup, a function attribute
+// and an occupancy query.  -> static error string, or nullptr when the device is ready.
+const char* noalloc_setup(int dev) {
+  NoallocDev& d = g_noalloc_dev[dev];
+  if (d.ready) return nullptr;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { cudaGetLastError(); return "cudaGetDeviceProperties failed"; }
+  if (prop.major != 10) return "libmori is built for sm_100a (B200) only";
+  unsigned long long* ptr = nullptr;
+  if (cudaGetSymbolAddress((void**)&ptr, g_noalloc_evict_scratch) != cudaSuccess || ptr == nullptr) {
+    cudaGetLastError();
+    return "cudaGetSymbolAddress(g_noalloc_evict_scratch) failed";
+  }
+  // cluster of 16 CTAs where the device can co-schedule that non-portable size, else the portable 8
+  bool ok = true;
+  const void* ks[] = {(const void*)mori::evict_order_cluster_kernel<2>, (const void*)mori::evict_order_cluster_kernel<4>,
+                      (const void*)mori::evict_order_cluster_kernel<8>, (const void*)mori::evict_order_cluster_kernel<16>};
+  for (const void* k : ks) ok = ok && cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+  if (ok) {
+    cudaLaunchConfig_t lc{};
+    lc.gridDim = dim3(16); lc.blockDim = dim3(1024);
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 16; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.attrs = at; lc.numAttrs = 1;
+    int n_clusters = 0;
+    ok = cudaOccupancyMaxActiveClusters(&n_clusters, mori::evict_order_cluster_kernel<8>, &lc) == cudaSuccess && n_clusters >= 1;
+  }
+  cudaGetLastError();
+  d.cluster = ok ? 16 : 8;
+  d.scratch = ptr;
+  d.ready = true;
+  return nullptr;
+}
+}  // namespace
+
 extern "C" {
+
+int mori_eviction_order_noalloc(void* stream, int32_t which_tier, int64_t n_pages, const int32_t* page_owner,
+                                int32_t n_programs, const uint8_t* program_tier, const uint32_t* last_access,
+                                int32_t* victims, int32_t* n_resident, const char** why) {
+  const char* dummy;
+  const char*& msg = why ? *why : dummy;
+  msg = "";
+  if (which_tier != MORI_TIER_GPU && which_tier != MORI_TIER_CPU) { msg = "which_tier must be MORI_TIER_GPU or MORI_TIER_CPU"; return MORI_ERR_INVALID_ARG; }
+  if (n_pages < 0 || n_programs < 0) { msg = "n_pages / n_programs is negative"; return MORI_ERR_INVALID_ARG; }
+  if (n_pages > MORI_NOALLOC_MAX_PAGES) {
+    msg = "n_pages exceeds MORI_NOALLOC_MAX_PAGES (65536): the static scratch of this entry point is 1 MiB; "
+          "use mori_eviction_order for larger pools";
+    return MORI_ERR_CAPACITY;
+  }
+  if (n_pages > 0 && (!page_owner || !last_access || !victims || !n_resident || (n_programs > 0 && !program_tier))) {
+    msg = "NULL array"; return MORI_ERR_INVALID_ARG;
+  }
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); msg = "no current CUDA device"; return MORI_ERR_CUDA; }
+  if (dev < 0 || dev >= kNoallocMaxDevices) { msg = "device ordinal beyond 63"; return MORI_ERR_UNSUPPORTED; }
+  {
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (const char* e = noalloc_setup(dev)) { msg = e; return e[0] == 'l' ? MORI_ERR_UNSUPPORTED : MORI_ERR_CUDA; }
+  }
+  const NoallocDev& d = g_noalloc_dev[dev];
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (n_pages == 0) {
+    if (n_resident && cudaMemsetAsync(n_resident, 0, sizeof(int32_t), s) != cudaSuccess) {
+      cudaGetLastError(); msg = "cudaMemsetAsync(n_resident) failed"; return MORI_ERR_CUDA;
+    }
+    return MORI_OK;
+  }
+  mori::EvictArgs a{n_pages, n_programs, which_tier == MORI_TIER_GPU ? 0 : 1, 0, page_owner, program_tier, last_access};
+  const int csize = d.cluster;
+  const long long seg = ((n_pages + csize - 1) / csize + 1023) / 1024 * 1024;
+  const int rounds = (int)(seg / 1024);                              // <= 8 at the maximum with a cluster of 8
+  uint64_t* b0 = reinterpret_cast<uint64_t*>(d.scratch);             // the DEVICE address, not the symbol
+  uint64_t* b1 = b0 + MORI_NOALLOC_MAX_PAGES;
+  cudaLaunchConfig_t lc{};
+  lc.gridDim = dim3(csize); lc.blockDim = dim3(1024); lc.dynamicSmemBytes = 0; lc.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = csize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  lc.attrs = at; lc.numAttrs = 1;
+  cudaError_t le;
+  if (rounds <= 2) le = cudaLaunchKernelEx(&lc, mori::evict_order_cluster_kernel<2>, a, b0, b1, victims, n_resident);
+  else if (rounds <= 4) le = cudaLaunchKernelEx(&lc, mori::evict_order_cluster_kernel<4>, a, b0, b1, victims, n_resident);
+  else if (rounds <= 8) le = cudaLaunchKernelEx(&lc, mori::evict_order_cluster_kernel<8>, a, b0, b1, victims, n_resident);
+  else le = cudaLaunchKernelEx(&lc, mori::evict_order_cluster_kernel<16>, a, b0, b1, victims, n_resident);
+  if (le != cudaSuccess) { cudaGetLastError(); msg = "launch of the eviction-order kernel failed"; return MORI_ERR_CUDA; }
+  return MORI_OK;
+}
 
 const char* mori_last_error(const mori_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 
