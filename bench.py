@@ -761,6 +761,7 @@ def run_ours(args):
     with_oracle = world == 1 and not args.no_cpu_baseline
     rp = rank_partition_leg(with_oracle=with_oracle) if rank == 0 else None
     evl = eviction_leg(with_oracle=with_oracle) if rank == 0 else None
+    sml = small_move_leg() if rank == 0 else None
     cpu = None
     if rank == 0 and with_oracle:
         cpu = cpu_baseline(args.config, f_busy=args.f_busy)
@@ -812,6 +813,7 @@ def run_ours(args):
             "gather_scatter": gs,
             "rank_partition": rp,
             "eviction_order": evl,
+            "small_move": sml,
             "waiting_queue_bfd": waiting_queue,
             "cpu_baseline": cpu,
         }
@@ -1009,6 +1011,78 @@ def three_tier_leg(args):
                       "epochs": {"timed": epochs, "moved_GiB_by_pair": {k: v / GIB for k, v in sorted(moved.items())},
                                  "GBps_all_pairs_host_timed": tot / t_move / 1e9 if t_move > 0 else 0.0,
                                  "note": "host wall-clock around TierRunner.execute (three contexts, joins included)"}}))
+
+
+def small_move_leg(reps=60):
+    """The one-launch path of a small move, warm: cfg 1's geometry (16 KiB pages) and the 17-page
+    (272 KiB) demotion its trace produces, repeated through the C ABI with the same bracketing an
+    epoch's transfer region has (event, mori_after_stream, mori_demote / mori_promote,
+    mori_stream_wait, event) -- median device microseconds -- beside a plain pinned memcpy of the
+    same bytes, alone between two events and joined through a side stream the same way.  cfg 1's own
+    epochs contain this move exactly once, cold (no move in its warm-up epochs)."""
+    import torch
+    from paper_2606_00866_b200 import binding
+    L, H, D, T, P, S = 2, 2, 64, 16, 64, 256
+    page = L * 2 * H * T * D * 2
+    pool = torch.zeros(P * page, dtype=torch.uint8, device="cuda")
+    arena = torch.zeros(S * page, dtype=torch.uint8).pin_memory()
+    m = binding.Mori(L, H, D, T, pool, arena)
+    cur = torch.cuda.current_stream()
+    rng = np.random.default_rng(SEED)
+    n = 17
+    g = np.ascontiguousarray(rng.permutation(P)[:n], dtype=np.int32)
+    h = np.arange(n, dtype=np.int32)
+    lib, hc = m._lib, m._h
+
+    def region(fn):
+        ts = []
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(cur)
+            m.mori_after_stream(binding.BOTH, cur)
+            fn()
+            m.mori_stream_wait(cur, binding.BOTH)
+            e1.record(cur)
+            m.mori_sync(binding.BOTH)
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        return float(np.median(ts[5:]))
+    dem_us = region(lambda: lib.mori_demote(hc, n, g.ctypes.data, h.ctypes.data, 0, None))
+    pro_us = region(lambda: lib.mori_promote(hc, n, h.ctypes.data, g.ctypes.data, 0, 0, None))
+    nbytes = n * page
+    d_buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    h_buf = arena[:nbytes]
+    side = torch.cuda.Stream()
+
+    def memcpy(joined, d2h):
+        ts = []
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(cur)
+            if joined:
+                side.wait_event(e0)
+                with torch.cuda.stream(side):
+                    (h_buf.copy_(d_buf, non_blocking=True) if d2h else d_buf.copy_(h_buf, non_blocking=True))
+                cur.wait_stream(side)
+            else:
+                (h_buf.copy_(d_buf, non_blocking=True) if d2h else d_buf.copy_(h_buf, non_blocking=True))
+            e1.record(cur)
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        return float(np.median(ts[5:]))
+    out = {"pages": n, "bytes": nbytes, "demote_us": dem_us, "promote_us": pro_us,
+           "memcpy_d2h_bare_us": memcpy(False, True), "memcpy_d2h_joined_us": memcpy(True, True),
+           "memcpy_h2d_bare_us": memcpy(False, False), "memcpy_h2d_joined_us": memcpy(True, False)}
+    out["demote_GBps"] = nbytes / dem_us / 1e3
+    out["promote_GBps"] = nbytes / pro_us / 1e3
+    out["demote_frac_of_joined_memcpy"] = out["memcpy_d2h_joined_us"] / dem_us
+    out["promote_frac_of_joined_memcpy"] = out["memcpy_h2d_joined_us"] / pro_us
+    out["demote_frac_of_bare_memcpy"] = out["memcpy_d2h_bare_us"] / dem_us
+    out["promote_frac_of_bare_memcpy"] = out["memcpy_h2d_bare_us"] / pro_us
+    m.close()
+    return out
 
 
 def launch_floor(m, cur, reps=200):

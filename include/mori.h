@@ -199,6 +199,8 @@ int mori_sync(mori_ctx* ctx, int32_t which);
 /* Device-side ordering against a caller stream (cudaStream_t), no host blocking:
  *   mori_after_stream   work enqueued later in direction(s) `which` starts after everything
  *                       now in `stream` (e.g. the inference step that last touched the pages);
+ *                       costs one event record: each library stream waits on it only when it
+ *                       next gets work, so a direction that stays idle is never touched;
  *   mori_stream_wait    work enqueued later in `stream` starts after everything now enqueued
  *                       in direction(s) `which`. */
 int mori_after_stream(mori_ctx* ctx, int32_t which, void* stream);

@@ -66,6 +66,7 @@ struct Direction {
   cudaEvent_t kern_done[2] = {nullptr, nullptr}, copy_done[2] = {nullptr, nullptr};
   int buf = 0;
   bool copy_busy = false;                        // DMAs enqueued on `copy` since the last join
+  bool kern_busy = false;                        // anything enqueued on `kern` since the last join
   // index ring: pinned host (written by the CPU, read by the upload kernel) + device copy
   int32_t* idx_host = nullptr; int32_t* idx_host_dev = nullptr; int32_t* idx_dev = nullptr;
   long long idx_cap = 0, idx_used = 0;
@@ -109,6 +110,12 @@ struct mori_ctx {
   int32_t* sticky_order = nullptr;               // [kRankTickets][max_programs] positions scratch
   Direction dir[2];                              // 0 demote, 1 promote
   std::vector<cudaEvent_t> free_events;
+  // mori_after_stream is lazy: the caller-stream event is kept here and each of the four library
+  // streams waits on it only when it next gets work (an epoch that only demotes a few pages never
+  // touches the promote streams or the DMA streams).  streams_left: bit 2*dir = kernel stream,
+  // bit 2*dir+1 = DMA stream.  Entries whose event has completed are dropped at mori_sync.
+  struct PendingAfter { cudaEvent_t ev; int streams_left; };
+  std::vector<PendingAfter> pending_after;
   std::vector<cudaEvent_t> free_timing_events;   // profiling spans reuse their events (creating one costs microseconds)
   bool profiling = false;
   bool timeline = false; cudaEvent_t prof_base = nullptr;   // mori_profile(ctx, 2)
@@ -744,6 +751,7 @@ int mori_destroy(mori_ctx* c) {
     if (d.kern) cudaStreamDestroy(d.kern);
     if (d.copy) cudaStreamDestroy(d.copy);
   }
+  for (auto& p : c->pending_after) cudaEventDestroy(p.ev);
   for (auto ev : c->free_events) cudaEventDestroy(ev);
   for (auto ev : c->free_timing_events) cudaEventDestroy(ev);
   if (c->prof_base) cudaEventDestroy(c->prof_base);
@@ -1063,6 +1071,36 @@ int mori_scatter_pages(mori_ctx* c, void* stream, int64_t n_pages, const int32_t
   return MORI_OK;
 }
 
+// Enqueues the waits that earlier mori_after_stream calls owe the streams of direction `di` that
+// are about to get work, and recycles the events no stream needs any more.
+static int consume_pending_after(mori_ctx* c, int di, bool kern, bool copy) {
+  if (c->pending_after.empty()) return MORI_OK;
+  Direction& d = c->dir[di];
+  const int bit_k = 1 << (2 * di), bit_c = 1 << (2 * di + 1);
+  for (auto& p : c->pending_after) {
+    if (kern && (p.streams_left & bit_k)) { CK(c, cudaStreamWaitEvent(d.kern, p.ev, 0)); p.streams_left &= ~bit_k; }
+    if (copy && (p.streams_left & bit_c)) { CK(c, cudaStreamWaitEvent(d.copy, p.ev, 0)); p.streams_left &= ~bit_c; }
+  }
+  size_t keep = 0;
+  for (auto& p : c->pending_after) {
+    if (p.streams_left) c->pending_after[keep++] = p;
+    else c->free_events.push_back(p.ev);
+  }
+  c->pending_after.resize(keep);
+  return MORI_OK;
+}
+
+// Drops the pending entries whose caller-stream event has already completed: the dependency holds.
+static void prune_pending_after(mori_ctx* c) {
+  size_t keep = 0;
+  for (auto& p : c->pending_after) {
+    if (cudaEventQuery(p.ev) == cudaSuccess) c->free_events.push_back(p.ev);
+    else c->pending_after[keep++] = p;
+  }
+  cudaGetLastError();                              // cudaErrorNotReady is not an error
+  c->pending_after.resize(keep);
+}
+
 // Shared body of mori_demote (dir 0) and mori_promote (dir 1).
 //   wait_pool   ticket of the OTHER direction after which this call may touch the POOL
 //   wait_arena  ticket of the OTHER direction after which this call may touch the ARENA
@@ -1102,6 +1140,8 @@ static int migrate(mori_ctx* c, int di, long long total, const int32_t* gpu_page
     path = (small || total * pb / runs < kAutoMinRunBytes) ? MORI_PATH_ZEROCOPY : MORI_PATH_STAGED;
   }
 
+  if (int rc = consume_pending_after(c, di, true, path == MORI_PATH_STAGED)) return rc;
+  d.kern_busy = true;
   // one stream carries the whole call on every path but STAGED: it waits for both tickets
   auto wait_both = [&](cudaStream_t s) -> int {
     if (int rc = wait_ticket(c, other, wait_pool, s)) return rc;
@@ -1252,23 +1292,28 @@ int mori_sync(mori_ctx* c, int32_t which) {
     }
     d.idx_used = 0;
     d.copy_busy = false;
+    d.kern_busy = false;
     prof_collect(c, d);
   }
+  prune_pending_after(c);
   return c->sticky;
 }
 
 int mori_after_stream(mori_ctx* c, int32_t which, void* stream) {
   if (!c || which < 1 || which > 3) return MORI_ERR_INVALID_ARG;
   if (c->sticky) return c->sticky;
+  if (c->pending_after.size() >= 16) {             // a caller that never joins: settle the old ones now
+    prune_pending_after(c);
+    for (int i = 0; i < 2 && !c->pending_after.empty(); ++i)
+      if (int rc = consume_pending_after(c, i, true, true)) return rc;
+  }
   cudaEvent_t ev = get_event(c, false);
   if (!ev) return c->sticky;
   CK(c, cudaEventRecord(ev, static_cast<cudaStream_t>(stream)));
+  int left = 0;
   for (int i = 0; i < 2; ++i)
-    if (which & (1 << i)) {
-      CK(c, cudaStreamWaitEvent(c->dir[i].kern, ev, 0));
-      CK(c, cudaStreamWaitEvent(c->dir[i].copy, ev, 0));
-    }
-  c->free_events.push_back(ev);
+    if (which & (1 << i)) left |= 3 << (2 * i);    // the direction's kernel and DMA streams
+  c->pending_after.push_back({ev, left});          // waited on when those streams next get work
   return MORI_OK;
 }
 
@@ -1279,6 +1324,7 @@ int mori_stream_wait(mori_ctx* c, void* stream, int32_t which) {
     if (which & (1 << i))
       for (cudaStream_t s : {c->dir[i].kern, c->dir[i].copy}) {
         if (s == c->dir[i].copy && !c->dir[i].copy_busy) continue;   // nothing enqueued there since the last join
+        if (s == c->dir[i].kern && !c->dir[i].kern_busy) continue;
         cudaEvent_t ev = get_event(c, false);
         if (!ev) return c->sticky;
         CK(c, cudaEventRecord(ev, s));

@@ -225,3 +225,48 @@ def test_profile_timeline_and_launch_floor(mori):
     oracle.promote(L, chunk, pool_m, arena_m, h, (g + 120).astype(np.int32))
     assert np.array_equal(arena.numpy(), arena_m) and np.array_equal(pool.cpu().numpy(), pool_m)
     m.close()
+
+
+def test_after_stream_is_lazy_but_still_orders_every_library_stream(mori):
+    """mori_after_stream only records an event; a library stream waits on it when it next gets work.
+    A side stream sleeps, then rewrites the whole pool and the whole arena.  A small demotion (one
+    launch on the kernel stream) and a large STAGED promotion (whose first operations are DMAs on the
+    DMA stream) issued right after mori_after_stream must both see the NEW bytes."""
+    L, H, D, T, P, S = 2, 8, 128, 16, 700, 700                   # 128 KiB pages
+    m, pool, arena, pool_m, arena_m, chunk = _ctx(mori, L, H, D, T, P, S, path=0, kernel=0, seed=11)
+    g = torch.Generator(device="cpu").manual_seed(12)
+    new_pool = torch.randint(0, 256, (pool.numel(),), dtype=torch.uint8, generator=g)
+    new_arena = torch.randint(0, 256, (arena.numel(),), dtype=torch.uint8, generator=g)
+    d_new_pool, d_new_arena = new_pool.cuda(), new_arena.cuda()
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    for rep in range(2):                                          # the second round reuses a recycled event
+        with torch.cuda.stream(side):
+            torch.cuda._sleep(40_000_000)                         # ~20 ms: the library would win any race
+            pool.copy_(d_new_pool)
+            arena.copy_(d_new_arena, non_blocking=True)
+        m.mori_after_stream(mori.BOTH, side)
+        g_small = np.array([3, 699, 42, 7], np.int32)
+        h_small = np.array([650, 2, 651, 699], np.int32)
+        g_big = (100 + np.arange(500)).astype(np.int32)
+        h_big = (100 + np.arange(500)).astype(np.int32)            # one run of 62.5 MiB -> STAGED
+        l0 = m.mori_launch_count()
+        m.mori_demote(g_small, h_small)
+        assert m.mori_launch_count() - l0 == 1                     # the one-launch path
+        m.mori_promote(h_big, g_big[::-1].copy())
+        m.mori_sync(mori.BOTH)
+        side.synchronize()
+        pool_m, arena_m = new_pool.numpy().copy(), new_arena.numpy().copy()
+        oracle.demote(L, chunk, pool_m, arena_m, g_small, h_small)
+        oracle.promote(L, chunk, pool_m, arena_m, h_big, g_big[::-1].copy())
+        assert np.array_equal(arena.numpy(), arena_m), (rep, "the demotion did not wait for the side stream")
+        assert np.array_equal(pool.cpu().numpy(), pool_m), (rep, "the promotion's DMAs did not wait for the side stream")
+        # restore different contents for the next round, so that stale data would show
+        d_new_pool, d_new_arena = d_new_pool.flip(0).contiguous(), d_new_arena.flip(0).contiguous()
+        new_pool, new_arena = new_pool.flip(0).contiguous(), new_arena.flip(0).contiguous()
+    # many after_stream calls with no work and no join in between must not grow without bound
+    for _ in range(100):
+        m.mori_after_stream(mori.BOTH, side)
+    m.mori_demote(np.array([1], np.int32), np.array([1], np.int32))
+    m.mori_sync(mori.BOTH)
+    m.close()
